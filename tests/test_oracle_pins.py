@@ -1,0 +1,383 @@
+"""Pins P1-P13: the CPU oracle checked against what the paper and the mathematics fix --
+closed forms, brute force in numpy float64 on tiny inputs, invariants, library routines.  CPU only."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle as orc
+import saf3r_synth as sy
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def rand_bits(rng, shape, scale=1.0):
+    return sy.f32_to_bf16_bits(rng.standard_normal(shape).astype(np.float32) * np.float32(scale))
+
+
+def ocfg(d):
+    return orc.make_cfg(**d)
+
+
+def lists_to_mask(row_ptr, col_idx, N, B):
+    NB = (N + B - 1) // B
+    m = np.zeros((N, N), bool)
+    for I in range(NB):
+        for J in col_idx[row_ptr[I]:row_ptr[I + 1]]:
+            m[I * B:(I + 1) * B, J * B:(J + 1) * B] = True
+    return m
+
+
+def brute_masked_attention(q, k, v, mask):
+    """softmax(QK^T/sqrt(D) restricted to mask) V in float64 with a dense matrix (plain definition)."""
+    qf, kf, vf = (sy.bf16_bits_to_f32(x).astype(np.float64) for x in (q, k, v))
+    z = qf @ kf.T / np.sqrt(qf.shape[1])
+    z = np.where(mask, z, -np.inf)
+    m = z.max(axis=1, keepdims=True)
+    m = np.where(np.isfinite(m), m, 0.0)
+    w = np.exp(z - m)
+    l = w.sum(axis=1, keepdims=True)
+    out = np.where(l > 0, (w @ vf) / np.where(l > 0, l, 1.0), 0.0)
+    with np.errstate(divide="ignore"):
+        lse = (m + np.log(l))[:, 0]
+    return out, lse
+
+
+ALL_CFGS_TINY = [
+    sy.cfg(type=sy.HEAD_DENSE),
+    sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=3, offset=1),
+    sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=0, keep_blocks=5),
+    sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_ANCHOR, anchor_frame=1),
+    sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_FRAME_LOCAL),
+    sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_POSITION_BAND, band_radius=2),
+    sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=4),
+    sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=3),
+    sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=3, score_mode=sy.SCORE_COSINE),
+    sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=1),
+    sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=2, score_mode=sy.SCORE_COSINE),
+]
+
+
+# ---------------------------------------------------------------- P1
+@pytest.mark.parametrize("N,B,D", [(90, 8, 8), (1044, 64, 64)])
+def test_p1_keep_all_lists_reproduce_dense(N, B, D):
+    rng = np.random.default_rng(1)
+    q, k, v = (rand_bits(rng, (N, D)) for _ in range(3))
+    NB = (N + B - 1) // B
+    row_ptr = np.arange(NB + 1, dtype=np.int64) * NB
+    col = np.tile(np.arange(NB, dtype=np.int32), NB)
+    rows = slice(0, N) if N < 200 else slice(0, 128)
+    qb = None if N < 200 else np.array([0, 1], np.int64)
+    o1, l1 = orc.attn_lists(q, k, v, B, row_ptr, col, qb)
+    o2, l2 = orc.attn_dense(q, k, v, rows.start, rows.stop)
+    assert np.abs(o1[rows] - o2[rows]).max() <= 1e-6
+    assert np.abs(l1[rows] - l2[rows]).max() <= 1e-5
+
+
+# ---------------------------------------------------------------- P2
+@pytest.mark.parametrize("ci", range(len(ALL_CFGS_TINY)))
+@pytest.mark.parametrize("S,T,B,D", [(4, 23, 8, 8), (3, 32, 4, 8)])
+def test_p2_bruteforce_tiny(ci, S, T, B, D):
+    rng = np.random.default_rng(100 + ci)
+    N = S * T
+    q, k, v = rand_bits(rng, (N, D), 1.5), rand_bits(rng, (N, D), 1.5), rand_bits(rng, (N, D))
+    hl = orc.select_head(q, k, S, T, B, ocfg(ALL_CFGS_TINY[ci]))
+    NB = (N + B - 1) // B
+    for I in range(NB):
+        row = hl.col_idx[hl.row_ptr[I]:hl.row_ptr[I + 1]]
+        assert len(row) >= 1 and np.all(np.diff(row) > 0) and row[0] >= 0 and row[-1] < NB
+    out, lse = orc.attn_lists(q, k, v, B, hl.row_ptr, hl.col_idx)
+    ref, ref_lse = brute_masked_attention(q, k, v, lists_to_mask(hl.row_ptr, hl.col_idx, N, B))
+    assert np.abs(out - ref).max() <= 2e-6
+    assert np.abs(lse - ref_lse).max() <= 2e-6
+
+
+def test_p2_empty_list_convention():
+    rng = np.random.default_rng(5)
+    N, B, D = 40, 8, 8
+    q, k, v = (rand_bits(rng, (N, D)) for _ in range(3))
+    row_ptr = np.array([0, 0, 2, 2, 3, 3], np.int64)
+    col = np.array([1, 4, 0], np.int32)
+    out, lse = orc.attn_lists(q, k, v, B, row_ptr, col)
+    for I in (0, 2, 4):
+        assert np.all(out[I * B:(I + 1) * B] == 0) and np.all(np.isneginf(lse[I * B:(I + 1) * B]))
+    ref, _ = brute_masked_attention(q, k, v, lists_to_mask(row_ptr, col, N, B))
+    assert np.abs(out - ref).max() <= 2e-6
+
+
+# ---------------------------------------------------------------- P3
+def test_p3_rows_sum_to_one_and_lse_bound():
+    rng = np.random.default_rng(3)
+    S, T, B, D = 4, 23, 8, 8
+    N = S * T
+    q, k = rand_bits(rng, (N, D), 2.0), rand_bits(rng, (N, D), 2.0)
+    ones = sy.f32_to_bf16_bits(np.ones((N, D), np.float32))
+    _, lse_dense = orc.attn_dense(q, k, ones)
+    for c in ALL_CFGS_TINY:
+        hl = orc.select_head(q, k, S, T, B, ocfg(c))
+        out, lse = orc.attn_lists(q, k, ones, B, hl.row_ptr, hl.col_idx)
+        assert np.abs(out - 1.0).max() <= 1e-6          # sum_j softmax_ij * 1 = 1
+        assert np.all(lse <= lse_dense + 1e-6)          # a subset of the keys cannot have a larger log-sum-exp
+
+
+# ---------------------------------------------------------------- P4
+def test_p4_uniform_stride_closed_form():
+    rng = np.random.default_rng(4)
+    S, T, B, D = 5, 29, 4, 8
+    N = S * T
+    NB = (N + B - 1) // B
+    q, k = rand_bits(rng, (N, D)), rand_bits(rng, (N, D))
+    for s, o in [(1, 0), (2, 0), (3, 2), (7, 6), (NB, 0), (NB + 5, 3)]:
+        hl = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=s, offset=o)))
+        expect = np.arange(o, NB, s, dtype=np.int32)
+        assert len(expect) == -(-(NB - o) // s)                     # ceil((NB - o)/s), "fixed stride"
+        for I in range(NB):
+            assert np.array_equal(hl.col_idx[hl.row_ptr[I]:hl.row_ptr[I + 1]], expect)
+    for n in (1, 2, 5, NB // 2, NB):
+        hl = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=0, keep_blocks=n)))
+        row = hl.col_idx[hl.row_ptr[0]:hl.row_ptr[1]]
+        assert len(row) == n and row[0] == 0 and np.all(np.diff(row) > 0)
+        assert np.array_equal(hl.col_idx, np.tile(row, NB))
+    # keep_blocks form equals the stride set when s | NB
+    S2, T2 = 4, 24          # N = 96, B = 4 -> NB = 24
+    q2, k2 = rand_bits(rng, (96, D)), rand_bits(rng, (96, D))
+    for s in (2, 3, 4, 6, 8):
+        a = orc.select_head(q2, k2, S2, T2, 4, ocfg(sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=s)))
+        b = orc.select_head(q2, k2, S2, T2, 4, ocfg(sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=0, keep_blocks=24 // s)))
+        assert np.array_equal(a.col_idx, b.col_idx)
+
+
+# ---------------------------------------------------------------- P5
+def test_p5_probe_equals_column_mean_of_full_scores():
+    """ranking keys by the column-wise average of S = QK^T/sqrt(D) equals ranking by qbar K^T/sqrt(D);
+    block-lifted: the probe of block J is the mean of S over all queries and the keys of J."""
+    rng = np.random.default_rng(6)
+    S, T, B, D = 4, 23, 8, 8
+    N = S * T
+    NB = (N + B - 1) // B
+    q, k = rand_bits(rng, (N, D), 1.3), rand_bits(rng, (N, D), 1.3)
+    qf, kf = sy.bf16_bits_to_f32(q).astype(np.float64), sy.bf16_bits_to_f32(k).astype(np.float64)
+    Sfull = qf @ kf.T / np.sqrt(D)
+    colmean = Sfull.mean(axis=0)
+    blockmean = np.array([colmean[J * B:(J + 1) * B].mean() for J in range(NB)])
+    n = 4
+    hl = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=n)), want_scores=True)
+    assert np.abs(hl.scores[0] - blockmean).max() <= 1e-6
+    expect = np.sort(np.argsort(-blockmean, kind="stable")[:n])
+    for I in range(NB):
+        assert np.array_equal(hl.col_idx[hl.row_ptr[I]:hl.row_ptr[I + 1]], expect)
+    # token level (B = 1): exactly the paper's statement
+    hl1 = orc.select_head(q, k, S, T, 1, ocfg(sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=7)), want_scores=True)
+    assert np.abs(hl1.scores[0] - colmean).max() <= 1e-6
+    assert np.array_equal(hl1.col_idx[:7], np.sort(np.argsort(-colmean, kind="stable")[:7]))
+
+
+# ---------------------------------------------------------------- P6
+def test_p6_per_frame_topk_counts_match_paper_fractions():
+    gold = {}
+    for line in open(os.path.join(GOLD, "paper_key_fractions.txt")):
+        if line.strip() and not line.startswith("#"):
+            name, val = line.split()
+            gold[name] = float(val)
+    # token granularity (B = 1) is the paper's own setting: K keys from each frame's T tokens -> K/T of all keys.
+    rng = np.random.default_rng(7)
+    S, T, D = 3, 40, 8
+    N = S * T
+    q, k = rand_bits(rng, (N, D)), rand_bits(rng, (N, D))
+    for K in (2, 4):
+        hl = orc.select_head(q, k, S, T, 1, ocfg(sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=K)))
+        assert np.all(np.diff(hl.row_ptr) == S * K)
+        frac = (S * K) / N
+        assert abs(frac - K / T) < 1e-12
+    # the paper's printed numbers: K/T at T = 1024 tokens per frame gives 0.2 % / 0.4 %, and (1/32)/(2/T) = 16
+    T_paper = 1024
+    assert round(100 * 2 / T_paper, 1) == gold["topk_k2_fraction_percent"]
+    assert round(100 * 4 / T_paper, 1) == gold["topk_k4_fraction_percent"]
+    assert (1 / 32) / (2 / T_paper) == gold["stride32_vs_k2_sparsity_ratio"]
+    # block granularity: S * k_f blocks per q-block when k_f <= min_g |C_g|
+    S, T, B = 4, 23, 4
+    N = S * T
+    q, k = rand_bits(rng, (N, D)), rand_bits(rng, (N, D))
+    for kf in (1, 2, 3):
+        hl = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=kf)), want_scores=True)
+        assert np.all(np.diff(hl.row_ptr) == S * kf)
+        NB = (N + B - 1) // B
+        frame_of_block = (np.arange(NB) * B) // T
+        for I in range(NB):
+            row = hl.col_idx[hl.row_ptr[I]:hl.row_ptr[I + 1]]
+            for g in range(S):
+                kept = [J for J in row if frame_of_block[J] == g]
+                rest = [J for J in range(NB) if frame_of_block[J] == g and J not in kept]
+                assert len(kept) == kf
+                assert min(hl.scores[I][kept]) >= max(hl.scores[I][rest])     # property: kept dominate the rest of the frame
+
+
+# ---------------------------------------------------------------- P7
+@pytest.mark.parametrize("cosine", [False, True])
+def test_p7_pooled_score_is_mean_of_token_pair_scores(cosine):
+    """PAPER.md:L126 "block-level similarities averaged over multiple tokens": s[I][J] = mean over token pairs."""
+    rng = np.random.default_rng(8)
+    S, T, B, D = 3, 23, 8, 8          # N = 69, tail block of 5 tokens
+    N = S * T
+    NB = (N + B - 1) // B
+    q, k = rand_bits(rng, (N, D), 1.2), rand_bits(rng, (N, D), 1.2)
+    qf, kf = sy.bf16_bits_to_f32(q).astype(np.float64), sy.bf16_bits_to_f32(k).astype(np.float64)
+    if cosine:
+        tok = (qf / np.linalg.norm(qf, axis=1, keepdims=True)) @ (kf / np.linalg.norm(kf, axis=1, keepdims=True)).T
+    else:
+        tok = qf @ kf.T / np.sqrt(D)
+    expect = np.array([[tok[I * B:(I + 1) * B, J * B:(J + 1) * B].mean() for J in range(NB)] for I in range(NB)])
+    c = sy.cfg(type=sy.HEAD_BLOCK_TOPK, keep_blocks=2, score_mode=sy.SCORE_COSINE if cosine else sy.SCORE_DOT)
+    hl = orc.select_head(q, k, S, T, B, ocfg(c), want_scores=True)
+    assert np.abs(hl.scores - expect).max() <= 1e-6
+    # and the pieces: pooled vectors and a single score row
+    qt, kt = orc.pool(q, B, cosine), orc.pool(k, B, cosine)
+    row = orc.score_row(qt[2], kt, 1.0 if cosine else 1.0 / np.sqrt(D))
+    assert np.abs(row - expect[2]).max() <= 1e-6
+    assert np.abs(orc.mean_query(q) - qf.mean(axis=0)).max() <= 1e-6
+
+
+# ---------------------------------------------------------------- P8
+def test_p8_static_closed_forms():
+    rng = np.random.default_rng(9)
+    D = 8
+    for S, T, B in [(4, 23, 8), (5, 261, 64), (3, 1374, 128)]:
+        N = S * T
+        NB = (N + B - 1) // B
+        q = k = rand_bits(rng, (N, D))
+        for a in range(S):
+            hl = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_ANCHOR, anchor_frame=a)))
+            lo, hi = (a * T) // B, ((a + 1) * T - 1) // B
+            assert np.all(np.diff(hl.row_ptr) == hi - lo + 1)
+            assert np.array_equal(hl.col_idx[:hi - lo + 1], np.arange(lo, hi + 1))
+            # every token of the anchor frame is covered and no block lies fully outside the frame
+            assert lo * B <= a * T and (hi + 1) * B >= min(N, (a + 1) * T)
+        # frame-local: a q-block's list covers exactly the frames of its tokens
+        hl = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_FRAME_LOCAL)))
+        tok_frame = np.arange(N) // T
+        for I in range(NB):
+            row = hl.col_idx[hl.row_ptr[I]:hl.row_ptr[I + 1]]
+            frames = set(tok_frame[I * B:(I + 1) * B])
+            need = {j // B for j in range(N) if tok_frame[j] in frames}
+            assert set(row) == need
+        # position band with r >= T is dense
+        hl = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_POSITION_BAND, band_radius=T)))
+        assert np.all(np.diff(hl.row_ptr) == NB)
+    # S = 1: frame-local == dense
+    q = k = rand_bits(rng, (50, D))
+    hl = orc.select_head(q, k, 1, 50, 8, ocfg(sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_FRAME_LOCAL)))
+    assert np.all(np.diff(hl.row_ptr) == 7)
+    # position band r = 0 at token granularity (B = 1): query (f, p) attends key (g, p) for every frame g
+    S, T = 4, 11
+    q = k = rand_bits(rng, (S * T, D))
+    hl = orc.select_head(q, k, S, T, 1, ocfg(sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_POSITION_BAND, band_radius=0)))
+    for i in range(S * T):
+        assert np.array_equal(hl.col_idx[hl.row_ptr[i]:hl.row_ptr[i + 1]], np.arange(S) * T + i % T)
+    hl = orc.select_head(q, k, S, T, 1, ocfg(sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_POSITION_BAND, band_radius=2)))
+    for i in range(S * T):
+        p = i % T
+        exp = sorted(g * T + pp for g in range(S) for pp in range(max(0, p - 2), min(T - 1, p + 2) + 1))
+        assert list(hl.col_idx[hl.row_ptr[i]:hl.row_ptr[i + 1]]) == exp
+
+
+# ---------------------------------------------------------------- P9
+def test_p9_softmax_special_cases():
+    rng = np.random.default_rng(10)
+    N, B, D = 44, 8, 8
+    NB = 6
+    k, v = rand_bits(rng, (N, D)), rand_bits(rng, (N, D))
+    row_ptr = np.arange(NB + 1, dtype=np.int64) * 2
+    col = np.array([0, 5, 1, 2, 0, 3, 2, 4, 1, 5, 3, 4], np.int32)
+    vf = sy.bf16_bits_to_f32(v).astype(np.float64)
+    # Q = 0  =>  o_i = mean of v over A(i)
+    zero = np.zeros((N, D), np.uint16)
+    out, lse = orc.attn_lists(zero, k, v, B, row_ptr, col)
+    for I in range(NB):
+        keys = np.concatenate([np.arange(J * B, min(N, (J + 1) * B)) for J in col[2 * I:2 * I + 2]])
+        assert np.abs(out[I * B:(I + 1) * B] - vf[keys].mean(axis=0)).max() <= 1e-6
+        assert np.abs(lse[I * B:(I + 1) * B] - np.log(len(keys))).max() <= 1e-6
+    # V constant => o = that constant
+    q = rand_bits(rng, (N, D), 3.0)
+    cst = sy.f32_to_bf16_bits(np.full((N, D), 0.375, np.float32))
+    out, _ = orc.attn_lists(q, k, cst, B, row_ptr, col)
+    assert np.abs(out - 0.375).max() <= 1e-6
+    # one dominant key => o_i -> v_j
+    kd = sy.bf16_bits_to_f32(k).copy() * 0.01
+    qd = np.zeros((N, D), np.float32)
+    qd[:, 0] = 40.0
+    kd[13, 0] = 40.0                                         # key 13 (block 1) gets logit 40*40/sqrt(8)
+    out, _ = orc.attn_lists(sy.f32_to_bf16_bits(qd), sy.f32_to_bf16_bits(kd), v, B,
+                            np.arange(NB + 1, dtype=np.int64), np.ones(NB, np.int32))
+    assert np.abs(out - vf[13]).max() <= 1e-6
+    # permuting tokens inside a k-block (K and V together) leaves O unchanged
+    perm = np.arange(N)
+    perm[8:16] = 8 + rng.permutation(8)
+    o1, _ = orc.attn_lists(q, k, v, B, row_ptr, col)
+    o2, _ = orc.attn_lists(q, k[perm], v[perm], B, row_ptr, col)
+    assert np.abs(o1 - o2).max() <= 1e-6
+
+
+# ---------------------------------------------------------------- P10
+def test_p10_topn_total_order():
+    rng = np.random.default_rng(11)
+    for NB in (1, 5, 33, 200):
+        s = rng.standard_normal(NB).astype(np.float32)
+        s[rng.integers(0, NB, NB // 3)] = 0.5                # planted ties
+        if NB > 4:
+            s[[1, 3]] = s.max() + 1                          # tie at the top
+        for n in {1, 2, NB // 2 + 1, NB}:
+            expect = np.sort(np.argsort(-s.astype(np.float64), kind="stable")[:n])    # library: stable sort = (score desc, index asc)
+            assert np.array_equal(orc.topn(s, n, False), expect)
+            assert np.array_equal(orc.topn(s, n, True), expect)
+    s = np.array([1, 7, 7, 7, 3], np.float32)
+    assert list(orc.topn(s, 2, True)) == [1, 2] and list(orc.topn(s, 2, False)) == [1, 2]
+
+
+# ---------------------------------------------------------------- P11
+def test_p11_planted_structure_is_recovered_on_c1():
+    L = sy.config_c1()
+    sh = L.shape
+    S, T, B, NB = sh.S, sh.T, sh.B, sh.NB
+    # head 2: same-position, per-frame top-1 -> in every OTHER frame the kept block overlaps the q-block's own positions
+    hl = orc.select_head(L.q[2], L.k[2], S, T, B, ocfg(L.cfgs[2]))
+    hits = tot = 0
+    for I in range(NB):
+        t0, t1 = I * B, min(sh.N, (I + 1) * B)
+        if t0 // T != (t1 - 1) // T:
+            continue
+        p0, p1 = t0 % T, (t1 - 1) % T
+        for J in hl.col_idx[hl.row_ptr[I]:hl.row_ptr[I + 1]]:
+            j0, j1 = J * B, min(sh.N, (J + 1) * B) - 1
+            # positions covered by block J (may wrap a frame boundary)
+            pos = {j % T for j in range(j0, j1 + 1)}
+            tot += 1
+            hits += bool(pos & set(range(max(0, p0 - 20), min(T, p1 + 21))))
+    assert hits / tot >= 0.9
+    # head 3: sink -> probe top-S picks the S blocks that hold the special tokens (positions 0..4 of each frame)
+    hl = orc.select_head(L.q[3], L.k[3], S, T, B, ocfg(L.cfgs[3]))
+    assert sorted(hl.col_idx[:S]) == sorted({(f * T) // B for f in range(S)})
+
+
+# ---------------------------------------------------------------- P12
+def test_p12_masked_attention_matches_torch_sdpa_on_c1():
+    import torch
+    L = sy.config_c1()
+    sh = L.shape
+    for h in range(sh.H):
+        hl = orc.select_head(L.q[h], L.k[h], sh.S, sh.T, sh.B, ocfg(L.cfgs[h]))
+        out, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, hl.row_ptr, hl.col_idx)
+        mask = torch.from_numpy(lists_to_mask(hl.row_ptr, hl.col_idx, sh.N, sh.B))
+        qf, kf, vf = (torch.from_numpy(sy.bf16_bits_to_f32(x)) for x in (L.q[h], L.k[h], L.v[h]))
+        ref = torch.nn.functional.scaled_dot_product_attention(qf[None], kf[None], vf[None], attn_mask=mask[None])[0].numpy()
+        assert np.abs(out - ref).max() <= 1e-5
+
+
+# ---------------------------------------------------------------- P13
+def test_p13_nmse():
+    rng = np.random.default_rng(13)
+    a = rng.standard_normal((50, 8)).astype(np.float32)
+    assert orc.nmse(a, a) == 0.0
+    b = a + np.float32(0.1) * rng.standard_normal((50, 8)).astype(np.float32)
+    exp = ((a.astype(np.float64) - b) ** 2).sum() / (a.astype(np.float64) ** 2).sum()
+    assert abs(orc.nmse(a, b) - exp) <= 1e-12
+    assert abs(orc.nmse(a, np.zeros_like(a)) - 1.0) <= 1e-12       # dropping the head entirely ("Skip")
