@@ -1,0 +1,137 @@
+/*
+ * saf3r.h -- C ABI of the B200-native (sm_100a) SAF3R hot path.
+ *
+ * The hot path is the per-head dynamic sparse cross-view global attention of SAF3R
+ * (arxiv/paper_2607_03612; line numbers below are /root/reference/PAPER.md):
+ *   step 1  saf3r_select      -- online pattern adaptation (Sec. 4.3) restated at token-block
+ *                                granularity: pool Q/K into blocks, score block pairs, select a per-head block mask
+ *                                according to the head's type (Sec. 4.1).
+ *   step 2  saf3r_sparse_attn -- block-sparse softmax attention over the selected K/V blocks.
+ *   dense   saf3r_dense_attn  -- O_full = softmax(QK^T/sqrt(D))V, the library's own speedup baseline.
+ *
+ * Conventions
+ *   - Pointers named *_dev are DEVICE pointers owned by the caller (e.g. torch tensors); pointers named *_host are
+ *     plain host memory.  The library allocates no device memory after saf3r_create.
+ *   - q, k, v, out: bf16 (out optionally fp32), logical layout [H][N][D] addressed through two element strides
+ *     (stride_head, stride_token); the head_dim stride is 1.  N = num_frames * tokens_per_frame.
+ *     q/k/v base pointers must be 16-byte aligned and both strides multiples of 8 elements (TMA requirement).
+ *   - Token t belongs to frame floor(t/T) at in-frame position t mod T; block J holds tokens [J*B, min((J+1)*B, N)).
+ *   - Asynchrony: select / *_attn enqueue work on `cuda_stream` (a cudaStream_t passed as void*) and return.
+ *     Argument errors are returned synchronously before anything is enqueued.
+ *   - Errors: every call returns a saf3r_status; text via saf3r_last_error(ctx).  SAF3R_ERR_CUDA is sticky.
+ *   - There is no CPU fallback: on a machine without an sm_100 device saf3r_create fails with SAF3R_ERR_UNSUPPORTED.
+ */
+#ifndef SAF3R_H_
+#define SAF3R_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SAF3R_MAX_HEADS 64 /* per call; a batch folds into the head dimension */
+
+typedef struct saf3r_ctx saf3r_ctx; /* opaque; owns its tensor-map cache, a tiny device scratch and the error string */
+
+typedef enum {
+  SAF3R_OK = 0,
+  SAF3R_ERR_INVALID_ARG = 1,
+  SAF3R_ERR_UNSUPPORTED = 2, /* head_dim != 64, block not in {64,128}, H > SAF3R_MAX_HEADS, non-sm_100 device */
+  SAF3R_ERR_CAPACITY = 3,    /* lists / workspace buffer too small (required sizes: saf3r_query_sizes) */
+  SAF3R_ERR_CUDA = 4
+} saf3r_status;
+
+/* Head types = the paper's four tailored kernels + dense. */
+typedef enum {
+  SAF3R_HEAD_DENSE = 0,            /* all k-blocks (O_full) */
+  SAF3R_HEAD_UNIFORM_STRIDE = 1,   /* "Uniform Sampling Kernel", PAPER.md:L102 (scanning heads; also c_base, L106) */
+  SAF3R_HEAD_STATIC = 2,           /* "Static Kernel", PAPER.md:L96 (position heads) */
+  SAF3R_HEAD_QUERY_PROBE_TOPK = 3, /* "Query-Probe Top-K Kernel", PAPER.md:L98, L122-124 (vertical-line heads) */
+  SAF3R_HEAD_BLOCK_TOPK = 4        /* block-wise similarity Top-K, PAPER.md:L100, L126 (correspondence heads) */
+} saf3r_head_type;
+typedef enum { SAF3R_STATIC_ANCHOR = 0, SAF3R_STATIC_FRAME_LOCAL = 1, SAF3R_STATIC_POSITION_BAND = 2 } saf3r_static_mode;
+typedef enum { SAF3R_SCOPE_GLOBAL = 0, SAF3R_SCOPE_PER_FRAME = 1 } saf3r_topk_scope;
+typedef enum { SAF3R_SCORE_DOT = 0, SAF3R_SCORE_COSINE = 1 } saf3r_score_mode;
+
+/* One per head; plain host memory; all fields int32.  Selection rules (list of q-block I, ascending k-block indices):
+ *   DENSE            {0..NB-1}
+ *   UNIFORM_STRIDE   stride>=1: {offset + i*stride < NB} (0 <= offset < stride);  stride==0: {floor(i*NB/keep_blocks)}
+ *   STATIC/ANCHOR    blocks covering frame `anchor_frame`
+ *   STATIC/FRAME_LOCAL  blocks covering the frame(s) the tokens of q-block I belong to
+ *   STATIC/POSITION_BAND  for the in-frame positions [pa,pb] of q-block I: blocks covering positions
+ *                    [max(0,pa-r), min(T-1,pb+r)] of EVERY frame, r = band_radius
+ *   QUERY_PROBE_TOPK top-`keep_blocks` of p[J] = qbar . Ktilde_J / sqrt(D), same list for every I
+ *   BLOCK_TOPK       s[I][J] = Qtilde_I . Ktilde_J * c (c = 1/sqrt(D) for DOT; COSINE pools L2-normalised tokens, c = 1);
+ *                    GLOBAL: top-`keep_blocks` of the row; PER_FRAME: top-`topk_per_frame` inside each frame's
+ *                    candidate blocks {J : floor(J*B/T) = g}, union over frames g.
+ *   Top-n uses the total order (score descending, then index ascending). */
+typedef struct {
+  int32_t type;
+  int32_t stride, offset;
+  int32_t keep_blocks;
+  int32_t static_mode, anchor_frame, band_radius;
+  int32_t topk_scope, topk_per_frame;
+  int32_t score_mode;
+} saf3r_head_cfg;
+
+typedef struct {
+  int32_t num_frames, tokens_per_frame, num_heads, head_dim, block;
+  int64_t stride_head, stride_token; /* element strides of q/k/v/out */
+} saf3r_shape;
+
+/* CSR block lists: list of (h, I) = col_idx[row_ptr[h*NB+I] .. row_ptr[h*NB+I+1]), ascending, unique, 0 <= J < NB.
+ * An open format: callers may pass hand-made lists to saf3r_sparse_attn.  An empty list yields zero output rows
+ * and lse = -inf. */
+typedef struct {
+  int64_t *row_ptr; /* dev, [H*NB + 1] */
+  int32_t *col_idx; /* dev */
+  int64_t capacity; /* entries available in col_idx */
+} saf3r_lists;
+
+/* Create a context on CUDA device `device` (must be sm_100).  Returns SAF3R_ERR_UNSUPPORTED otherwise. */
+saf3r_status saf3r_create(saf3r_ctx **ctx, int device);
+void saf3r_destroy(saf3r_ctx *ctx);
+const char *saf3r_last_error(const saf3r_ctx *ctx);
+
+/* Host-only sizing.  List lengths are a closed form of (shape, cfg) for every head type, never of the data.
+ * list_entries: total col_idx entries saf3r_select will write.  workspace_bytes: device scratch saf3r_select needs
+ * (pooled Qtilde/Ktilde fp32, qbar, row lengths). cfg: host array [H]. */
+saf3r_status saf3r_query_sizes(const saf3r_shape *shape, const saf3r_head_cfg *cfg_host, int64_t *list_entries,
+                               size_t *workspace_bytes);
+
+/* Step 1: pool -> score -> select.  Writes out_lists->row_ptr (all H*NB+1 entries) and col_idx.
+ * SAF3R_ERR_CAPACITY if out_lists->capacity or workspace_bytes is too small. */
+saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const saf3r_shape *shape,
+                          const saf3r_head_cfg *cfg_host, void *workspace_dev, size_t workspace_bytes,
+                          saf3r_lists *out_lists, void *cuda_stream);
+
+/* Step 2: o_i = sum_j softmax_j(q_i.k_j/sqrt(D)) v_j over j in the blocks of list(h, blk(i)), j < N.
+ * out_dev: bf16 (out_is_fp32 = 0) or fp32 (1), same [H][N][D] strides as q.  lse_dev_or_null: fp32 [H][N] contiguous,
+ * natural-log log-sum-exp of the kept logits. */
+saf3r_status saf3r_sparse_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const void *v_dev,
+                               const saf3r_shape *shape, const saf3r_lists *lists, void *out_dev, int out_is_fp32,
+                               float *lse_dev_or_null, void *cuda_stream);
+
+/* Dense mode of the same kernel (implicit list 0..NB-1, no list reads). */
+saf3r_status saf3r_dense_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const void *v_dev,
+                              const saf3r_shape *shape, void *out_dev, int out_is_fp32, float *lse_dev_or_null,
+                              void *cuda_stream);
+
+/* End-to-end convenience for HOST buffers (one global-attention layer): copies q/k/v (contiguous [H][N][D] bf16, ideally
+ * pinned) to the device scratch, runs select + sparse_attn, copies the bf16 output back to out_host, all on
+ * `cuda_stream`; returns after enqueueing (synchronise the stream before reading out_host).
+ * scratch_dev must hold saf3r_layer_host_scratch_bytes(...) bytes; shape strides are ignored (contiguous). */
+saf3r_status saf3r_layer_host_scratch_bytes(const saf3r_shape *shape, const saf3r_head_cfg *cfg_host, size_t *bytes);
+saf3r_status saf3r_layer_host(saf3r_ctx *ctx, const void *q_host, const void *k_host, const void *v_host,
+                              const saf3r_shape *shape, const saf3r_head_cfg *cfg_host, void *scratch_dev,
+                              size_t scratch_bytes, void *out_host, void *cuda_stream);
+
+/* Number of kernels the library has launched on this context since creation (for bench.py's gpu_launches). */
+int64_t saf3r_launch_count(const saf3r_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SAF3R_H_ */

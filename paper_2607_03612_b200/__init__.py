@@ -1,0 +1,218 @@
+"""paper_2607_03612_b200 -- thin Python binding of the SAF3R C-ABI library (include/saf3r.h).
+
+Argument marshalling only: every step of the hot path (pool, score, select, block-sparse / dense attention) runs in the
+hand-written sm_100a kernels of csrc/.  PyTorch is used for device memory and streams, nothing else.  There is no CPU
+fallback: importing works anywhere, but creating a context without the built library or without an sm_100 GPU raises.
+
+Function names mirror the C entry points: query_sizes, select, sparse_attn, dense_attn, layer_host.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libsaf3r.so")
+
+MAX_HEADS = 64
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CAPACITY, ERR_CUDA = range(5)
+_STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "CAPACITY", 4: "CUDA"}
+
+HEAD_DENSE, HEAD_UNIFORM_STRIDE, HEAD_STATIC, HEAD_QUERY_PROBE_TOPK, HEAD_BLOCK_TOPK = range(5)
+STATIC_ANCHOR, STATIC_FRAME_LOCAL, STATIC_POSITION_BAND = range(3)
+SCOPE_GLOBAL, SCOPE_PER_FRAME = range(2)
+SCORE_DOT, SCORE_COSINE = range(2)
+
+EXPORTS = ("saf3r_create", "saf3r_destroy", "saf3r_last_error", "saf3r_query_sizes", "saf3r_select", "saf3r_sparse_attn",
+           "saf3r_dense_attn", "saf3r_layer_host_scratch_bytes", "saf3r_layer_host", "saf3r_launch_count")
+
+
+class Saf3rError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"saf3r: {_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class HeadCfg(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in (
+        "type", "stride", "offset", "keep_blocks", "static_mode", "anchor_frame", "band_radius",
+        "topk_scope", "topk_per_frame", "score_mode")]
+
+
+class ShapeC(C.Structure):
+    _fields_ = [("num_frames", C.c_int32), ("tokens_per_frame", C.c_int32), ("num_heads", C.c_int32),
+                ("head_dim", C.c_int32), ("block", C.c_int32), ("stride_head", C.c_int64), ("stride_token", C.c_int64)]
+
+
+class ListsC(C.Structure):
+    _fields_ = [("row_ptr", C.c_void_p), ("col_idx", C.c_void_p), ("capacity", C.c_int64)]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree libsaf3r.so; raises if it has not been built (python -m paper_2607_03612_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2607_03612_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i64, i32 = C.c_void_p, C.c_int64, C.c_int
+        L.saf3r_create.argtypes = [C.POINTER(vp), i32]
+        L.saf3r_destroy.argtypes = [vp]
+        L.saf3r_destroy.restype = None
+        L.saf3r_last_error.argtypes = [vp]
+        L.saf3r_last_error.restype = C.c_char_p
+        L.saf3r_query_sizes.argtypes = [C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(i64), C.POINTER(C.c_size_t)]
+        L.saf3r_select.argtypes = [vp, vp, vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), vp, C.c_size_t, C.POINTER(ListsC), vp]
+        L.saf3r_sparse_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(ListsC), vp, i32, vp, vp]
+        L.saf3r_dense_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), vp, i32, vp, vp]
+        L.saf3r_layer_host_scratch_bytes.argtypes = [C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(C.c_size_t)]
+        L.saf3r_layer_host.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), vp, C.c_size_t, vp, vp]
+        L.saf3r_launch_count.argtypes = [vp]
+        L.saf3r_launch_count.restype = i64
+        _lib = L
+    return _lib
+
+
+def make_cfgs(cfgs) -> "C.Array[HeadCfg]":
+    """cfgs: list of dicts (the ten int32 fields) or HeadCfg."""
+    arr = (HeadCfg * len(cfgs))()
+    for i, c in enumerate(cfgs):
+        if isinstance(c, HeadCfg):
+            arr[i] = c
+        else:
+            for k, v in c.items():
+                setattr(arr[i], k, int(v))
+    return arr
+
+
+def make_shape(S: int, T: int, H: int, D: int, B: int, stride_head: int | None = None, stride_token: int | None = None) -> ShapeC:
+    st = D if stride_token is None else stride_token
+    sh = S * T * st if stride_head is None else stride_head
+    return ShapeC(S, T, H, D, B, sh, st)
+
+
+@dataclass
+class Lists:
+    row_ptr: "torch.Tensor"   # int64 [H*NB+1], device
+    col_idx: "torch.Tensor"   # int32 [capacity], device
+
+    def c(self) -> ListsC:
+        return ListsC(self.row_ptr.data_ptr(), self.col_idx.data_ptr(), self.col_idx.numel())
+
+
+def _stream_ptr(stream=None):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+class Context:
+    """Owns one saf3r_ctx on a CUDA device."""
+
+    def __init__(self, device: int = 0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("saf3r needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.lib = load_library()
+        self.device = device
+        h = C.c_void_p()
+        st = self.lib.saf3r_create(C.byref(h), device)
+        if st != OK:
+            raise Saf3rError(st, "saf3r_create failed (needs an sm_100 device)")
+        self.h = h
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.saf3r_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st: int):
+        if st != OK:
+            raise Saf3rError(st, self.lib.saf3r_last_error(self.h).decode())
+
+    def launch_count(self) -> int:
+        return int(self.lib.saf3r_launch_count(self.h))
+
+    # ---- saf3r_query_sizes
+    def query_sizes(self, shape: ShapeC, cfgs) -> tuple[int, int]:
+        return query_sizes(shape, cfgs)
+
+    # ---- saf3r_select
+    def select(self, q, k, shape: ShapeC, cfgs, workspace=None, lists: Lists | None = None, stream=None) -> Lists:
+        import torch
+        arr = make_cfgs(cfgs)
+        entries, ws_bytes = query_sizes(shape, arr)
+        dev = q.device
+        if workspace is None:
+            workspace = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+        if lists is None:
+            N = shape.num_frames * shape.tokens_per_frame
+            NB = (N + shape.block - 1) // shape.block
+            lists = Lists(torch.empty(shape.num_heads * NB + 1, dtype=torch.int64, device=dev),
+                          torch.empty(max(entries, 1), dtype=torch.int32, device=dev))
+        lc = lists.c()
+        self._check(self.lib.saf3r_select(self.h, q.data_ptr(), k.data_ptr(), C.byref(shape), arr, workspace.data_ptr(),
+                                          workspace.numel() * workspace.element_size(), C.byref(lc), _stream_ptr(stream)))
+        return lists
+
+    # ---- saf3r_sparse_attn / saf3r_dense_attn
+    def sparse_attn(self, q, k, v, shape: ShapeC, lists: Lists, out=None, out_fp32: bool = False, want_lse: bool = False, stream=None):
+        return self._attn(q, k, v, shape, lists, out, out_fp32, want_lse, stream)
+
+    def dense_attn(self, q, k, v, shape: ShapeC, out=None, out_fp32: bool = False, want_lse: bool = False, stream=None):
+        return self._attn(q, k, v, shape, None, out, out_fp32, want_lse, stream)
+
+    def _attn(self, q, k, v, shape, lists, out, out_fp32, want_lse, stream):
+        import torch
+        if out is None:
+            out = torch.empty(q.shape, dtype=torch.float32 if out_fp32 else torch.bfloat16, device=q.device)
+        N = shape.num_frames * shape.tokens_per_frame
+        lse = torch.empty((shape.num_heads, N), dtype=torch.float32, device=q.device) if want_lse else None
+        lp = lse.data_ptr() if lse is not None else None
+        if lists is not None:
+            lc = lists.c()
+            st = self.lib.saf3r_sparse_attn(self.h, q.data_ptr(), k.data_ptr(), v.data_ptr(), C.byref(shape), C.byref(lc),
+                                            out.data_ptr(), int(out_fp32), lp, _stream_ptr(stream))
+        else:
+            st = self.lib.saf3r_dense_attn(self.h, q.data_ptr(), k.data_ptr(), v.data_ptr(), C.byref(shape),
+                                           out.data_ptr(), int(out_fp32), lp, _stream_ptr(stream))
+        self._check(st)
+        return (out, lse) if want_lse else out
+
+    # ---- saf3r_layer_host
+    def layer_host_scratch_bytes(self, shape: ShapeC, cfgs) -> int:
+        arr = make_cfgs(cfgs)
+        b = C.c_size_t()
+        self._check(self.lib.saf3r_layer_host_scratch_bytes(C.byref(shape), arr, C.byref(b)))
+        return int(b.value)
+
+    def layer_host(self, q_host, k_host, v_host, shape: ShapeC, cfgs, scratch, out_host, stream=None):
+        """q_host/k_host/v_host/out_host: (pinned) CPU tensors, contiguous [H][N][D] bf16.  Enqueues H2D + select +
+        sparse_attn + D2H on the stream; synchronise before reading out_host."""
+        arr = make_cfgs(cfgs)
+        self._check(self.lib.saf3r_layer_host(self.h, q_host.data_ptr(), k_host.data_ptr(), v_host.data_ptr(), C.byref(shape),
+                                              arr, scratch.data_ptr(), scratch.numel() * scratch.element_size(),
+                                              out_host.data_ptr(), _stream_ptr(stream)))
+        return out_host
+
+
+def query_sizes(shape: ShapeC, cfgs) -> tuple[int, int]:
+    """Host-only: (list entries, workspace bytes) saf3r_select needs.  Works without a GPU."""
+    L = load_library()
+    arr = cfgs if isinstance(cfgs, C.Array) else make_cfgs(cfgs)
+    n, w = C.c_int64(), C.c_size_t()
+    st = L.saf3r_query_sizes(C.byref(shape), arr, C.byref(n), C.byref(w))
+    if st != OK:
+        raise Saf3rError(st, "saf3r_query_sizes rejected (shape, cfg)")
+    return int(n.value), int(w.value)

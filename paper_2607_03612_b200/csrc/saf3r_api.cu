@@ -1,0 +1,395 @@
+// C ABI of the SAF3R hot path (include/saf3r.h): argument validation, host-side list sizing, tensor maps, launches.
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "saf3r.h"
+#include "attn_kernel.cuh"
+#include "select_kernels.cuh"
+
+using namespace saf3r;
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct MapKey {
+  const void *ptr;
+  int64_t N, stride_head, stride_token;
+  int32_t H, B;
+  bool operator==(const MapKey &o) const {
+    return ptr == o.ptr && N == o.N && stride_head == o.stride_head && stride_token == o.stride_token && H == o.H && B == o.B;
+  }
+};
+
+struct saf3r_ctx {
+  int device = 0;
+  int sm_count = 0;
+  EncodeTiledFn encode = nullptr;
+  std::string err;
+  bool sticky_cuda = false;
+  int64_t launches = 0;
+  std::vector<std::pair<MapKey, CUtensorMap>> maps;  // small LRU-less cache
+};
+
+static saf3r_status fail(saf3r_ctx *ctx, saf3r_status st, const std::string &msg) {
+  if (ctx) ctx->err = msg;
+  return st;
+}
+static saf3r_status cuda_fail(saf3r_ctx *ctx, cudaError_t e, const char *where) {
+  ctx->sticky_cuda = true;
+  ctx->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return SAF3R_ERR_CUDA;
+}
+#define CU_CHECK(call)                                          \
+  do {                                                          \
+    cudaError_t e__ = (call);                                   \
+    if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call); \
+  } while (0)
+
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static const char *validate_shape(const saf3r_shape *s, bool need_strides) {
+  if (!s) return "shape is null";
+  if (s->num_frames < 1 || s->tokens_per_frame < 1 || s->num_heads < 1) return "num_frames, tokens_per_frame, num_heads must be >= 1";
+  if (need_strides) {
+    if (s->stride_token < s->head_dim || s->stride_token % 8 || s->stride_head % 8) return "strides must be multiples of 8 elements and stride_token >= head_dim";
+  }
+  return nullptr;
+}
+static const char *unsupported_shape(const saf3r_shape *s) {
+  if (s->head_dim != 64) return "head_dim must be 64";
+  if (s->block != 64 && s->block != 128) return "block must be 64 or 128";
+  if (s->num_heads > SAF3R_MAX_HEADS) return "num_heads exceeds SAF3R_MAX_HEADS";
+  if ((int64_t)s->num_frames * s->tokens_per_frame > 0x7FFFFFFFll - 256) return "N too large";
+  return nullptr;
+}
+static SelGeom make_geom(const saf3r_shape *s) {
+  SelGeom g;
+  g.S = s->num_frames; g.T = s->tokens_per_frame; g.H = s->num_heads; g.B = s->block;
+  g.N = (int64_t)s->num_frames * s->tokens_per_frame;
+  g.NB = (int32_t)((g.N + g.B - 1) / g.B);
+  g.stride_head = s->stride_head; g.stride_token = s->stride_token;
+  return g;
+}
+static const char *validate_cfg(const SelGeom &g, const saf3r_head_cfg *cfg) {
+  if (!cfg) return "cfg is null";
+  for (int h = 0; h < g.H; ++h) {
+    const saf3r_head_cfg &c = cfg[h];
+    switch (c.type) {
+      case SAF3R_HEAD_DENSE: break;
+      case SAF3R_HEAD_UNIFORM_STRIDE:
+        if (c.stride < 0) return "UNIFORM_STRIDE: stride must be >= 0";
+        if (c.stride >= 1 && (c.offset < 0 || c.offset >= c.stride || c.offset >= g.NB)) return "UNIFORM_STRIDE: need 0 <= offset < min(stride, NB)";
+        if (c.stride == 0 && (c.keep_blocks < 1 || c.keep_blocks > g.NB)) return "UNIFORM_STRIDE: need 1 <= keep_blocks <= NB";
+        break;
+      case SAF3R_HEAD_STATIC:
+        if (c.static_mode < 0 || c.static_mode > 2) return "STATIC: bad static_mode";
+        if (c.static_mode == SAF3R_STATIC_ANCHOR && (c.anchor_frame < 0 || c.anchor_frame >= g.S)) return "STATIC/ANCHOR: anchor_frame out of range";
+        if (c.static_mode == SAF3R_STATIC_POSITION_BAND && c.band_radius < 0) return "STATIC/POSITION_BAND: band_radius must be >= 0";
+        break;
+      case SAF3R_HEAD_QUERY_PROBE_TOPK:
+        if (c.keep_blocks < 1 || c.keep_blocks > g.NB) return "QUERY_PROBE_TOPK: need 1 <= keep_blocks <= NB";
+        break;
+      case SAF3R_HEAD_BLOCK_TOPK:
+        if (c.score_mode < 0 || c.score_mode > 1) return "BLOCK_TOPK: bad score_mode";
+        if (c.topk_scope == SAF3R_SCOPE_GLOBAL) {
+          if (c.keep_blocks < 1 || c.keep_blocks > g.NB) return "BLOCK_TOPK/GLOBAL: need 1 <= keep_blocks <= NB";
+        } else if (c.topk_scope == SAF3R_SCOPE_PER_FRAME) {
+          if (c.topk_per_frame < 1) return "BLOCK_TOPK/PER_FRAME: topk_per_frame must be >= 1";
+        } else return "BLOCK_TOPK: bad topk_scope";
+        break;
+      default: return "unknown head type";
+    }
+  }
+  return nullptr;
+}
+
+struct WsLayout {
+  size_t qt, kt, qbar, rowlen, probe, total;
+};
+static WsLayout ws_layout(const SelGeom &g) {
+  WsLayout w;
+  size_t off = 0;
+  w.qt = off; off = align256(off + (size_t)g.H * g.NB * 64 * sizeof(float));
+  w.kt = off; off = align256(off + (size_t)g.H * g.NB * 64 * sizeof(float));
+  w.qbar = off; off = align256(off + (size_t)g.H * 64 * sizeof(float));
+  w.rowlen = off; off = align256(off + (size_t)g.H * g.NB * sizeof(int32_t));
+  w.probe = off; off = align256(off + (size_t)g.H * g.NB * sizeof(int32_t));
+  w.total = off;
+  return w;
+}
+static int64_t total_entries(const SelGeom &g, const saf3r_head_cfg *cfg) {
+  int64_t tot = 0;
+  for (int h = 0; h < g.H; ++h) {
+    const saf3r_head_cfg &c = cfg[h];
+    const bool per_row = c.type == SAF3R_HEAD_STATIC && c.static_mode != SAF3R_STATIC_ANCHOR;
+    if (per_row) {
+      for (int64_t I = 0; I < g.NB; ++I) tot += row_length(g, c, I);
+    } else {
+      tot += row_length(g, c, 0) * g.NB;
+    }
+  }
+  return tot;
+}
+
+extern "C" {
+
+saf3r_status saf3r_create(saf3r_ctx **out, int device) {
+  if (!out) return SAF3R_ERR_INVALID_ARG;
+  *out = nullptr;
+  saf3r_ctx *ctx = new saf3r_ctx();
+  ctx->device = device;
+  cudaDeviceProp prop;
+  cudaError_t e = cudaSetDevice(device);
+  if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
+  if (e != cudaSuccess) {
+    fprintf(stderr, "saf3r_create: no usable CUDA device %d (%s); there is no CPU fallback\n", device, cudaGetErrorString(e));
+    delete ctx;
+    return SAF3R_ERR_UNSUPPORTED;
+  }
+  if (prop.major != 10) {
+    fprintf(stderr, "saf3r_create: device %d is sm_%d%d; this library is sm_100a only\n", device, prop.major, prop.minor);
+    delete ctx;
+    return SAF3R_ERR_UNSUPPORTED;
+  }
+  ctx->sm_count = prop.multiProcessorCount;
+  void *fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+  if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) {
+    fprintf(stderr, "saf3r_create: cuTensorMapEncodeTiled not available\n");
+    delete ctx;
+    return SAF3R_ERR_UNSUPPORTED;
+  }
+  ctx->encode = (EncodeTiledFn)fn;
+  e = cudaFuncSetAttribute(saf3r_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128>::kTotal);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  if (e != cudaSuccess) {
+    fprintf(stderr, "saf3r_create: cudaFuncSetAttribute failed: %s\n", cudaGetErrorString(e));
+    delete ctx;
+    return SAF3R_ERR_CUDA;
+  }
+  *out = ctx;
+  return SAF3R_OK;
+}
+
+void saf3r_destroy(saf3r_ctx *ctx) { delete ctx; }
+
+const char *saf3r_last_error(const saf3r_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int64_t saf3r_launch_count(const saf3r_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+saf3r_status saf3r_query_sizes(const saf3r_shape *shape, const saf3r_head_cfg *cfg, int64_t *list_entries, size_t *workspace_bytes) {
+  if (validate_shape(shape, false) || !cfg) return SAF3R_ERR_INVALID_ARG;
+  if (unsupported_shape(shape)) return SAF3R_ERR_UNSUPPORTED;
+  const SelGeom g = make_geom(shape);
+  if (validate_cfg(g, cfg)) return SAF3R_ERR_INVALID_ARG;
+  if (list_entries) *list_entries = total_entries(g, cfg);
+  if (workspace_bytes) *workspace_bytes = ws_layout(g).total;
+  return SAF3R_OK;
+}
+
+saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const saf3r_shape *shape, const saf3r_head_cfg *cfg,
+                          void *ws, size_t ws_bytes, saf3r_lists *lists, void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_shape(shape, true)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  const SelGeom g = make_geom(shape);
+  if (const char *m = validate_cfg(g, cfg)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (!q || !k || !ws || !lists || !lists->row_ptr || !lists->col_idx) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  if (((uintptr_t)q | (uintptr_t)k) & 15) return fail(ctx, SAF3R_ERR_INVALID_ARG, "q/k must be 16-byte aligned");
+  const WsLayout w = ws_layout(g);
+  const int64_t need = total_entries(g, cfg);
+  if (ws_bytes < w.total || lists->capacity < need) {
+    char buf[160];
+    snprintf(buf, sizeof buf, "capacity: need %lld list entries (have %lld), %zu workspace bytes (have %zu)", (long long)need,
+             (long long)lists->capacity, w.total, ws_bytes);
+    return fail(ctx, SAF3R_ERR_CAPACITY, buf);
+  }
+  cudaStream_t st = (cudaStream_t)stream_;
+  uint8_t *wsb = (uint8_t *)ws;
+  float *qt = (float *)(wsb + w.qt), *kt = (float *)(wsb + w.kt), *qbar = (float *)(wsb + w.qbar);
+  int32_t *rowlen = (int32_t *)(wsb + w.rowlen), *probe = (int32_t *)(wsb + w.probe);
+
+  HeadCfgArray ca;
+  memset(&ca, 0, sizeof ca);
+  PoolFlags pf;
+  memset(&pf, 0, sizeof pf);
+  bool any_pool = false, any_probe = false, any_block = false;
+  for (int h = 0; h < g.H; ++h) {
+    ca.c[h] = cfg[h];
+    if (cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK) { pf.f[h] = 3; any_probe = true; }
+    if (cfg[h].type == SAF3R_HEAD_BLOCK_TOPK) { pf.f[h] = 3 | (cfg[h].score_mode == SAF3R_SCORE_COSINE ? 4 : 0); any_block = true; }
+    any_pool |= pf.f[h] != 0;
+  }
+  const int64_t rows = (int64_t)g.H * g.NB;
+  rowlen_kernel<<<(unsigned)((rows + 255) / 256), 256, 0, st>>>(rowlen, g, ca);
+  scan_kernel<<<1, 1024, 0, st>>>(rowlen, lists->row_ptr, rows);
+  ctx->launches += 2;
+  if (any_pool) {
+    pool_kernel<<<dim3(g.NB, g.H, 2), 256, 0, st>>>((const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, g, pf);
+    ctx->launches += 1;
+  }
+  if (any_probe) {
+    qbar_kernel<<<g.H, 256, 0, st>>>(qt, qbar, g, ca);
+    const size_t sm = (size_t)g.NB * 4 + 256 * 4;
+    if (sm > 220 * 1024) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the probe kernel");
+    probe_kernel<<<g.H, 256, sm, st>>>(kt, qbar, probe, g, ca);
+    ctx->launches += 2;
+  }
+  int R = 8;
+  size_t sm = 0;
+  if (any_block) {
+    const size_t budget = 220 * 1024 - 8 * 256 * 4;
+    while (R > 1 && (size_t)R * (g.NB + 64) * 4 > budget) --R;
+    if ((size_t)R * (g.NB + 64) * 4 > budget) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the select kernel");
+    sm = (size_t)R * (g.NB + 64) * 4 + 8 * 256 * 4;
+  }
+  select_kernel<<<dim3((g.NB + R - 1) / R, g.H), 256, sm, st>>>(qt, kt, probe, lists->row_ptr, lists->col_idx, g, ca, R);
+  ctx->launches += 1;
+  CU_CHECK(cudaGetLastError());
+  return SAF3R_OK;
+}
+
+static saf3r_status get_map(saf3r_ctx *ctx, const void *ptr, const SelGeom &g, CUtensorMap *out) {
+  MapKey key{ptr, g.N, g.stride_head, g.stride_token, g.H, g.B};
+  for (auto &kv : ctx->maps)
+    if (kv.first == key) { *out = kv.second; return SAF3R_OK; }
+  CUtensorMap m;
+  const cuuint64_t dims[3] = {64, (cuuint64_t)g.N, (cuuint64_t)g.H};
+  const cuuint64_t strides[2] = {(cuuint64_t)g.stride_token * 2, (cuuint64_t)g.stride_head * 2};
+  const cuuint32_t box[3] = {64, (cuuint32_t)g.B, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  // with one head the head stride is irrelevant but must still be a valid (multiple of 16, >= row extent) value
+  cuuint64_t strides_fixed[2] = {strides[0], strides[1]};
+  if (g.H == 1 && strides_fixed[1] < strides_fixed[0] * (cuuint64_t)g.N) strides_fixed[1] = strides_fixed[0] * (cuuint64_t)g.N;
+  CUresult r = ctx->encode(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void *>(ptr), dims, strides_fixed, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    char buf[96];
+    snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return fail(ctx, SAF3R_ERR_INVALID_ARG, buf);
+  }
+  if (ctx->maps.size() >= 64) ctx->maps.erase(ctx->maps.begin());
+  ctx->maps.emplace_back(key, m);
+  *out = m;
+  return SAF3R_OK;
+}
+
+static saf3r_status attn_common(saf3r_ctx *ctx, const void *q, const void *k, const void *v, const saf3r_shape *shape,
+                                const saf3r_lists *lists, void *out, int out_is_fp32, float *lse, void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_shape(shape, true)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  if (!q || !k || !v || !out) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  if (((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) return fail(ctx, SAF3R_ERR_INVALID_ARG, "q/k/v/out must be 16-byte aligned");
+  if (lists && (!lists->row_ptr || !lists->col_idx)) return fail(ctx, SAF3R_ERR_INVALID_ARG, "lists has null arrays");
+  const SelGeom g = make_geom(shape);
+  CUtensorMap mq, mk, mv;
+  saf3r_status s;
+  if ((s = get_map(ctx, q, g, &mq)) != SAF3R_OK) return s;
+  if ((s = get_map(ctx, k, g, &mk)) != SAF3R_OK) return s;
+  if ((s = get_map(ctx, v, g, &mv)) != SAF3R_OK) return s;
+  AttnParams p;
+  p.row_ptr = lists ? lists->row_ptr : nullptr;
+  p.col_idx = lists ? lists->col_idx : nullptr;
+  p.out = out;
+  p.lse = lse;
+  p.out_stride_head = shape->stride_head;
+  p.out_stride_token = shape->stride_token;
+  p.N = (int32_t)g.N; p.NB = g.NB; p.H = g.H;
+  p.out_fp32 = out_is_fp32 ? 1 : 0;
+  p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)shape->head_dim));
+  cudaStream_t st = (cudaStream_t)stream_;
+  dim3 grid(g.NB, g.H);
+  if (g.B == 128)
+    saf3r_attn_kernel<128><<<grid, kAttnThreads, AttnSmem<128>::kTotal, st>>>(mq, mk, mv, p);
+  else
+    saf3r_attn_kernel<64><<<grid, kAttnThreads, AttnSmem<64>::kTotal, st>>>(mq, mk, mv, p);
+  ctx->launches += 1;
+  CU_CHECK(cudaGetLastError());
+  return SAF3R_OK;
+}
+
+saf3r_status saf3r_sparse_attn(saf3r_ctx *ctx, const void *q, const void *k, const void *v, const saf3r_shape *shape,
+                               const saf3r_lists *lists, void *out, int out_is_fp32, float *lse, void *stream) {
+  if (!lists) return fail(ctx, SAF3R_ERR_INVALID_ARG, "lists is null");
+  return attn_common(ctx, q, k, v, shape, lists, out, out_is_fp32, lse, stream);
+}
+
+saf3r_status saf3r_dense_attn(saf3r_ctx *ctx, const void *q, const void *k, const void *v, const saf3r_shape *shape, void *out,
+                              int out_is_fp32, float *lse, void *stream) {
+  return attn_common(ctx, q, k, v, shape, nullptr, out, out_is_fp32, lse, stream);
+}
+
+struct HostLayout {
+  size_t q, k, v, out, ws, row_ptr, col_idx, total;
+  int64_t entries;
+};
+static HostLayout host_layout(const SelGeom &g, const saf3r_head_cfg *cfg) {
+  HostLayout l;
+  const size_t t = align256((size_t)g.H * g.N * 64 * 2);
+  size_t off = 0;
+  l.q = off; off += t;
+  l.k = off; off += t;
+  l.v = off; off += t;
+  l.out = off; off += t;
+  l.ws = off; off += ws_layout(g).total;
+  l.row_ptr = off; off = align256(off + ((size_t)g.H * g.NB + 1) * 8);
+  l.entries = total_entries(g, cfg);
+  l.col_idx = off; off = align256(off + (size_t)(l.entries > 0 ? l.entries : 1) * 4);
+  l.total = off;
+  return l;
+}
+
+saf3r_status saf3r_layer_host_scratch_bytes(const saf3r_shape *shape, const saf3r_head_cfg *cfg, size_t *bytes) {
+  if (validate_shape(shape, false) || !cfg || !bytes) return SAF3R_ERR_INVALID_ARG;
+  if (unsupported_shape(shape)) return SAF3R_ERR_UNSUPPORTED;
+  const SelGeom g = make_geom(shape);
+  if (validate_cfg(g, cfg)) return SAF3R_ERR_INVALID_ARG;
+  *bytes = host_layout(g, cfg).total;
+  return SAF3R_OK;
+}
+
+saf3r_status saf3r_layer_host(saf3r_ctx *ctx, const void *qh, const void *kh, const void *vh, const saf3r_shape *shape_in,
+                              const saf3r_head_cfg *cfg, void *scratch, size_t scratch_bytes, void *out_host, void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_shape(shape_in, false)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape_in)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  saf3r_shape shape = *shape_in;
+  shape.stride_token = 64;
+  shape.stride_head = (int64_t)shape.num_frames * shape.tokens_per_frame * 64;
+  const SelGeom g = make_geom(&shape);
+  if (const char *m = validate_cfg(g, cfg)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (!qh || !kh || !vh || !scratch || !out_host) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  const HostLayout l = host_layout(g, cfg);
+  if (scratch_bytes < l.total) return fail(ctx, SAF3R_ERR_CAPACITY, "scratch too small (see saf3r_layer_host_scratch_bytes)");
+  cudaStream_t st = (cudaStream_t)stream_;
+  uint8_t *sb = (uint8_t *)scratch;
+  const size_t bytes = (size_t)g.H * g.N * 64 * 2;
+  CU_CHECK(cudaMemcpyAsync(sb + l.q, qh, bytes, cudaMemcpyHostToDevice, st));
+  CU_CHECK(cudaMemcpyAsync(sb + l.k, kh, bytes, cudaMemcpyHostToDevice, st));
+  CU_CHECK(cudaMemcpyAsync(sb + l.v, vh, bytes, cudaMemcpyHostToDevice, st));
+  saf3r_lists lists{(int64_t *)(sb + l.row_ptr), (int32_t *)(sb + l.col_idx), l.entries > 0 ? l.entries : 1};
+  saf3r_status s = saf3r_select(ctx, sb + l.q, sb + l.k, &shape, cfg, sb + l.ws, ws_layout(g).total, &lists, stream_);
+  if (s != SAF3R_OK) return s;
+  s = saf3r_sparse_attn(ctx, sb + l.q, sb + l.k, sb + l.v, &shape, &lists, sb + l.out, 0, nullptr, stream_);
+  if (s != SAF3R_OK) return s;
+  CU_CHECK(cudaMemcpyAsync(out_host, sb + l.out, bytes, cudaMemcpyDeviceToHost, st));
+  return SAF3R_OK;
+}
+
+}  // extern "C"

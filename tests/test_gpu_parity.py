@@ -1,0 +1,229 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element, on seeded inputs.
+Tolerances (north_star): block-index lists bit-exact except counted near-ties (1e-4 relative of the cut);
+attention outputs (bf16 in, fp32 accumulate) max-abs 1e-2 and mean-abs 1e-3."""
+import numpy as np
+import pytest
+
+import oracle as orc
+import saf3r_synth as sy
+from parity_util import (c_shape, check_attention, compare_lists, concat_lists, oracle_lists, to_dev, upload)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    import paper_2607_03612_b200 as sf
+    return sf, sf.Context(0), torch
+
+
+def small_layer(S, G, H, B, gens, cfgs, seed):
+    sh = sy.Shape(S=S, G=G, H=H, D=64, B=B)
+    return sy.make_layer(sh, gens, cfgs, seed)
+
+
+def dev_lists(sf, torch, row_ptr, col):
+    col = col if col.size else np.zeros(1, np.int32)
+    return sf.Lists(torch.from_numpy(row_ptr).cuda(), torch.from_numpy(col).cuda())
+
+
+ALL_KINDS = [
+    (sy.GEN_UNIFORM, sy.cfg(type=sy.HEAD_DENSE)),
+    (sy.GEN_UNIFORM, sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=3, offset=1)),
+    (sy.GEN_UNIFORM, sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=0, keep_blocks=5)),
+    (sy.GEN_ANCHOR, sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_ANCHOR, anchor_frame=1)),
+    (sy.GEN_FRAME_LOCAL, sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_FRAME_LOCAL)),
+    (sy.GEN_SAME_POSITION, sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_POSITION_BAND, band_radius=10)),
+    (sy.GEN_SINK, sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=4)),
+    (sy.GEN_SAME_POSITION, sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=5)),
+    (sy.GEN_SAME_POSITION, sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=5, score_mode=sy.SCORE_COSINE)),
+    (sy.GEN_SAME_POSITION, sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=1)),
+    (sy.GEN_SAME_POSITION, sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=2, score_mode=sy.SCORE_COSINE)),
+    (sy.GEN_UNIFORM, sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=7)),
+]
+
+
+# ------------------------------------------------------------------------------------------------ dense mode
+@pytest.mark.parametrize("S,G,B", [(4, 16, 64), (3, 17, 128), (1, 6, 128), (1, 6, 64)])
+def test_dense_attn_matches_oracle(env, S, G, B):
+    sf, ctx, torch = env
+    gens = [sy.GEN_UNIFORM, sy.GEN_SAME_POSITION, sy.GEN_SINK]
+    L = small_layer(S, G, 3, B, gens, [sy.cfg(type=sy.HEAD_DENSE)] * 3, seed=11)
+    q, k, v = upload(L)
+    out, lse = ctx.dense_attn(q, k, v, c_shape(sf, L.shape), out_fp32=True, want_lse=True)
+    out_bf = ctx.dense_attn(q, k, v, c_shape(sf, L.shape))
+    torch.cuda.synchronize()
+    for h in range(3):
+        ref, ref_lse = orc.attn_dense(L.q[h], L.k[h], L.v[h])
+        check_attention(out[h].cpu().numpy(), ref, f"dense fp32 head {h}")
+        assert np.abs(lse[h].cpu().numpy() - ref_lse).max() <= 1e-2
+        d = np.abs(out_bf[h].float().cpu().numpy() - ref)
+        assert d.max() <= 2e-2          # bf16 output adds its own rounding (|o| up to ~4): parity is judged on fp32 out
+
+
+# ------------------------------------------------------------------------------------------------ sparse attention, oracle lists
+@pytest.mark.parametrize("S,G,B", [(4, 16, 64), (4, 17, 128)])
+def test_sparse_attn_with_oracle_lists(env, S, G, B):
+    sf, ctx, torch = env
+    gens = [g for g, _ in ALL_KINDS]
+    cfgs = [c for _, c in ALL_KINDS]
+    L = small_layer(S, G, len(gens), B, gens, cfgs, seed=12)
+    hls = oracle_lists(L)
+    row_ptr, col = concat_lists(hls)
+    q, k, v = upload(L)
+    out, lse = ctx.sparse_attn(q, k, v, c_shape(sf, L.shape), dev_lists(sf, torch, row_ptr, col), out_fp32=True, want_lse=True)
+    torch.cuda.synchronize()
+    for h, hl in enumerate(hls):
+        ref, ref_lse = orc.attn_lists(L.q[h], L.k[h], L.v[h], B, hl.row_ptr, hl.col_idx)
+        check_attention(out[h].cpu().numpy(), ref, f"sparse head {h} ({gens[h]})")
+        assert np.abs(lse[h].cpu().numpy() - ref_lse).max() <= 1e-2
+
+
+def test_sparse_attn_empty_and_handmade_lists(env):
+    sf, ctx, torch = env
+    L = small_layer(3, 17, 2, 128, [sy.GEN_UNIFORM, sy.GEN_SINK], [sy.cfg(type=sy.HEAD_DENSE)] * 2, seed=13)
+    NB = L.shape.NB                      # N = 882 -> NB = 7, tail 114
+    rng = np.random.default_rng(0)
+    rows = []
+    for r in range(2 * NB):
+        n = [0, 1, NB, 3][r % 4]
+        rows.append(np.sort(rng.choice(NB, n, replace=False)).astype(np.int32))
+    rows[1] = np.array([NB - 1], np.int32)       # only the tail block
+    row_ptr = np.concatenate([[0], np.cumsum([len(r) for r in rows])]).astype(np.int64)
+    col = np.concatenate(rows)
+    q, k, v = upload(L)
+    out, lse = ctx.sparse_attn(q, k, v, c_shape(sf, L.shape), dev_lists(sf, torch, row_ptr, col), out_fp32=True, want_lse=True)
+    torch.cuda.synchronize()
+    for h in range(2):
+        rp = row_ptr[h * NB:(h + 1) * NB + 1]
+        ref, ref_lse = orc.attn_lists(L.q[h], L.k[h], L.v[h], 128, rp - rp[0], col[rp[0]:rp[-1]])
+        o = out[h].cpu().numpy()
+        check_attention(o, ref, f"handmade head {h}")
+        ls = lse[h].cpu().numpy()
+        empty = np.isneginf(ref_lse)
+        assert empty.any() and np.all(np.isneginf(ls[empty])) and np.all(o[empty] == 0)
+        assert np.abs(ls[~empty] - ref_lse[~empty]).max() <= 1e-2
+
+
+def test_strided_layout_nhd(env):
+    """[N][H][D] tensors through the two strides."""
+    sf, ctx, torch = env
+    L = small_layer(2, 17, 3, 128, [sy.GEN_UNIFORM] * 3, [sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=2)] * 3, seed=14)
+    sh = L.shape
+    q, k, v = (t.permute(1, 0, 2).contiguous() for t in upload(L))       # [N][H][D]
+    shape = sf.make_shape(sh.S, sh.T, sh.H, sh.D, sh.B, stride_head=sh.D, stride_token=sh.H * sh.D)
+    lists = ctx.select(q, k, shape, L.cfgs)
+    out = torch.zeros_like(q, dtype=torch.float32)
+    ctx.sparse_attn(q, k, v, shape, lists, out=out, out_fp32=True)
+    torch.cuda.synchronize()
+    for h, hl in enumerate(oracle_lists(L)):
+        ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, hl.row_ptr, hl.col_idx)
+        check_attention(out[:, h].cpu().numpy(), ref, f"NHD head {h}")
+
+
+# ------------------------------------------------------------------------------------------------ select
+@pytest.mark.parametrize("S,G,B", [(4, 16, 64), (5, 17, 128), (7, 9, 64)])
+def test_select_matches_oracle_all_head_types(env, S, G, B):
+    sf, ctx, torch = env
+    gens = [g for g, _ in ALL_KINDS]
+    cfgs = [c for _, c in ALL_KINDS]
+    L = small_layer(S, G, len(gens), B, gens, cfgs, seed=15)
+    q, k, _ = upload(L)
+    lists = ctx.select(q, k, c_shape(sf, L.shape), L.cfgs)
+    torch.cuda.synchronize()
+    stats = compare_lists(L, lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy(), oracle_lists(L))
+    print("near-ties:", stats)
+    assert stats["tie_floored"] <= 0.01 * stats["entries"]
+
+
+def test_c1_end_to_end(env):
+    sf, ctx, torch = env
+    L = sy.config_c1()
+    sh = L.shape
+    q, k, v = upload(L)
+    shape = c_shape(sf, sh)
+    lists = ctx.select(q, k, shape, L.cfgs)
+    out = ctx.sparse_attn(q, k, v, shape, lists, out_fp32=True)
+    torch.cuda.synchronize()
+    hls = oracle_lists(L)
+    rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
+    stats = compare_lists(L, rp, col, hls)
+    assert stats["tie_floored"] == 0
+    for h in range(sh.H):
+        # protocol (iii): oracle attention evaluated on the GPU's own lists
+        r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
+        ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, r - r[0], col[r[0]:r[-1]])
+        check_attention(out[h].cpu().numpy(), ref, f"C1 head {h}")
+
+
+def test_layer_host_end_to_end(env):
+    sf, ctx, torch = env
+    L = sy.config_c1()
+    sh = L.shape
+    shape = c_shape(sf, sh)
+    qh, kh, vh = (torch.from_numpy(x.view(np.int16)).view(torch.bfloat16).pin_memory() for x in (L.q, L.k, L.v))
+    out_h = torch.empty_like(qh).pin_memory()
+    scratch = torch.empty(ctx.layer_host_scratch_bytes(shape, L.cfgs), dtype=torch.uint8, device="cuda")
+    ctx.layer_host(qh, kh, vh, shape, L.cfgs, scratch, out_h)
+    torch.cuda.synchronize()
+    for h, hl in enumerate(oracle_lists(L)):
+        ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, hl.row_ptr, hl.col_idx)
+        assert np.abs(out_h[h].float().numpy() - ref).max() <= 2e-2
+
+
+def test_errors_are_reported(env):
+    sf, ctx, torch = env
+    L = sy.config_c1()
+    q, k, v = upload(L)
+    bad = sf.make_shape(4, 261, 4, 32, 64)
+    with pytest.raises(sf.Saf3rError) as ei:
+        ctx.dense_attn(q, k, v, bad)
+    assert ei.value.status == sf.ERR_UNSUPPORTED
+    shape = c_shape(sf, L.shape)
+    small = sf.Lists(torch.zeros(4 * 17 + 1, dtype=torch.int64, device="cuda"), torch.zeros(3, dtype=torch.int32, device="cuda"))
+    with pytest.raises(sf.Saf3rError) as ei:
+        ctx.select(q, k, shape, L.cfgs, lists=small)
+    assert ei.value.status == sf.ERR_CAPACITY
+    with pytest.raises(sf.Saf3rError) as ei:
+        ctx.select(q, k, shape, [sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=0)] * 4)
+    assert ei.value.status == sf.ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------------------------------------ C2 (VGGT shape), full size
+def test_c2_full_size_lists_and_sampled_attention(env):
+    sf, ctx, torch = env
+    L = sy.config_c2()
+    sh = L.shape
+    q, k, v = upload(L)
+    shape = c_shape(sf, sh)
+    lists = ctx.select(q, k, shape, L.cfgs)
+    out = ctx.sparse_attn(q, k, v, shape, lists, out_fp32=True)
+    torch.cuda.synchronize()
+    hls = oracle_lists(L)
+    rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
+    stats = compare_lists(L, rp, col, hls)
+    print("C2 near-ties:", stats)
+    assert stats["tie_floored"] <= 1e-3 * stats["entries"]
+    rng = np.random.default_rng(2)
+    o = out.cpu().numpy()
+    for h in range(sh.H):
+        qb = np.unique(np.concatenate([rng.choice(sh.NB, 6, replace=False), [0, sh.NB - 1]])).astype(np.int64)
+        r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
+        ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, r - r[0], col[r[0]:r[-1]], qb)
+        check_attention(o[h], ref, f"C2 head {h} ({L.gens[h]})")
+
+
+def test_c2_dense_sampled_rows(env):
+    sf, ctx, torch = env
+    L = sy.config_c2()
+    sh = L.shape
+    q, k, v = upload(L)
+    out = ctx.dense_attn(q, k, v, c_shape(sf, sh), out_fp32=True)
+    torch.cuda.synchronize()
+    for h in (0, 5, 9, 13):
+        i0 = (h * 9973) % (sh.N - 64)
+        ref, _ = orc.attn_dense(L.q[h], L.k[h], L.v[h], i0, i0 + 64)
+        check_attention(out[h].cpu().numpy(), ref, f"C2 dense head {h}")
+        ref, _ = orc.attn_dense(L.q[h], L.k[h], L.v[h], sh.N - 64, sh.N)
+        check_attention(out[h].cpu().numpy(), ref, f"C2 dense tail head {h}")
