@@ -1,0 +1,331 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for BASELINE.json's metric: global-attention layer ms (and dense-equivalent / executed
+TFLOP/s) at 100 frames.
+
+A "step" is one pass of the whole hot path over one synthetic global-attention layer of config C3
+(S=100 frames x 1374 tokens, N=137400, H=16, D=64, B=128): saf3r_select (pool -> score -> select) followed by
+saf3r_sparse_attn, with a seeded per-layer mix of head types and sparsity.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config c2|c3|c4|c5]
+
+N > 1 (torchrun): every rank runs the same number of independent layers (the path shards over independent
+layers/heads with no data-path collective) -> "scaling": "weak".
+--impl reference times the CPU oracle (oracle/), as it stands, on the host cores on a bounded sample of the workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import saf3r_synth as sy  # noqa: E402
+
+METRIC = "global_attn_layer_ms"
+UNIT = "ms/layer"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "tflops_burst": d["bf16_tflops"], "tflops_sustained": d["bf16_tflops_sustained"],
+                "source": "measured"}
+    return {"hbm_gbs": 6650.0, "tflops_burst": 1590.0, "tflops_sustained": 1400.0, "source": "fallback"}
+
+
+def shape_for(name: str) -> sy.Shape:
+    return {"c2": sy.shape_c2, "c3": sy.shape_c3, "c4": sy.shape_c4, "c5": sy.shape_c5}[name]()
+
+
+def make_layers(name: str, count: int):
+    sh = shape_for(name)
+    layers = []
+    for l in range(count):
+        if name == "c3":
+            layers.append(sy.config_c3_layer(l, sh=sh))
+        else:
+            gens, cfgs = sy.mixed_heads(sh)
+            layers.append(sy.make_layer(sh, gens, cfgs, seed={"c2": 2, "c4": 4, "c5": 5}[name] * 1000 + l, layer=l))
+    return layers
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.stop, self.t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self.stop.is_set():
+            try:
+                o = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                   capture_output=True, text=True, timeout=5).stdout.strip()
+                if o:
+                    self.rows.append([x.strip() for x in o.split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.2)
+
+    def __enter__(self):
+        self.t = threading.Thread(target=self._run, daemon=True)
+        self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.t.join(timeout=6)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 7 for n, v in zip(names, r[3:7]) if v.lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(sm)}
+
+
+def cpu_oracle_layer_ms(L: sy.Layer, qblocks_per_head: int, one_per_type: bool = False):
+    """The oracle as it stands on the host cores: selection of every head + attention on a bounded sample of q-blocks per
+    head, extrapolated to the layer (attention time scaled by NB / sampled).  one_per_type: time one head of each head
+    type and scale by the number of heads of that type (keeps a reference step to a few seconds)."""
+    import oracle as orc
+    sh = L.shape
+    rng = np.random.default_rng(0)
+    heads, weight = list(range(sh.H)), [1.0] * sh.H
+    if one_per_type:
+        first = {}
+        for h, g in enumerate(L.gens):
+            first.setdefault(g, h)
+        heads = sorted(first.values())
+        weight = [float(sum(1 for g in L.gens if g == L.gens[h])) for h in heads]
+    t_sel = t_att = 0.0
+    for h, w in zip(heads, weight):
+        t0 = time.perf_counter()
+        hl = orc.select_head(L.q[h], L.k[h], sh.S, sh.T, sh.B, orc.make_cfg(**L.cfgs[h]))
+        t1 = time.perf_counter()
+        qb = np.sort(rng.choice(sh.NB, qblocks_per_head, replace=False)).astype(np.int64)
+        orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, hl.row_ptr, hl.col_idx, qb, want_lse=False)
+        t2 = time.perf_counter()
+        t_sel += w * (t1 - t0)
+        t_att += w * (t2 - t1) * sh.NB / qblocks_per_head
+    return (t_sel + t_att) * 1e3, t_sel * 1e3, orc.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    sh = shape_for(args.config)
+    nq = 1 if args.config != "c2" else 2
+    layers = make_layers(args.config, 1)
+    times = []
+    for i in range(args.warmup + args.steps):
+        ms, _, cores = cpu_oracle_layer_ms(layers[0], nq, one_per_type=True)
+        if i >= args.warmup:
+            times.append(ms)
+    v = float(np.mean(times))
+    sample = (f"per step: select + attention on {nq} sampled q-block(s) for one head of each head type, scaled by heads per type and "
+              f"by NB/{nq} (extrapolated to the layer)")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(args.config, sh), "note": "CPU oracle (oracle/), not tuned"},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def workload_name(cfg: str, sh: sy.Shape) -> str:
+    return (f"{cfg.upper()}: one global-attention layer, S={sh.S} frames x T={sh.T} tokens, N={sh.N}, H={sh.H}, D={sh.D}, "
+            f"block {sh.B}, seeded per-layer mix of head types (uniform-stride / frame-local / same-position block top-k / "
+            f"sink query-probe) and sparsity")
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2607_03612_b200 as sf
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+    peaks = load_peaks()
+    sh = shape_for(args.config)
+    n_res = min(args.resident_layers, args.steps)
+    layers = make_layers(args.config, n_res)
+    ctx = sf.Context(local)
+    shape = sf.make_shape(sh.S, sh.T, sh.H, sh.D, sh.B)
+    stream = torch.cuda.current_stream()
+
+    def up(x):
+        return torch.from_numpy(x.view(np.int16)).to(dev).view(torch.bfloat16)
+
+    dl = []
+    for L in layers:
+        q, k, v = up(L.q), up(L.k), up(L.v)
+        entries, ws_bytes = sf.query_sizes(shape, L.cfgs)
+        lists = sf.Lists(torch.empty(sh.H * sh.NB + 1, dtype=torch.int64, device=dev),
+                         torch.empty(max(entries, 1), dtype=torch.int32, device=dev))
+        ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+        out = torch.empty_like(q)
+        dl.append(dict(q=q, k=k, v=v, lists=lists, ws=ws, out=out, cfgs=L.cfgs, entries=entries, ws_bytes=ws_bytes))
+
+    def step(i, ev=None):
+        d = dl[i % n_res]
+        if ev:
+            ev[0].record(stream)
+        ctx.select(d["q"], d["k"], shape, d["cfgs"], workspace=d["ws"], lists=d["lists"])
+        if ev:
+            ev[1].record(stream)
+        ctx.sparse_attn(d["q"], d["k"], d["v"], shape, d["lists"], out=d["out"])
+        if ev:
+            ev[2].record(stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        step(i)
+    barrier()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    launches0 = ctx.launch_count()
+    with ClockSampler(local) as clk:
+        barrier()
+        t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t_beg.record(stream)
+        for i in range(args.steps):
+            step(i, evs[i])
+        t_end.record(stream)
+        barrier()
+    launches = ctx.launch_count() - launches0
+    total_ms = t_beg.elapsed_time(t_end)
+    if world > 1:
+        t = torch.tensor([total_ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    sel_ms = [e[0].elapsed_time(e[1]) for e in evs]
+    att_ms = [e[1].elapsed_time(e[2]) for e in evs]
+
+    # work per step
+    pairs = [d["entries"] for d in dl]
+    exec_flop = [4.0 * sh.B * sh.B * sh.D * pairs[i % n_res] for i in range(args.steps)]
+    dense_flop = 4.0 * sh.N * sh.N * sh.D * sh.H
+    att_s = float(np.sum(att_ms)) * 1e-3
+    exec_tflops = float(np.sum(exec_flop)) / att_s / 1e12
+    ms_per_step = total_ms / args.steps
+    value = total_ms / (args.steps * world)
+
+    result = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic",
+        "config": {"workload": workload_name(args.config, sh), "resident_layers": n_res,
+                   "l2": "inputs (844 MB of Q/K/V per layer at C3) exceed the 126 MB L2; layers rotate" if args.config != "c2"
+                   else "inputs 270 MB/layer exceed L2; layers rotate",
+                   "kept_pair_ratio": float(np.mean(pairs)) / (sh.H * sh.NB * sh.NB)},
+        "gpu_launches": int(launches),
+        "select_ms": float(np.mean(sel_ms)), "sparse_attn_ms": float(np.mean(att_ms)),
+        "executed_tflops": exec_tflops, "dense_equiv_tflops": dense_flop * args.steps / (total_ms * 1e-3) / 1e12,
+    }
+
+    if rank == 0:
+        result["clocks"] = clk.summary()
+        # roofline of the dominant kernel (block-sparse attention): executed FLOP per launch / mean launch duration
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tp):
+            traffic = json.load(open(tp)).get("saf3r_attn_kernel_bytes_per_launch")
+        result["roofline"] = {"bound": "tensor", "achieved": exec_tflops, "peak": peaks["tflops_sustained"], "unit": "TFLOP/s",
+                              "frac": exec_tflops / peaks["tflops_sustained"], "traffic": traffic,
+                              "kernel": "saf3r_attn_kernel", "peak_source": f"{peaks['source']} sustained bf16 (kernel timed inside a long step)",
+                              "frac_of_burst": exec_tflops / peaks["tflops_burst"]}
+        # selection pass against HBM: algorithmic bytes = Q and/or K of the heads whose rule reads them
+        need = [sum((2 if c["type"] in (sy.HEAD_QUERY_PROBE_TOPK, sy.HEAD_BLOCK_TOPK) else 0) for c in d["cfgs"]) for d in dl]
+        sel_bytes = [need[i % n_res] * sh.N * sh.D * 2 for i in range(args.steps)]
+        sel_gbs = float(np.sum(sel_bytes)) / (float(np.sum(sel_ms)) * 1e-3) / 1e9
+        result["select_roofline"] = {"bound": "hbm", "achieved": sel_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                     "frac": sel_gbs / peaks["hbm_gbs"], "note": "whole select call (pool+score+select) over the pool stage's algorithmic bytes"}
+
+        if not args.skip_dense:
+            d = dl[0]
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ctx.dense_attn(d["q"], d["k"], d["v"], shape, out=d["out"])
+            e0.record(stream)
+            for _ in range(args.dense_reps):
+                ctx.dense_attn(d["q"], d["k"], d["v"], shape, out=d["out"])
+            e1.record(stream)
+            torch.cuda.synchronize()
+            dense_ms = e0.elapsed_time(e1) / args.dense_reps
+            result["dense_attn_ms"] = dense_ms
+            result["dense_tflops"] = dense_flop / (dense_ms * 1e-3) / 1e12
+            result["speedup_vs_own_dense"] = dense_ms / ms_per_step
+
+        # e2e through the C ABI with HOST buffers (pinned), H2D + D2H inside the timed region
+        if not args.skip_e2e:
+            L = layers[0]
+            qh, kh, vh = (torch.from_numpy(x.view(np.int16)).view(torch.bfloat16).pin_memory() for x in (L.q, L.k, L.v))
+            oh = torch.empty_like(qh).pin_memory()
+            scratch = torch.empty(ctx.layer_host_scratch_bytes(shape, L.cfgs), dtype=torch.uint8, device=dev)
+            e_steps = max(2, min(args.steps, 6))
+            for _ in range(2):
+                ctx.layer_host(qh, kh, vh, shape, L.cfgs, scratch, oh)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(e_steps):
+                ctx.layer_host(qh, kh, vh, shape, L.cfgs, scratch, oh)
+                torch.cuda.synchronize()
+            e_ms = (time.perf_counter() - t0) * 1e3 / e_steps
+            nbytes = qh.numel() * 2
+            result["e2e"] = {"value": e_ms, "unit": UNIT, "h2d_bytes_per_step": 3 * nbytes, "d2h_bytes_per_step": nbytes,
+                             "steps": e_steps, "api": "saf3r_layer_host (pinned host q/k/v -> device, select + sparse_attn, out -> host)"}
+
+        if world == 1 and not args.skip_cpu:
+            ms, sel, cores = cpu_oracle_layer_ms(layers[0], 1)
+            result["cpu_baseline"] = {"value": ms, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                      "sample": f"layer 0: full select of all {sh.H} heads ({sel:.0f} ms) + attention on 1 sampled "
+                                                f"q-block/head scaled by NB={sh.NB} (extrapolated)"}
+        print(json.dumps(result))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=24)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c3", choices=["c2", "c3", "c4", "c5"])
+    ap.add_argument("--resident-layers", type=int, default=4)
+    ap.add_argument("--dense-reps", type=int, default=2)
+    ap.add_argument("--skip-dense", action="store_true")
+    ap.add_argument("--skip-e2e", action="store_true")
+    ap.add_argument("--skip-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
