@@ -1,13 +1,15 @@
 // Block-sparse / dense softmax attention for sm_100a (step a-4 / a-5 of DESIGN.md).
 //
-// One CTA per (head h, q-block I).  Six warps:
-//   warps 0-3  softmax: thread r owns q-row r (= TMEM lane r): reads S from TMEM, online softmax, writes P (bf16) to smem
-//   warp  4    TMA producer: Q tile once, then one (K_J, V_J) tile pair per list entry into a 2-stage ring
-//   warp  5    TMEM allocator + MMA issuer (one thread): S = Q K_J^T (tcgen05, SS) ; O += P V_J (tcgen05, SS)
-// Accumulators live in TMEM: S at columns [0,B), O at columns [128,192).  Two CTAs are resident per SM, so one CTA's
-// softmax overlaps the other's MMAs.
+// One CTA per (head h, q-block I), two CTAs resident per SM (one CTA's softmax overlaps the other's MMAs).  Warps:
+//   warps 0-3  softmax: thread r owns q-row r (= TMEM lane r).  One pass: S (fp32, TMEM) -> registers, row max
+//              (lazy: the running max only moves when it grows by more than 2^8), p = exp2(s*c - m*c), row sum,
+//              P (bf16) -> TMEM.  O is rescaled in TMEM only when the max moved.
+//   warp  4    TMA producer: Q tile once, then one (K_J, V_J) tile pair per list entry into a 3-stage ring
+//   warp  5    TMEM allocator + MMA issuer (one thread): S = Q K_J^T (tcgen05 SS), O += P V_J (tcgen05 TS: P from TMEM)
+// TMEM columns: S [0,B) fp32, O [128,192) fp32, P [192,192+B/2) packed bf16.
 #pragma once
 #include "ptx.cuh"
+#include "saf3r.h"
 
 namespace saf3r {
 
@@ -20,21 +22,23 @@ struct AttnParams {
   int32_t N, NB, H;
   int32_t out_fp32;
   float scale_log2;  // (1/sqrt(D)) * log2(e)
+  uint8_t head_order[SAF3R_MAX_HEADS];  // blockIdx.y -> head, longest lists first
 };
 
-constexpr int kD = 64;            // head_dim (bf16: one 128-byte swizzle row)
+constexpr int kD = 64;  // head_dim (bf16: one 128-byte swizzle row)
 constexpr int kAttnThreads = 192;
-constexpr int kStages = 2;
+constexpr int kStages = 3;
 constexpr int kTmemCols = 256;
-constexpr int kTmemO = 128;       // first O column
+constexpr int kTmemO = 128;  // first O column
+constexpr int kTmemP = 192;  // first P column
+constexpr float kLazyLog2 = 8.f;  // rescale only when the row max grows by more than 2^8 (in exp2 units)
 
 template <int B>
 struct AttnSmem {
-  static constexpr int kQ = 0;                               // 128 x 64 bf16 (only the first B rows are loaded)
-  static constexpr int kK = kQ + 128 * 128;                  // kStages x (B x 64 bf16)
+  static constexpr int kQ = 0;                       // 128 x 64 bf16 (only the first B rows are loaded)
+  static constexpr int kK = kQ + 128 * 128;          // kStages x (B x 64 bf16)
   static constexpr int kV = kK + kStages * B * 128;
-  static constexpr int kP = kV + kStages * B * 128;          // B/64 atoms of [128 rows][64 keys] bf16
-  static constexpr int kBar = kP + 128 * B * 2;
+  static constexpr int kBar = kV + kStages * B * 128;
   static constexpr int kTotal = kBar + 128;
 };
 
@@ -46,17 +50,17 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
   using L = AttnSmem<B>;
   const uint32_t sbase = smem_u32(smem);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int I = blockIdx.x, h = blockIdx.y;
+  const int I = blockIdx.x, h = p.head_order[blockIdx.y];
 
-  // barriers
   const uint32_t bar = sbase + L::kBar;
   const uint32_t bar_q = bar + 0;
   const uint32_t bar_kv_full = bar + 8;    // [kStages]
-  const uint32_t bar_kv_empty = bar + 24;  // [kStages]
-  const uint32_t bar_s_full = bar + 40;
-  const uint32_t bar_p_full = bar + 48;
-  const uint32_t bar_o_done = bar + 56;
-  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::kBar + 64);
+  const uint32_t bar_kv_empty = bar + 32;  // [kStages]
+  const uint32_t bar_s_full = bar + 56;    // MMA -> softmax: S(e) is in TMEM
+  const uint32_t bar_s_free = bar + 64;    // softmax -> MMA: S(e) has been read into registers (128 arrivals)
+  const uint32_t bar_p_full = bar + 72;    // softmax -> MMA: P(e) is in TMEM, O rescaled (128 arrivals)
+  const uint32_t bar_o_done = bar + 80;    // MMA -> softmax: PV(e) complete
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::kBar + 96);
 
   int64_t e0 = 0;
   int n_ent = p.NB;
@@ -74,6 +78,7 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
       mbar_init(bar_kv_empty + 8 * s, 1);
     }
     mbar_init(bar_s_full, 1);
+    mbar_init(bar_s_free, 128);
     mbar_init(bar_p_full, 128);
     mbar_init(bar_o_done, 1);
     fence_mbar_init();
@@ -96,14 +101,15 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
       mbar_arrive_expect_tx(bar_q, B * 128);
       tma_load_3d(sbase + L::kQ, &map_q, bar_q, 0, I * B, h);
       int Jn = p.row_ptr ? p.col_idx[e0] : 0;
+      int s = 0, ph = 0;
       for (int e = 0; e < n_ent; ++e) {
-        const int s = e % kStages, n = e / kStages;
         const int J = Jn;
         if (e + 1 < n_ent) Jn = p.row_ptr ? p.col_idx[e0 + e + 1] : e + 1;
-        mbar_wait(bar_kv_empty + 8 * s, (n & 1) ^ 1);
+        mbar_wait(bar_kv_empty + 8 * s, ph ^ 1);
         mbar_arrive_expect_tx(bar_kv_full + 8 * s, 2 * B * 128);
         tma_load_3d(sbase + L::kK + s * B * 128, &map_k, bar_kv_full + 8 * s, 0, J * B, h);
         tma_load_3d(sbase + L::kV + s * B * 128, &map_v, bar_kv_full + 8 * s, 0, J * B, h);
+        if (++s == kStages) { s = 0; ph ^= 1; }
       }
     }
   } else if (warp == 5) {
@@ -112,110 +118,119 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
       constexpr uint32_t idesc_qk = umma_idesc_bf16(B, false);
       constexpr uint32_t idesc_pv = umma_idesc_bf16(kD, true);
       const uint64_t qdesc = umma_desc_sw128(sbase + L::kQ);
-      const uint32_t tS = tmem, tO = tmem + kTmemO;
-      auto issue_qk = [&](int e) {
-        const int s = e % kStages, n = e / kStages;
-        mbar_wait(bar_kv_full + 8 * s, n & 1);
+      const uint32_t tS = tmem, tO = tmem + kTmemO, tP = tmem + kTmemP;
+      int sq = 0, phq = 0;  // stage / phase of the next QK
+      auto issue_qk = [&]() {
+        mbar_wait(bar_kv_full + 8 * sq, phq);
         tc_fence_after();
-        const uint64_t kdesc = umma_desc_sw128(sbase + L::kK + s * B * 128);
+        const uint64_t kdesc = umma_desc_sw128(sbase + L::kK + sq * B * 128);
 #pragma unroll
         for (int k = 0; k < kD / 16; ++k) umma_ss(tS, qdesc + 2 * k, kdesc + 2 * k, idesc_qk, k > 0);
         umma_commit(bar_s_full);
+        if (++sq == kStages) { sq = 0; phq ^= 1; }
       };
       mbar_wait(bar_q, 0);
-      issue_qk(0);
+      issue_qk();
+      int sv = 0;
       for (int e = 0; e < n_ent; ++e) {
-        const int s = e % kStages;
-        // P(e) is in smem and S has been read  ->  S may be overwritten by QK(e+1), then O += P(e) V(e)
+        if (e + 1 < n_ent) {
+          mbar_wait(bar_s_free, e & 1);  // S(e) is in registers -> overwrite it with S(e+1) while softmax(e) runs
+          issue_qk();
+        }
         mbar_wait(bar_p_full, e & 1);
         tc_fence_after();
-        if (e + 1 < n_ent) issue_qk(e + 1);
-        const uint64_t vdesc = umma_desc_sw128(sbase + L::kV + s * B * 128);
+        const uint64_t vdesc = umma_desc_sw128(sbase + L::kV + sv * B * 128);
 #pragma unroll
-        for (int kk = 0; kk < B / 16; ++kk) {
-          const uint64_t pdesc = umma_desc_sw128(sbase + L::kP + (kk / 4) * (128 * 128) + (kk % 4) * 32);
-          umma_ss(tO, pdesc, vdesc + (uint64_t)kk * 128, idesc_pv, (e > 0 || kk > 0) ? 1u : 0u);
-        }
-        umma_commit(bar_kv_empty + 8 * s);
+        for (int kk = 0; kk < B / 16; ++kk)
+          umma_ts(tO, tP + kk * 8, vdesc + (uint64_t)kk * 128, idesc_pv, (e > 0 || kk > 0) ? 1u : 0u);
+        umma_commit(bar_kv_empty + 8 * sv);
         umma_commit(bar_o_done);
+        if (++sv == kStages) sv = 0;
       }
     }
   } else {
     // ------------------------------------------------------------ softmax warps (thread r <-> q-row r)
     const int r = threadIdx.x;
     const uint32_t lane_off = (uint32_t)(warp * 32) << 16;
-    const uint32_t tS = tmem + lane_off, tO = tmem + lane_off + kTmemO;
+    const uint32_t tS = tmem + lane_off, tO = tmem + lane_off + kTmemO, tP = tmem + lane_off + kTmemP;
     const int tail = p.N - (p.NB - 1) * B;  // valid keys in the last k-block
     const int64_t tok = (int64_t)I * B + r;
     const bool row_valid = (r < B) && (tok < p.N);
-    float m = -INFINITY, l = 0.f;
     const float c = p.scale_log2;
+    const float lazy_raw = kLazyLog2 / c;  // threshold on the raw logits
+    float m = -INFINITY, l = 0.f;
     const int J_last = (n_ent > 0) ? (p.row_ptr ? p.col_idx[e0 + n_ent - 1] : p.NB - 1) : -1;
+    const bool last_is_tail = (J_last == p.NB - 1) && (tail < B);
 
     for (int e = 0; e < n_ent; ++e) {
-      const int ncols = (e == n_ent - 1 && J_last == p.NB - 1) ? tail : B;
+      uint32_t v[B];
       mbar_wait(bar_s_full, e & 1);
       tc_fence_after();
-      // pass 1: row max of the raw logits
-      float mx = -INFINITY;
-#pragma unroll 1
-      for (int cb = 0; cb < B; cb += 32) {
-        uint32_t v[32];
-        tmem_ld32(tS + cb, v);
-        tmem_ld_wait();
 #pragma unroll
-        for (int i = 0; i < 32; ++i)
-          if (cb + i < ncols) mx = fmaxf(mx, __uint_as_float(v[i]));
+      for (int cb = 0; cb < B; cb += 32) tmem_ld32(tS + cb, *reinterpret_cast<uint32_t(*)[32]>(&v[cb]));
+      tmem_ld_wait();
+      tc_fence_before();
+      mbar_arrive(bar_s_free);
+      if (e == n_ent - 1 && last_is_tail) {
+#pragma unroll
+        for (int i = 0; i < B; ++i)
+          if (i >= tail) v[i] = 0xff800000u;  // -inf
       }
-      const float m_new = fmaxf(m, mx);
-      const float alpha = ex2_approx((m - m_new) * c);
-      const float mc = m_new * c;
-      // PV(e-1) must be complete before P smem is overwritten and O is rescaled
+      // row max (3-input max)
+      float mx0 = __uint_as_float(v[0]), mx1 = __uint_as_float(v[1]);
+#pragma unroll
+      for (int i = 2; i < B; i += 4) {
+        mx0 = max3(mx0, __uint_as_float(v[i]), __uint_as_float(v[i + 1]));
+        if (i + 3 < B) mx1 = max3(mx1, __uint_as_float(v[i + 2]), __uint_as_float(v[i + 3]));
+      }
+      const float mx = fmaxf(mx0, mx1);
+      // lazy running max: move it only when some row of the warp grew by more than 2^8
+      float alpha = 1.f;
+      const bool moved = __any_sync(0xffffffffu, mx > m + lazy_raw);
+      if (moved) {
+        const float m_new = fmaxf(m, mx);
+        alpha = ex2_approx((m - m_new) * c);
+        m = m_new;
+      }
+      const float nmc = -m * c;
+      // p = exp2(s*c - m*c); row sum; pack to bf16
+      uint32_t pk[B / 2];
+      uint64_t acc0 = 0ull, acc1 = 0ull;  // two packed fp32x2 partial sums
+      const uint64_t c2 = pack_f32x2(c, c), nmc2 = pack_f32x2(nmc, nmc);
+#pragma unroll
+      for (int i = 0; i < B; i += 4) {
+        float x0, x1, x2, x3;
+        unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(v[i]), __uint_as_float(v[i + 1])), c2, nmc2), x0, x1);
+        unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(v[i + 2]), __uint_as_float(v[i + 3])), c2, nmc2), x2, x3);
+        x0 = ex2_approx(x0); x1 = ex2_approx(x1); x2 = ex2_approx(x2); x3 = ex2_approx(x3);
+        acc0 = add_f32x2(acc0, pack_f32x2(x0, x1));
+        acc1 = add_f32x2(acc1, pack_f32x2(x2, x3));
+        pk[i >> 1] = pack_bf16x2(x0, x1);
+        pk[(i >> 1) + 1] = pack_bf16x2(x2, x3);
+      }
+      float s0, s1, s2, s3;
+      unpack_f32x2(acc0, s0, s1);
+      unpack_f32x2(acc1, s2, s3);
+      l = l * alpha + ((s0 + s1) + (s2 + s3));
+      // PV(e-1) must be complete before P is overwritten and O is rescaled
       if (e > 0) {
         mbar_wait(bar_o_done, (e - 1) & 1);
         tc_fence_after();
-      }
-      // pass 2: p = exp2(s*c - m*c), row sum, P -> smem (K-major, 128B swizzle)
-      float sum = 0.f;
-#pragma unroll 1
-      for (int cb = 0; cb < B; cb += 32) {
-        uint32_t v[32];
-        tmem_ld32(tS + cb, v);
-        tmem_ld_wait();
-        uint32_t pk[16];
+        if (moved) {
 #pragma unroll
-        for (int i = 0; i < 32; i += 2) {
-          float p0 = (cb + i < ncols) ? ex2_approx(fmaf(__uint_as_float(v[i]), c, -mc)) : 0.f;
-          float p1 = (cb + i + 1 < ncols) ? ex2_approx(fmaf(__uint_as_float(v[i + 1]), c, -mc)) : 0.f;
-          sum += p0 + p1;
-          pk[i >> 1] = pack_bf16x2(p0, p1);
-        }
-        // keys cb..cb+31 of row r: atom = cb/64, 16-byte chunks ((cb%64)/8 .. +3), chunk index XOR (r%8)
-        const uint32_t rowbase = sbase + L::kP + (cb >> 6) * (128 * 128) + (r >> 3) * 1024 + (r & 7) * 128;
+          for (int cb = 0; cb < kD; cb += 32) {
+            uint32_t o[32];
+            tmem_ld32(tO + cb, o);
+            tmem_ld_wait();
 #pragma unroll
-        for (int q4 = 0; q4 < 4; ++q4) {
-          const uint32_t chunk = (uint32_t)(((cb & 63) >> 3) + q4) ^ (uint32_t)(r & 7);
-          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(rowbase + chunk * 16), "r"(pk[4 * q4]),
-                       "r"(pk[4 * q4 + 1]), "r"(pk[4 * q4 + 2]), "r"(pk[4 * q4 + 3])
-                       : "memory");
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+            tmem_st32(tO + cb, o);
+          }
         }
       }
-      l = l * alpha + sum;
-      m = m_new;
-      // rescale O (warp-uniform decision; tcgen05.ld/st are .sync.aligned)
-      if (e > 0 && __any_sync(0xffffffffu, alpha != 1.f)) {
-#pragma unroll 1
-        for (int cb = 0; cb < kD; cb += 32) {
-          uint32_t v[32];
-          tmem_ld32(tO + cb, v);
-          tmem_ld_wait();
 #pragma unroll
-          for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(__uint_as_float(v[i]) * alpha);
-          tmem_st32(tO + cb, v);
-        }
-        tmem_st_wait();
-      }
-      fence_proxy_async_smem();
+      for (int cb = 0; cb < B / 2; cb += 32) tmem_st32(tP + cb, *reinterpret_cast<uint32_t(*)[32]>(&pk[cb]));
+      tmem_st_wait();
       tc_fence_before();
       mbar_arrive(bar_p_full);
     }
@@ -262,7 +277,10 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 5) tmem_dealloc(tmem, kTmemCols);
+  if (warp == 5) {
+    __syncwarp();
+    tmem_dealloc(tmem, kTmemCols);
+  }
 }
 
 }  // namespace saf3r

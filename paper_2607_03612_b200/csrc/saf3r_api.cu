@@ -36,6 +36,9 @@ struct saf3r_ctx {
   bool sticky_cuda = false;
   int64_t launches = 0;
   std::vector<std::pair<MapKey, CUtensorMap>> maps;  // small LRU-less cache
+  // per-head list totals of the lists saf3r_select last wrote into a given row_ptr buffer (scheduling hint only)
+  struct LenHint { const int64_t *row_ptr; int32_t H, NB; int64_t len[SAF3R_MAX_HEADS]; };
+  std::vector<LenHint> hints;
 };
 
 static saf3r_status fail(saf3r_ctx *ctx, saf3r_status st, const std::string &msg) {
@@ -125,16 +128,19 @@ static WsLayout ws_layout(const SelGeom &g) {
   w.total = off;
   return w;
 }
-static int64_t total_entries(const SelGeom &g, const saf3r_head_cfg *cfg) {
+static int64_t total_entries(const SelGeom &g, const saf3r_head_cfg *cfg, int64_t *per_head = nullptr) {
   int64_t tot = 0;
   for (int h = 0; h < g.H; ++h) {
     const saf3r_head_cfg &c = cfg[h];
     const bool per_row = c.type == SAF3R_HEAD_STATIC && c.static_mode != SAF3R_STATIC_ANCHOR;
+    int64_t t = 0;
     if (per_row) {
-      for (int64_t I = 0; I < g.NB; ++I) tot += row_length(g, c, I);
+      for (int64_t I = 0; I < g.NB; ++I) t += row_length(g, c, I);
     } else {
-      tot += row_length(g, c, 0) * g.NB;
+      t = row_length(g, c, 0) * g.NB;
     }
+    if (per_head) per_head[h] = t;
+    tot += t;
   }
   return tot;
 }
@@ -209,7 +215,9 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
   if (!q || !k || !ws || !lists || !lists->row_ptr || !lists->col_idx) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
   if (((uintptr_t)q | (uintptr_t)k) & 15) return fail(ctx, SAF3R_ERR_INVALID_ARG, "q/k must be 16-byte aligned");
   const WsLayout w = ws_layout(g);
-  const int64_t need = total_entries(g, cfg);
+  saf3r_ctx::LenHint hint;
+  memset(&hint, 0, sizeof hint);
+  const int64_t need = total_entries(g, cfg, hint.len);
   if (ws_bytes < w.total || lists->capacity < need) {
     char buf[160];
     snprintf(buf, sizeof buf, "capacity: need %lld list entries (have %lld), %zu workspace bytes (have %zu)", (long long)need,
@@ -258,6 +266,14 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
   select_kernel<<<dim3((g.NB + R - 1) / R, g.H), 256, sm, st>>>(qt, kt, probe, lists->row_ptr, lists->col_idx, g, ca, R);
   ctx->launches += 1;
   CU_CHECK(cudaGetLastError());
+  hint.row_ptr = lists->row_ptr; hint.H = g.H; hint.NB = g.NB;
+  bool found = false;
+  for (auto &hh : ctx->hints)
+    if (hh.row_ptr == hint.row_ptr) { hh = hint; found = true; }
+  if (!found) {
+    if (ctx->hints.size() >= 32) ctx->hints.erase(ctx->hints.begin());
+    ctx->hints.push_back(hint);
+  }
   return SAF3R_OK;
 }
 
@@ -312,6 +328,20 @@ static saf3r_status attn_common(saf3r_ctx *ctx, const void *q, const void *k, co
   p.N = (int32_t)g.N; p.NB = g.NB; p.H = g.H;
   p.out_fp32 = out_is_fp32 ? 1 : 0;
   p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)shape->head_dim));
+  // heads with the longest lists first (list lengths are per-head nearly uniform; dense mode: identity)
+  {
+    const int64_t *head_len = nullptr;
+    if (lists)
+      for (auto &hh : ctx->hints)
+        if (hh.row_ptr == lists->row_ptr && hh.H == g.H && hh.NB == g.NB) head_len = hh.len;
+    int64_t len[SAF3R_MAX_HEADS];
+    for (int h = 0; h < g.H; ++h) len[h] = head_len ? head_len[h] : 0;
+    for (int h = 0; h < g.H; ++h) p.head_order[h] = (uint8_t)h;
+    for (int a = 1; a < g.H; ++a)  // insertion sort, descending, stable
+      for (int b = a; b > 0 && len[p.head_order[b - 1]] < len[p.head_order[b]]; --b) {
+        uint8_t t = p.head_order[b]; p.head_order[b] = p.head_order[b - 1]; p.head_order[b - 1] = t;
+      }
+  }
   cudaStream_t st = (cudaStream_t)stream_;
   dim3 grid(g.NB, g.H);
   if (g.B == 128)
