@@ -13,7 +13,7 @@ import os
 from dataclasses import dataclass
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libsaf3r.so")
+LIB_PATH = os.environ.get("SAF3R_LIB", os.path.join(HERE, "libsaf3r.so"))  # env override: kernel-variant experiments only
 
 MAX_HEADS = 64
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CAPACITY, ERR_CUDA = range(5)
