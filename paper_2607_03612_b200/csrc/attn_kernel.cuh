@@ -19,6 +19,10 @@
 #define SAF3R_SPLIT_128 80  // columns of a 128-wide tile whose exponentials use the MUFU (rest: FMA-pipe polynomial)
 #endif
 
+#ifndef SAF3R_MUFU_WARP0
+#define SAF3R_MUFU_WARP0 0  // first warp of the MUFU softmax group (the FMA group takes the other of warps 0-3 / 4-7)
+#endif
+
 namespace saf3r {
 
 struct AttnParams {
@@ -206,7 +210,7 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
   extern __shared__ __align__(1024) uint8_t smem[];
   using L = AttnSmem<B>;
   const uint32_t sbase = smem_u32(smem);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = threadIdx.x >> 5;
   const int I = blockIdx.x, h = p.head_order[blockIdx.y];
 
   const uint32_t bar = sbase + L::kBar;
@@ -329,7 +333,7 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
         }
       }
     }
-  } else if (warp < 4) {
+  } else if (warp >= SAF3R_MUFU_WARP0 && warp < SAF3R_MUFU_WARP0 + 4) {
     setmaxnreg_inc<kRegsMufu>();
     softmax_half<B, 0, L::kSplit, false>(p, smem, tmem, n_ent, e0, h, I, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
   } else {

@@ -115,15 +115,14 @@ static const char *validate_cfg(const SelGeom &g, const saf3r_head_cfg *cfg) {
 }
 
 struct WsLayout {
-  size_t qt, kt, qbar, rowlen, probe, total;
+  size_t qt, kt, qpart, probe, total;
 };
 static WsLayout ws_layout(const SelGeom &g) {
   WsLayout w;
   size_t off = 0;
   w.qt = off; off = align256(off + (size_t)g.H * g.NB * 64 * sizeof(float));
   w.kt = off; off = align256(off + (size_t)g.H * g.NB * 64 * sizeof(float));
-  w.qbar = off; off = align256(off + (size_t)g.H * 64 * sizeof(float));
-  w.rowlen = off; off = align256(off + (size_t)g.H * g.NB * sizeof(int32_t));
+  w.qpart = off; off = align256(off + (size_t)g.H * ((g.NB + 7) / 8) * 64 * sizeof(float));
   w.probe = off; off = align256(off + (size_t)g.H * g.NB * sizeof(int32_t));
   w.total = off;
   return w;
@@ -178,7 +177,7 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
   e = cudaFuncSetAttribute(saf3r_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e != cudaSuccess) {
     fprintf(stderr, "saf3r_create: cudaFuncSetAttribute failed: %s\n", cudaGetErrorString(e));
     delete ctx;
@@ -226,36 +225,53 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
   }
   cudaStream_t st = (cudaStream_t)stream_;
   uint8_t *wsb = (uint8_t *)ws;
-  float *qt = (float *)(wsb + w.qt), *kt = (float *)(wsb + w.kt), *qbar = (float *)(wsb + w.qbar);
-  int32_t *rowlen = (int32_t *)(wsb + w.rowlen), *probe = (int32_t *)(wsb + w.probe);
+  float *qt = (float *)(wsb + w.qt), *kt = (float *)(wsb + w.kt) /* transposed [H][64][NB] */, *qpart = (float *)(wsb + w.qpart);
+  int32_t *probe = (int32_t *)(wsb + w.probe);
 
   HeadCfgArray ca;
   memset(&ca, 0, sizeof ca);
-  PoolFlags pf;
-  memset(&pf, 0, sizeof pf);
-  bool any_pool = false, any_probe = false, any_block = false;
+  PoolJobs jobs;
+  memset(&jobs, 0, sizeof jobs);
+  ProbeHeads ph;
+  memset(&ph, 0, sizeof ph);
+  RowPtrPlan plan;
+  memset(&plan, 0, sizeof plan);
+  bool any_block = false;
+  int64_t base = 0;
   for (int h = 0; h < g.H; ++h) {
     ca.c[h] = cfg[h];
-    if (cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK) { pf.f[h] = 3; any_probe = true; }
-    if (cfg[h].type == SAF3R_HEAD_BLOCK_TOPK) { pf.f[h] = 3 | (cfg[h].score_mode == SAF3R_SCORE_COSINE ? 4 : 0); any_block = true; }
-    any_pool |= pf.f[h] != 0;
+    const bool probe = cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK, block = cfg[h].type == SAF3R_HEAD_BLOCK_TOPK;
+    if (probe || block) {
+      for (int which = 0; which < 2; ++which) {
+        jobs.head[jobs.n] = (uint8_t)h;
+        jobs.which[jobs.n] = (uint8_t)which;
+        jobs.cosine[jobs.n] = (uint8_t)(block && cfg[h].score_mode == SAF3R_SCORE_COSINE);
+        jobs.part[jobs.n] = (uint8_t)(probe && which == 0);
+        ++jobs.n;
+      }
+    }
+    if (probe) ph.head[ph.n++] = (uint8_t)h;
+    any_block |= block;
+    const bool per_row = cfg[h].type == SAF3R_HEAD_STATIC && cfg[h].static_mode != SAF3R_STATIC_ANCHOR;
+    plan.const_len[h] = per_row ? -1 : (int32_t)row_length(g, cfg[h], 0);
+    plan.head_base[h] = base;
+    base += hint.len[h];
   }
-  const int64_t rows = (int64_t)g.H * g.NB;
-  rowlen_kernel<<<(unsigned)((rows + 255) / 256), 256, 0, st>>>(rowlen, g, ca);
-  scan_kernel<<<1, 1024, 0, st>>>(rowlen, lists->row_ptr, rows);
-  ctx->launches += 2;
-  if (any_pool) {
-    pool_kernel<<<dim3(g.NB, g.H, 2), 256, 0, st>>>((const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, g, pf);
+  plan.head_base[g.H] = base;
+  // launch 1: pooling (one warp per token block of every tensor a rule reads) + one row_ptr CTA per head
+  const int pool_ctas = jobs.n * ((g.NB + 7) / 8);
+  pool_rowptr_kernel<<<pool_ctas + g.H, 256, 0, st>>>((const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart,
+                                                     lists->row_ptr, g, jobs, plan, ca, pool_ctas);
+  ctx->launches += 1;
+  // launch 2: probe heads (qbar, probe scores, top-n)
+  if (ph.n > 0) {
+    const size_t sm = (size_t)g.NB * 4 + 256 * 4;
+    if (sm > 200 * 1024) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the probe kernel");
+    probe_kernel<<<ph.n, 1024, sm, st>>>(qpart, kt, probe, g, ca, ph);
     ctx->launches += 1;
   }
-  if (any_probe) {
-    qbar_kernel<<<g.H, 256, 0, st>>>(qt, qbar, g, ca);
-    const size_t sm = (size_t)g.NB * 4 + 256 * 4;
-    if (sm > 220 * 1024) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the probe kernel");
-    probe_kernel<<<g.H, 256, sm, st>>>(kt, qbar, probe, g, ca);
-    ctx->launches += 2;
-  }
-  int R = 8;
+  // launch 3: per-row emit / score + select
+  int R = 16;
   size_t sm = 0;
   if (any_block) {
     const size_t budget = 220 * 1024 - 8 * 256 * 4;

@@ -1,8 +1,8 @@
 // Online pattern adaptation at block granularity (steps a-1..a-3 of DESIGN.md):
-//   pool_kernel      Q,K bf16 -> Qtilde,Ktilde fp32 block means (HBM-bound stream)
-//   qbar_kernel      qbar = (1/N) sum_t q_t from the pooled block means
-//   rowlen_kernel    closed-form list length of every (head, q-block) row;  scan_kernel -> row_ptr
-//   probe_kernel     p[J] = qbar . Ktilde_J / sqrt(D), top-n -> one shared list per QUERY_PROBE head
+//   pool_rowptr_kernel  Q,K bf16 -> Qtilde,Ktilde fp32 block means (HBM-bound stream, one warp per block) and, in extra CTAs
+//                       of the same launch, row_ptr from the closed-form row lengths
+//   probe_kernel        qbar = (1/N) sum_t q_t from the pooled block means, p[J] = qbar . Ktilde_J / sqrt(D),
+//                       top-n -> one shared list per QUERY_PROBE head
 //   select_kernel    per (head, q-block): closed-form emit, probe-list copy, or score row + top-n / per-frame top-k
 #pragma once
 #include <cuda_runtime.h>
@@ -102,113 +102,154 @@ __host__ __device__ inline int64_t row_length(const SelGeom &g, const saf3r_head
   return closed_form_row(g, c, I, [](int64_t) {});
 }
 
-// ------------------------------------------------------------------------------------------------ pool
-// grid (NB, H, 2): z = 0 pools Q, z = 1 pools K.  256 threads: 8 threads per token row (16 B each), 32 rows per pass.
-// flags[h] bit0: pool Q, bit1: pool K, bit2: cosine (L2-normalise each token first).
-struct PoolFlags { uint8_t f[SAF3R_MAX_HEADS]; };
+// ------------------------------------------------------------------------------------------------ pool + row_ptr
+// One launch, two kinds of CTA (256 threads):
+//   blockIdx.x <  pool_ctas : 8 warps, ONE WARP PER TOKEN BLOCK.  job j = (tensor, head) pairs that the head's rule reads
+//                            (host-built list), warp w -> (job = w / NB, J = w % NB).  A warp streams its block's
+//                            B x 128 B with 16-byte loads (lane = 16-byte chunk (l&7) of rows (l>>3) + 4i, eight loads in
+//                            flight), accumulates in fp32, folds the four row groups with shuffles and writes the
+//                            64-float mean.  No shared memory, no block barrier.
+//   blockIdx.x >= pool_ctas : one CTA per head writes that head's row_ptr entries: head_base + I*len for heads whose
+//                            rows all have the same length, a block scan of the closed-form lengths otherwise.
+struct PoolJobs {
+  int32_t n;                            // number of (tensor, head) jobs
+  uint8_t head[2 * SAF3R_MAX_HEADS];
+  uint8_t which[2 * SAF3R_MAX_HEADS];   // 0 = Q, 1 = K
+  uint8_t cosine[2 * SAF3R_MAX_HEADS];  // L2-normalise each token first
+  uint8_t part[2 * SAF3R_MAX_HEADS];    // also write per-CTA token sums (Q of a QUERY_PROBE head, for qbar)
+};
+struct RowPtrPlan {
+  int64_t head_base[SAF3R_MAX_HEADS + 1];  // first entry of each head (host closed form); [H] = total
+  int32_t const_len[SAF3R_MAX_HEADS];      // >= 0: every row of the head has this length; -1: per-row closed form
+};
 
-__global__ void __launch_bounds__(256) pool_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
-                                                   float *__restrict__ qt, float *__restrict__ kt, SelGeom g, PoolFlags flags) {
-  const int J = blockIdx.x, h = blockIdx.y, which = blockIdx.z;
-  const uint8_t fl = flags.f[h];
-  if (!((fl >> which) & 1)) return;
-  const bool cosine = (fl >> 2) & 1;
-  const __nv_bfloat16 *src = (which ? k : q) + (int64_t)h * g.stride_head;
-  float *dst = (which ? kt : qt) + ((int64_t)h * g.NB + J) * 64;
+__device__ __forceinline__ uint4 ld_stream_16(const void *p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+
+__global__ void __launch_bounds__(256) pool_rowptr_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
+                                                          float *__restrict__ qt, float *__restrict__ ktT, float *__restrict__ qpart,
+                                                          int64_t *__restrict__ row_ptr, SelGeom g, PoolJobs jobs, RowPtrPlan plan,
+                                                          HeadCfgArray cfg, int pool_ctas) {
+  if ((int)blockIdx.x >= pool_ctas) {
+    // ---------------------------------------------------------------- row_ptr of one head
+    const int h = blockIdx.x - pool_ctas;
+    int64_t *rp = row_ptr + (int64_t)h * g.NB;
+    const int64_t base = plan.head_base[h];
+    if (plan.const_len[h] >= 0) {
+      for (int I = threadIdx.x; I < g.NB; I += 256) rp[I] = base + (int64_t)I * plan.const_len[h];
+    } else {
+      __shared__ int64_t sums[256];
+      const int per = (g.NB + 255) / 256;
+      const int a = min(g.NB, (int)threadIdx.x * per), b = min(g.NB, a + per);
+      int64_t s = 0;
+      for (int I = a; I < b; ++I) s += row_length(g, cfg.c[h], I);
+      sums[threadIdx.x] = s;
+      __syncthreads();
+      for (int off = 1; off < 256; off <<= 1) {
+        int64_t v = (int)threadIdx.x >= off ? sums[threadIdx.x - off] : 0;
+        __syncthreads();
+        sums[threadIdx.x] += v;
+        __syncthreads();
+      }
+      int64_t run = base + (threadIdx.x ? sums[threadIdx.x - 1] : 0);
+      for (int I = a; I < b; ++I) {
+        rp[I] = run;
+        run += row_length(g, cfg.c[h], I);
+      }
+    }
+    if (h == g.H - 1 && threadIdx.x == 0) row_ptr[(int64_t)g.H * g.NB] = plan.head_base[g.H];
+    return;
+  }
+  // ------------------------------------------------------------------ pool: one warp per token block
+  // CTA c of a job covers blocks 8c .. 8c+7 (jobs are padded to a multiple of 8 blocks, so a CTA never straddles jobs)
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int ctas_per_job = (g.NB + 7) / 8;
+  const int job = blockIdx.x / ctas_per_job, cta_in_job = blockIdx.x % ctas_per_job;
+  const int J = cta_in_job * 8 + warp;
+  __shared__ float qsum[8][64];
+  const bool want_part = jobs.part[job] != 0;  // Q of a QUERY_PROBE head: also emit this CTA's token sum (for qbar)
+  if (J >= g.NB) {
+    if (want_part) {
+      qsum[warp][lane] = 0.f;
+      qsum[warp][lane + 32] = 0.f;
+      __syncthreads();
+    }
+    return;
+  }
+  const int h = jobs.head[job], which = jobs.which[job];
+  const bool cosine = jobs.cosine[job] != 0;
   const int64_t t0 = (int64_t)J * g.B;
   const int cnt = (int)i64min(g.B, g.N - t0);
-  const int sub = threadIdx.x & 7, rg = threadIdx.x >> 3;  // 16-byte chunk within the row, row group
+  const int sub = lane & 7, rg = lane >> 3;
+  const __nv_bfloat16 *src = (which ? k : q) + (int64_t)h * g.stride_head + t0 * g.stride_token + sub * 8;
   float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  constexpr int kMaxPass = 4;  // B <= 128
-  uint4 raw[kMaxPass];
+  for (int r0 = 0; r0 < g.B; r0 += 32) {  // 8 loads of 16 B in flight per lane (rows r0 + rg + 4i)
+    uint4 raw[8];
 #pragma unroll
-  for (int ps = 0; ps < kMaxPass; ++ps) {
-    const int r = ps * 32 + rg;
-    raw[ps] = make_uint4(0, 0, 0, 0);
-    if (r < cnt) raw[ps] = __ldg(reinterpret_cast<const uint4 *>(src + (t0 + r) * g.stride_token) + sub);
-  }
-#pragma unroll
-  for (int ps = 0; ps < kMaxPass; ++ps) {
-    const uint32_t w[4] = {raw[ps].x, raw[ps].y, raw[ps].z, raw[ps].w};
-    float v[8];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      v[2 * i] = __uint_as_float(w[i] << 16);
-      v[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
-    }
-    float inv = 1.f;
-    if (cosine) {
-      float ss = 0.f;
-#pragma unroll
-      for (int i = 0; i < 8; ++i) ss = fmaf(v[i], v[i], ss);
-      ss += __shfl_xor_sync(0xffffffffu, ss, 1);
-      ss += __shfl_xor_sync(0xffffffffu, ss, 2);
-      ss += __shfl_xor_sync(0xffffffffu, ss, 4);
-      const float nrm = sqrtf(ss);
-      inv = nrm < 1e-20f ? 0.f : 1.f / nrm;
+    for (int i = 0; i < 8; ++i) {
+      const int r = r0 + rg + 4 * i;
+      raw[i] = make_uint4(0, 0, 0, 0);
+      if (r < cnt) raw[i] = ld_stream_16(src + (int64_t)r * g.stride_token);
     }
 #pragma unroll
-    for (int i = 0; i < 8; ++i) acc[i] = fmaf(v[i], inv, acc[i]);
-  }
-  __shared__ float part[32][65];
+    for (int i = 0; i < 8; ++i) {
+      const uint32_t w[4] = {raw[i].x, raw[i].y, raw[i].z, raw[i].w};
+      float v[8];
 #pragma unroll
-  for (int i = 0; i < 8; ++i) part[rg][sub * 8 + i] = acc[i];
-  __syncthreads();
-  if (threadIdx.x < 64) {
-    float s = 0.f;
+      for (int c = 0; c < 4; ++c) {
+        v[2 * c] = __uint_as_float(w[c] << 16);
+        v[2 * c + 1] = __uint_as_float(w[c] & 0xFFFF0000u);
+      }
+      float inv = 1.f;
+      if (cosine) {
+        float ss = 0.f;
 #pragma unroll
-    for (int r = 0; r < 32; ++r) s += part[r][threadIdx.x];
-    dst[threadIdx.x] = s / (float)cnt;
+        for (int c = 0; c < 8; ++c) ss = fmaf(v[c], v[c], ss);
+        ss += __shfl_xor_sync(0xffffffffu, ss, 1);
+        ss += __shfl_xor_sync(0xffffffffu, ss, 2);
+        ss += __shfl_xor_sync(0xffffffffu, ss, 4);
+        const float nrm = sqrtf(ss);
+        inv = nrm < 1e-20f ? 0.f : 1.f / nrm;
+      }
+#pragma unroll
+      for (int c = 0; c < 8; ++c) acc[c] = fmaf(v[c], inv, acc[c]);
+    }
   }
-}
-
-// ------------------------------------------------------------------------------------------------ qbar
-// grid (H); 256 threads = 4 groups x 64 dims.  qbar[d] = (1/N) sum_J c_J * Qtilde[J][d].
-__global__ void __launch_bounds__(256) qbar_kernel(const float *__restrict__ qt, float *__restrict__ qbar, SelGeom g,
-                                                   HeadCfgArray cfg) {
-  const int h = blockIdx.x;
-  if (cfg.c[h].type != SAF3R_HEAD_QUERY_PROBE_TOPK) return;
-  const int d = threadIdx.x & 63, grp = threadIdx.x >> 6;
-  float s = 0.f;
-  for (int J = grp; J < g.NB; J += 4) {
-    const float cnt = (float)i64min(g.B, g.N - (int64_t)J * g.B);
-    s = fmaf(qt[((int64_t)h * g.NB + J) * 64 + d], cnt, s);
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 8);
+    acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 16);
   }
-  __shared__ float part[4][64];
-  part[grp][d] = s;
-  __syncthreads();
-  if (grp == 0) qbar[h * 64 + d] = (part[0][d] + part[1][d] + part[2][d] + part[3][d]) / (float)g.N;
-}
-
-// ------------------------------------------------------------------------------------------------ row lengths + scan
-__global__ void rowlen_kernel(int32_t *__restrict__ rowlen, SelGeom g, HeadCfgArray cfg) {
-  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (r >= (int64_t)g.H * g.NB) return;
-  const int h = (int)(r / g.NB);
-  rowlen[r] = (int32_t)row_length(g, cfg.c[h], r % g.NB);
-}
-
-// single CTA, 1024 threads: exclusive scan of rowlen[n] into row_ptr[n+1] (int64)
-__global__ void __launch_bounds__(1024) scan_kernel(const int32_t *__restrict__ rowlen, int64_t *__restrict__ row_ptr, int64_t n) {
-  __shared__ int64_t sums[1024];
-  const int64_t per = (n + 1023) / 1024;
-  const int64_t a = i64min(n, threadIdx.x * per), b = i64min(n, a + per);
-  int64_t s = 0;
-  for (int64_t i = a; i < b; ++i) s += rowlen[i];
-  sums[threadIdx.x] = s;
-  __syncthreads();
-  for (int off = 1; off < 1024; off <<= 1) {  // Hillis-Steele inclusive scan
-    int64_t v = threadIdx.x >= off ? sums[threadIdx.x - off] : 0;
+  const float invc = 1.f / (float)cnt;
+  if (rg == 0) {
+    if (which == 0) {  // Qtilde row-major [H][NB][64]
+      float4 *dst = reinterpret_cast<float4 *>(qt + ((int64_t)h * g.NB + J) * 64 + sub * 8);
+      dst[0] = make_float4(acc[0] * invc, acc[1] * invc, acc[2] * invc, acc[3] * invc);
+      dst[1] = make_float4(acc[4] * invc, acc[5] * invc, acc[6] * invc, acc[7] * invc);
+    } else {  // Ktilde TRANSPOSED [H][64][NB]: the score kernels read it coalesced over J
+#pragma unroll
+      for (int c = 0; c < 8; ++c) ktT[((int64_t)h * 64 + sub * 8 + c) * g.NB + J] = acc[c] * invc;
+    }
+  }
+  if (want_part) {
+    if (rg == 0) {
+#pragma unroll
+      for (int c = 0; c < 8; ++c) qsum[warp][sub * 8 + c] = acc[c];
+    }
     __syncthreads();
-    sums[threadIdx.x] += v;
-    __syncthreads();
+    if (warp == 0) {  // warp 0 always owns a real block (J = 8c < NB)
+#pragma unroll
+      for (int d = lane; d < 64; d += 32) {
+        float t = 0.f;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) t += qsum[w][d];
+        qpart[((int64_t)h * ctas_per_job + cta_in_job) * 64 + d] = t;
+      }
+    }
   }
-  int64_t run = threadIdx.x ? sums[threadIdx.x - 1] : 0;
-  for (int64_t i = a; i < b; ++i) {
-    row_ptr[i] = run;
-    run += rowlen[i];
-  }
-  if (threadIdx.x == 1023) row_ptr[n] = sums[1023];
 }
 
 // ------------------------------------------------------------------------------------------------ warp-level top-n
@@ -310,29 +351,39 @@ __device__ inline void warp_per_frame_emit(const float *s, const SelGeom &g, int
 }
 
 // ------------------------------------------------------------------------------------------------ probe
-// grid (H), 256 threads, dynamic smem: NB floats + 256 uint32.  Writes the shared list of a QUERY_PROBE head to
-// probe_list[h][0..n).
-__global__ void __launch_bounds__(256) probe_kernel(const float *__restrict__ kt, const float *__restrict__ qbar,
-                                                    int32_t *__restrict__ probe_list, SelGeom g, HeadCfgArray cfg) {
-  const int h = blockIdx.x;
-  if (cfg.c[h].type != SAF3R_HEAD_QUERY_PROBE_TOPK) return;
+// grid (number of QUERY_PROBE heads), 1024 threads, dynamic smem: NB floats + 256 uint32.  qbar (16 row groups x 64 dims,
+// fixed summation order), probe scores, then warp 0 radix-selects.  Writes the head's shared list to probe_list[h][0..n).
+struct ProbeHeads { int32_t n; uint8_t head[SAF3R_MAX_HEADS]; };
+
+__global__ void __launch_bounds__(1024) probe_kernel(const float *__restrict__ qpart, const float *__restrict__ ktT,
+                                                     int32_t *__restrict__ probe_list, SelGeom g, HeadCfgArray cfg, ProbeHeads ph) {
+  const int h = ph.head[blockIdx.x];
   extern __shared__ float sm[];
   float *s = sm;
   uint32_t *hist = reinterpret_cast<uint32_t *>(sm + g.NB);
+  __shared__ float part[16][64];
   __shared__ float qb[64];
-  if (threadIdx.x < 64) qb[threadIdx.x] = qbar[h * 64 + threadIdx.x];
-  __syncthreads();
-  for (int J = threadIdx.x; J < g.NB; J += blockDim.x) {
-    const float4 *kr = reinterpret_cast<const float4 *>(kt + ((int64_t)h * g.NB + J) * 64);
-    float acc = 0.f;
+  {
+    const int d = threadIdx.x & 63, grp = threadIdx.x >> 6;
+    const int nparts = (g.NB + 7) / 8;
+    const float *base = qpart + (int64_t)h * nparts * 64 + d;
+    float a0 = 0.f;
+    for (int c = grp; c < nparts; c += 16) a0 += base[(int64_t)c * 64];
+    part[grp][d] = a0;
+    __syncthreads();
+    if (threadIdx.x < 64) {
+      float t = 0.f;
 #pragma unroll
-    for (int d4 = 0; d4 < 16; ++d4) {
-      const float4 kv = __ldg(kr + d4);
-      acc = fmaf(qb[4 * d4], kv.x, acc);
-      acc = fmaf(qb[4 * d4 + 1], kv.y, acc);
-      acc = fmaf(qb[4 * d4 + 2], kv.z, acc);
-      acc = fmaf(qb[4 * d4 + 3], kv.w, acc);
+      for (int i = 0; i < 16; ++i) t += part[i][threadIdx.x];
+      qb[threadIdx.x] = t / (float)g.N;
     }
+    __syncthreads();
+  }
+  for (int J = threadIdx.x; J < g.NB; J += blockDim.x) {
+    const float *kc = ktT + (int64_t)h * 64 * g.NB + J;
+    float acc = 0.f;
+#pragma unroll 16
+    for (int d = 0; d < 64; ++d) acc = fmaf(qb[d], __ldg(kc + (int64_t)d * g.NB), acc);
     s[J] = acc * 0.125f;
   }
   __syncthreads();
@@ -340,9 +391,9 @@ __global__ void __launch_bounds__(256) probe_kernel(const float *__restrict__ kt
 }
 
 // ------------------------------------------------------------------------------------------------ select
-// grid (ceil(NB/R), H), 256 threads (8 warps), R <= 8 rows per CTA.  dynamic smem: R*NB floats (scores) + R*64 floats
+// grid (ceil(NB/R), H), 256 threads (8 warps), R <= 16 rows per CTA (Ktilde is re-read once per CTA, so more rows = less L2 traffic).  dynamic smem: R*NB floats (scores) + R*64 floats
 // (Qtilde rows) + 8*256 uint32 (histograms).
-__global__ void __launch_bounds__(256) select_kernel(const float *__restrict__ qt, const float *__restrict__ kt,
+__global__ void __launch_bounds__(256) select_kernel(const float *__restrict__ qt, const float *__restrict__ ktT,
                                                      const int32_t *__restrict__ probe_list, const int64_t *__restrict__ row_ptr,
                                                      int32_t *__restrict__ col_idx, SelGeom g, HeadCfgArray cfg, int R) {
   const int h = blockIdx.y;
@@ -364,6 +415,19 @@ __global__ void __launch_bounds__(256) select_kernel(const float *__restrict__ q
       } else if (c.type == SAF3R_HEAD_UNIFORM_STRIDE && c.stride >= 1) {
         const int n = (g.NB - c.offset + c.stride - 1) / c.stride;
         for (int i = lane; i < n; i += 32) out[i] = c.offset + i * c.stride;
+      } else if (c.type == SAF3R_HEAD_UNIFORM_STRIDE) {  // keep_blocks form (n <= NB, so the indices are distinct)
+        for (int i = lane; i < c.keep_blocks; i += 32) out[i] = (int32_t)(((int64_t)i * g.NB) / c.keep_blocks);
+      } else if (c.type == SAF3R_HEAD_STATIC && c.static_mode != SAF3R_STATIC_POSITION_BAND) {  // one contiguous range
+        int64_t lo, hi;
+        if (c.static_mode == SAF3R_STATIC_ANCHOR) {
+          lo = ((int64_t)c.anchor_frame * g.T) / g.B;
+          hi = (((int64_t)c.anchor_frame + 1) * g.T - 1) / g.B;
+        } else {
+          const int64_t t0 = I * g.B, t1 = i64min(t0 + g.B, g.N);
+          lo = ((t0 / g.T) * g.T) / g.B;
+          hi = (((t1 - 1) / g.T + 1) * g.T - 1) / g.B;
+        }
+        for (int64_t J = lo + lane; J <= hi; J += 32) out[J - lo] = (int32_t)J;
       } else if (lane == 0) {
         int64_t w = 0;
         closed_form_row(g, c, I, [&](int64_t J) { out[w++] = (int32_t)J; });
@@ -380,12 +444,9 @@ __global__ void __launch_bounds__(256) select_kernel(const float *__restrict__ q
   const float cs = c.score_mode == SAF3R_SCORE_COSINE ? 1.f : 0.125f;
   for (int J = threadIdx.x; J < g.NB; J += blockDim.x) {
     float kv[64];
-    const float4 *kr = reinterpret_cast<const float4 *>(kt + ((int64_t)h * g.NB + J) * 64);
+    const float *kc = ktT + (int64_t)h * 64 * g.NB + J;
 #pragma unroll
-    for (int d4 = 0; d4 < 16; ++d4) {
-      const float4 t = __ldg(kr + d4);
-      kv[4 * d4] = t.x; kv[4 * d4 + 1] = t.y; kv[4 * d4 + 2] = t.z; kv[4 * d4 + 3] = t.w;
-    }
+    for (int d = 0; d < 64; ++d) kv[d] = __ldg(kc + (int64_t)d * g.NB);
     for (int r = 0; r < rows; ++r) {
       const float4 *qr = reinterpret_cast<const float4 *>(qrows + r * 64);
       float acc = 0.f;
