@@ -69,7 +69,9 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
   constexpr int kHalf = kFma ? 1 : 0;
   const int r = threadIdx.x & 127;
   const int pair_bar = 1 + (r >> 5);  // named barrier shared by the two warps that own these 32 rows
-  const uint32_t lane_off = (uint32_t)(r & ~31) << 16;
+  // TMEM lane block of this warp; the shuffle makes it warp-uniform by construction so that ptxas keeps the tcgen05.ld/st
+  // addresses in uniform registers instead of re-deriving them (R2UR) every iteration
+  const uint32_t lane_off = (uint32_t)(__shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0) & 3) << 21;
   const uint32_t tS = tmem + lane_off + C0, tO = tmem + lane_off + kTmemO + 32 * kHalf, tP = tmem + lane_off + kTmemP + C0 / 2;
   float *smax = reinterpret_cast<float *>(smem + L::kMax);
   float *ssum = reinterpret_cast<float *>(smem + L::kSum);

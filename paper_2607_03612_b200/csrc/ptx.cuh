@@ -19,17 +19,18 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-// Blocks until the phase with the given parity completes.  try_wait suspends the thread in hardware for up to the
-// time hint, so waiting warps do not burn issue slots that the softmax warps need.
+// Blocks until the phase with the given parity completes.  try_wait suspends the thread in hardware for a
+// system-dependent time, so waiting warps burn few issue slots (the variant with an explicit time hint compiles to a
+// longer PHASECHK / NANOSLEEP / TRYWAIT loop and measured slightly slower).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "WAIT_LOOP:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
       "@p bra WAIT_DONE;\n\t"
       "bra WAIT_LOOP;\n\t"
       "WAIT_DONE:\n\t}" ::"r"(bar),
-      "r"(parity), "r"(0x989680u)
+      "r"(parity)
       : "memory");
 }
 

@@ -35,6 +35,7 @@ struct saf3r_ctx {
   std::string err;
   bool sticky_cuda = false;
   int64_t launches = 0;
+  uint32_t *done_dev = nullptr;  // [SAF3R_MAX_HEADS] last-CTA-done counters of the pool kernel; zero between calls
   std::vector<std::pair<MapKey, CUtensorMap>> maps;  // small LRU-less cache
   // per-head list totals of the lists saf3r_select last wrote into a given row_ptr buffer (scheduling hint only)
   struct LenHint { const int64_t *row_ptr; int32_t H, NB; int64_t len[SAF3R_MAX_HEADS]; };
@@ -177,7 +178,9 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
   e = cudaFuncSetAttribute(saf3r_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(pool_rowptr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaMalloc(&ctx->done_dev, SAF3R_MAX_HEADS * sizeof(uint32_t));
+  if (e == cudaSuccess) e = cudaMemset(ctx->done_dev, 0, SAF3R_MAX_HEADS * sizeof(uint32_t));
   if (e != cudaSuccess) {
     fprintf(stderr, "saf3r_create: cudaFuncSetAttribute failed: %s\n", cudaGetErrorString(e));
     delete ctx;
@@ -187,7 +190,11 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
   return SAF3R_OK;
 }
 
-void saf3r_destroy(saf3r_ctx *ctx) { delete ctx; }
+void saf3r_destroy(saf3r_ctx *ctx) {
+  if (!ctx) return;
+  if (ctx->done_dev) cudaFree(ctx->done_dev);
+  delete ctx;
+}
 
 const char *saf3r_last_error(const saf3r_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 
@@ -232,52 +239,51 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
   memset(&ca, 0, sizeof ca);
   PoolJobs jobs;
   memset(&jobs, 0, sizeof jobs);
-  ProbeHeads ph;
-  memset(&ph, 0, sizeof ph);
   RowPtrPlan plan;
   memset(&plan, 0, sizeof plan);
-  bool any_block = false;
+  bool any_block = false, any_probe = false;
   int64_t base = 0;
   for (int h = 0; h < g.H; ++h) {
     ca.c[h] = cfg[h];
-    const bool probe = cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK, block = cfg[h].type == SAF3R_HEAD_BLOCK_TOPK;
-    if (probe || block) {
-      for (int which = 0; which < 2; ++which) {
-        jobs.head[jobs.n] = (uint8_t)h;
-        jobs.which[jobs.n] = (uint8_t)which;
-        jobs.cosine[jobs.n] = (uint8_t)(block && cfg[h].score_mode == SAF3R_SCORE_COSINE);
-        jobs.part[jobs.n] = (uint8_t)(probe && which == 0);
-        ++jobs.n;
-      }
-    }
-    if (probe) ph.head[ph.n++] = (uint8_t)h;
-    any_block |= block;
+    any_block |= cfg[h].type == SAF3R_HEAD_BLOCK_TOPK;
+    any_probe |= cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK;
     const bool per_row = cfg[h].type == SAF3R_HEAD_STATIC && cfg[h].static_mode != SAF3R_STATIC_ANCHOR;
     plan.const_len[h] = per_row ? -1 : (int32_t)row_length(g, cfg[h], 0);
     plan.head_base[h] = base;
     base += hint.len[h];
   }
   plan.head_base[g.H] = base;
-  // launch 1: pooling (one warp per token block of every tensor a rule reads) + one row_ptr CTA per head
+  // pool jobs: QUERY_PROBE heads first (their probe runs in the last pool CTA of the head, under the other heads' pooling)
+  for (int pass = 0; pass < 2; ++pass)
+    for (int h = 0; h < g.H; ++h) {
+      const bool probe = cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK, block = cfg[h].type == SAF3R_HEAD_BLOCK_TOPK;
+      if (!(pass == 0 ? probe : block)) continue;
+      for (int which = 0; which < 2; ++which) {
+        jobs.head[jobs.n] = (uint8_t)h;
+        jobs.which[jobs.n] = (uint8_t)which;
+        jobs.cosine[jobs.n] = (uint8_t)(block && cfg[h].score_mode == SAF3R_SCORE_COSINE);
+        jobs.probe[jobs.n] = (uint8_t)probe;
+        ++jobs.n;
+      }
+    }
+  // launch 1: pooling (one warp per token block of every tensor a rule reads; the last CTA of a QUERY_PROBE head also runs
+  // its probe) + one row_ptr CTA per head
   const int pool_ctas = jobs.n * ((g.NB + 7) / 8);
-  pool_rowptr_kernel<<<pool_ctas + g.H, 256, 0, st>>>((const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart,
-                                                     lists->row_ptr, g, jobs, plan, ca, pool_ctas);
+  const size_t pool_sm = any_probe ? (size_t)g.NB * 4 : 0;
+  if (pool_sm > 200 * 1024) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the probe stage");
+  pool_rowptr_kernel<<<pool_ctas + g.H, 256, pool_sm, st>>>((const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart, probe,
+                                                           lists->row_ptr, ctx->done_dev, g, jobs, plan, ca, pool_ctas);
   ctx->launches += 1;
-  // launch 2: probe heads (qbar, probe scores, top-n)
-  if (ph.n > 0) {
-    const size_t sm = (size_t)g.NB * 4 + 256 * 4;
-    if (sm > 200 * 1024) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the probe kernel");
-    probe_kernel<<<ph.n, 1024, sm, st>>>(qpart, kt, probe, g, ca, ph);
-    ctx->launches += 1;
-  }
-  // launch 3: per-row emit / score + select
-  int R = 16;
+  // launch 2: per-row emit / score + select.  R rows per CTA: 16, fewer when NB is large (two CTAs per SM if possible)
+  int R = kSelRows;
   size_t sm = 0;
   if (any_block) {
-    const size_t budget = 220 * 1024 - 8 * 256 * 4;
-    while (R > 1 && (size_t)R * (g.NB + 64) * 4 > budget) --R;
-    if ((size_t)R * (g.NB + 64) * 4 > budget) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the select kernel");
-    sm = (size_t)R * (g.NB + 64) * 4 + 8 * 256 * 4;
+    const size_t qbytes = 64 * kSelRows * 4, row = (size_t)g.NB * 4;
+    size_t budget = 108 * 1024 - qbytes;
+    if (row > budget) budget = 220 * 1024 - qbytes;
+    if (row > budget) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the select kernel");
+    while ((size_t)R * row > budget) --R;
+    sm = (size_t)R * row + qbytes;
   }
   select_kernel<<<dim3((g.NB + R - 1) / R, g.H), 256, sm, st>>>(qt, kt, probe, lists->row_ptr, lists->col_idx, g, ca, R);
   ctx->launches += 1;

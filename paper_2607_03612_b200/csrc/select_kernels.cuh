@@ -1,9 +1,9 @@
 // Online pattern adaptation at block granularity (steps a-1..a-3 of DESIGN.md):
-//   pool_rowptr_kernel  Q,K bf16 -> Qtilde,Ktilde fp32 block means (HBM-bound stream, one warp per block) and, in extra CTAs
-//                       of the same launch, row_ptr from the closed-form row lengths
-//   probe_kernel        qbar = (1/N) sum_t q_t from the pooled block means, p[J] = qbar . Ktilde_J / sqrt(D),
-//                       top-n -> one shared list per QUERY_PROBE head
-//   select_kernel    per (head, q-block): closed-form emit, probe-list copy, or score row + top-n / per-frame top-k
+//   pool_rowptr_kernel  Q,K bf16 -> Qtilde,Ktilde fp32 block means (HBM-bound stream, one warp per block); in extra CTAs
+//                       of the same launch, row_ptr from the closed-form row lengths; and, in the last pool CTA of each
+//                       QUERY_PROBE head, the probe: qbar = (1/N) sum_t q_t, p[J] = qbar . Ktilde_J / sqrt(D),
+//                       top-n -> one shared list per head
+//   select_kernel       per (head, q-block): closed-form emit, probe-list copy, or score row + top-n / per-frame top-k
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -102,13 +102,122 @@ __host__ __device__ inline int64_t row_length(const SelGeom &g, const saf3r_head
   return closed_form_row(g, c, I, [](int64_t) {});
 }
 
-// ------------------------------------------------------------------------------------------------ pool + row_ptr
+// ------------------------------------------------------------------------------------------------ warp-level top-n
+// Order-preserving key: larger float <-> larger key; -0 is folded onto +0 so that ties follow the float comparison.
+__device__ __forceinline__ uint32_t score_key(float s) {
+  uint32_t u = __float_as_uint(s);
+  if (u == 0x80000000u) u = 0u;
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+
+constexpr int kKeysPerLaneReg = 36;  // rows with NB <= 32*36 keep their keys in registers during the bisection
+
+// One warp: keep the n largest of key[0..NB) (order-preserving keys in shared memory) under (key desc, index asc);
+// write their indices ascending to out.  No atomics, no sort: a bitwise bisection finds the n-th largest key tau (one
+// warp-wide count of {key >= candidate} per bit, keys distributed over the lanes; it stops early as soon as a candidate
+// splits the row into exactly n and NB-n keys), then an ordered ballot compaction emits {key > tau} plus the first
+// `need` (by index) of {key == tau}.
+template <bool kRegs>
+__device__ __forceinline__ void warp_topn_bisect_impl(const uint32_t *key, int NB, int n, int32_t *out) {
+  const int lane = threadIdx.x & 31;
+  uint32_t kk[kRegs ? kKeysPerLaneReg : 1];
+  if (kRegs) {
+#pragma unroll
+    for (int i = 0; i < kKeysPerLaneReg; ++i) {
+      const int j = lane + 32 * i;
+      kk[i] = j < NB ? key[j] : 0u;  // key 0 is below every candidate (candidates have at least one bit set)
+    }
+  }
+  auto count_ge = [&](uint32_t cand) -> int {
+    int c = 0;
+    if (kRegs) {
+#pragma unroll
+      for (int i = 0; i < kKeysPerLaneReg; ++i) c += (kk[i] >= cand) ? 1 : 0;
+    } else {
+      for (int j = lane; j < NB; j += 32) c += (key[j] >= cand) ? 1 : 0;
+    }
+    return __reduce_add_sync(0xffffffffu, c);
+  };
+  uint32_t prefix = 0;
+  bool exact = false;
+  for (int bit = 31; bit >= 0; --bit) {
+    const uint32_t cand = prefix | (1u << bit);
+    const int c = count_ge(cand);
+    if (c >= n) {
+      prefix = cand;
+      if (c == n) { exact = true; break; }
+    }
+  }
+  // exact: the kept set is {key >= prefix}, i.e. {key > prefix-1} with no ties to take.  Otherwise prefix is the n-th
+  // largest key tau: keep {key > tau} and the first n - |{key > tau}| of the keys equal to tau.
+  uint32_t tau;
+  int need;
+  if (exact) {
+    tau = prefix - 1u;
+    need = 0;
+  } else {
+    tau = prefix;
+    need = n - (tau == 0xffffffffu ? 0 : count_ge(tau + 1u));
+  }
+  int written = 0, eq_seen = 0;
+  const uint32_t lt = (1u << lane) - 1u;
+  for (int j0 = 0; j0 < NB; j0 += 32) {
+    const int j = j0 + lane;
+    const uint32_t kv = j < NB ? key[j] : 0u;
+    const bool gt = j < NB && kv > tau, eq = j < NB && kv == tau && need > 0;
+    const uint32_t eqb = __ballot_sync(0xffffffffu, eq);
+    const bool take = gt || (eq && eq_seen + __popc(eqb & lt) < need);
+    const uint32_t tb = __ballot_sync(0xffffffffu, take);
+    if (take) out[written + __popc(tb & lt)] = j;
+    written += __popc(tb);
+    eq_seen += __popc(eqb);
+  }
+}
+__device__ __forceinline__ void warp_topn_bisect(const uint32_t *key, int NB, int n, int32_t *out) {
+  if (NB <= 32 * kKeysPerLaneReg) warp_topn_bisect_impl<true>(key, NB, n, out);
+  else warp_topn_bisect_impl<false>(key, NB, n, out);
+}
+
+// One warp: per-frame top-k (PER_FRAME scope): in every frame's candidate range keep the kf best; ascending output.
+__device__ inline void warp_per_frame_emit(const uint32_t *key, const SelGeom &g, int kf, int32_t *out) {
+  const int lane = threadIdx.x & 31;
+  int base = 0;
+  for (int f0 = 0; f0 < g.S; f0 += 32) {
+    const int f = f0 + lane;
+    int64_t lo = 0, hi = -1;
+    if (f < g.S) frame_candidates(g, f, lo, hi);
+    const int m = (int)i64max(0, hi - lo + 1);
+    const int keep = m < kf ? m : kf;
+    int inc = keep;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      int v = __shfl_up_sync(0xffffffffu, inc, off);
+      if (lane >= off) inc += v;
+    }
+    int pos = base + inc - keep;
+    for (int a = 0; a < m; ++a) {
+      const uint32_t sa = key[lo + a];
+      int rank = 0;
+      for (int b = 0; b < m; ++b) {
+        const uint32_t sb = key[lo + b];
+        rank += (sb > sa) || (sb == sa && b < a);
+      }
+      if (rank < kf) out[pos++] = (int32_t)(lo + a);
+    }
+    base += __shfl_sync(0xffffffffu, inc, 31);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ pool + row_ptr + probe
 // One launch, two kinds of CTA (256 threads):
 //   blockIdx.x <  pool_ctas : 8 warps, ONE WARP PER TOKEN BLOCK.  job j = (tensor, head) pairs that the head's rule reads
-//                            (host-built list), warp w -> (job = w / NB, J = w % NB).  A warp streams its block's
-//                            B x 128 B with 16-byte loads (lane = 16-byte chunk (l&7) of rows (l>>3) + 4i, eight loads in
-//                            flight), accumulates in fp32, folds the four row groups with shuffles and writes the
-//                            64-float mean.  No shared memory, no block barrier.
+//                            (host-built list, QUERY_PROBE heads first), warp w -> (job = w / NB, J = w % NB).  A warp
+//                            streams its block's B x 128 B with 16-byte loads (lane = 16-byte chunk (l&7) of rows
+//                            (l>>3) + 4i, eight loads in flight), accumulates in fp32, folds the four row groups with
+//                            shuffles and writes the 64-float mean.
+//                            The LAST pool CTA of a QUERY_PROBE head to finish (device counter, no waiting) runs the
+//                            head's probe: qbar = (1/N) sum_t q_t from the per-CTA token sums,
+//                            p[J] = qbar . Ktilde_J / sqrt(D), top-n -> probe_list[h][0..n).
 //   blockIdx.x >= pool_ctas : one CTA per head writes that head's row_ptr entries: head_base + I*len for heads whose
 //                            rows all have the same length, a block scan of the closed-form lengths otherwise.
 struct PoolJobs {
@@ -116,7 +225,7 @@ struct PoolJobs {
   uint8_t head[2 * SAF3R_MAX_HEADS];
   uint8_t which[2 * SAF3R_MAX_HEADS];   // 0 = Q, 1 = K
   uint8_t cosine[2 * SAF3R_MAX_HEADS];  // L2-normalise each token first
-  uint8_t part[2 * SAF3R_MAX_HEADS];    // also write per-CTA token sums (Q of a QUERY_PROBE head, for qbar)
+  uint8_t probe[2 * SAF3R_MAX_HEADS];   // the head is a QUERY_PROBE head (its Q job also writes per-CTA token sums)
 };
 struct RowPtrPlan {
   int64_t head_base[SAF3R_MAX_HEADS + 1];  // first entry of each head (host closed form); [H] = total
@@ -129,10 +238,37 @@ __device__ __forceinline__ uint4 ld_stream_16(const void *p) {
   return r;
 }
 
-__global__ void __launch_bounds__(256) pool_rowptr_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
+// Probe of one QUERY_PROBE head, run by the whole CTA (256 threads) once the head's Qtilde partial sums and Ktilde are
+// complete in global memory (they were written by other CTAs of this launch: read them with ld.cg).
+__device__ __noinline__ void probe_head(const float *qpart, const float *ktT, int32_t *probe_list, const SelGeom &g, int h, int n,
+                                  uint32_t *key /* dynamic smem, NB */, float (*part)[64], float *qb) {
+  const int nparts = (g.NB + 7) / 8;
+  {
+    const int d = threadIdx.x & 63, grp = threadIdx.x >> 6;
+    const float *base = qpart + (int64_t)h * nparts * 64 + d;
+    float a0 = 0.f;
+    for (int c = grp; c < nparts; c += 4) a0 += __ldcg(base + (int64_t)c * 64);
+    part[grp][d] = a0;
+    __syncthreads();
+    if (threadIdx.x < 64) qb[threadIdx.x] = ((part[0][threadIdx.x] + part[1][threadIdx.x]) + (part[2][threadIdx.x] + part[3][threadIdx.x])) / (float)g.N;
+    __syncthreads();
+  }
+  for (int J = threadIdx.x; J < g.NB; J += 256) {
+    const float *kc = ktT + (int64_t)h * 64 * g.NB + J;
+    float acc = 0.f;
+#pragma unroll 16
+    for (int d = 0; d < 64; ++d) acc = fmaf(qb[d], __ldcg(kc + (int64_t)d * g.NB), acc);
+    key[J] = score_key(acc * 0.125f);
+  }
+  __syncthreads();
+  if (threadIdx.x < 32) warp_topn_bisect(key, g.NB, n, probe_list + (int64_t)h * g.NB);
+}
+
+__global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
                                                           float *__restrict__ qt, float *__restrict__ ktT, float *__restrict__ qpart,
-                                                          int64_t *__restrict__ row_ptr, SelGeom g, PoolJobs jobs, RowPtrPlan plan,
-                                                          HeadCfgArray cfg, int pool_ctas) {
+                                                          int32_t *__restrict__ probe_list, int64_t *__restrict__ row_ptr,
+                                                          uint32_t *__restrict__ done /* ctx-owned [H], zero between calls */,
+                                                          SelGeom g, PoolJobs jobs, RowPtrPlan plan, HeadCfgArray cfg, int pool_ctas) {
   if ((int)blockIdx.x >= pool_ctas) {
     // ---------------------------------------------------------------- row_ptr of one head
     const int h = blockIdx.x - pool_ctas;
@@ -165,82 +301,82 @@ __global__ void __launch_bounds__(256) pool_rowptr_kernel(const __nv_bfloat16 *_
   }
   // ------------------------------------------------------------------ pool: one warp per token block
   // CTA c of a job covers blocks 8c .. 8c+7 (jobs are padded to a multiple of 8 blocks, so a CTA never straddles jobs)
+  extern __shared__ uint32_t probe_key[];  // NB keys, used only by the last CTA of a QUERY_PROBE head
+  __shared__ float qsum[8][64];
+  __shared__ float qb[64];
+  __shared__ int is_last;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ctas_per_job = (g.NB + 7) / 8;
   const int job = blockIdx.x / ctas_per_job, cta_in_job = blockIdx.x % ctas_per_job;
   const int J = cta_in_job * 8 + warp;
-  __shared__ float qsum[8][64];
-  const bool want_part = jobs.part[job] != 0;  // Q of a QUERY_PROBE head: also emit this CTA's token sum (for qbar)
-  if (J >= g.NB) {
-    if (want_part) {
-      qsum[warp][lane] = 0.f;
-      qsum[warp][lane + 32] = 0.f;
-      __syncthreads();
-    }
-    return;
-  }
   const int h = jobs.head[job], which = jobs.which[job];
-  const bool cosine = jobs.cosine[job] != 0;
-  const int64_t t0 = (int64_t)J * g.B;
-  const int cnt = (int)i64min(g.B, g.N - t0);
+  const bool probe = jobs.probe[job] != 0;
+  const bool want_part = probe && which == 0;  // Q of a QUERY_PROBE head: also emit this CTA's token sum (for qbar)
+  const bool valid = J < g.NB;
   const int sub = lane & 7, rg = lane >> 3;
-  const __nv_bfloat16 *src = (which ? k : q) + (int64_t)h * g.stride_head + t0 * g.stride_token + sub * 8;
   float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  for (int r0 = 0; r0 < g.B; r0 += 32) {  // 8 loads of 16 B in flight per lane (rows r0 + rg + 4i)
-    uint4 raw[8];
+  if (valid) {
+    const bool cosine = jobs.cosine[job] != 0;
+    const int64_t t0 = (int64_t)J * g.B;
+    const int cnt = (int)i64min(g.B, g.N - t0);
+    const __nv_bfloat16 *src = (which ? k : q) + (int64_t)h * g.stride_head + t0 * g.stride_token + sub * 8;
+    for (int r0 = 0; r0 < g.B; r0 += 32) {  // 8 loads of 16 B in flight per lane (rows r0 + rg + 4i)
+      uint4 raw[8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const int r = r0 + rg + 4 * i;
-      raw[i] = make_uint4(0, 0, 0, 0);
-      if (r < cnt) raw[i] = ld_stream_16(src + (int64_t)r * g.stride_token);
-    }
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const uint32_t w[4] = {raw[i].x, raw[i].y, raw[i].z, raw[i].w};
-      float v[8];
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        v[2 * c] = __uint_as_float(w[c] << 16);
-        v[2 * c + 1] = __uint_as_float(w[c] & 0xFFFF0000u);
-      }
-      float inv = 1.f;
-      if (cosine) {
-        float ss = 0.f;
-#pragma unroll
-        for (int c = 0; c < 8; ++c) ss = fmaf(v[c], v[c], ss);
-        ss += __shfl_xor_sync(0xffffffffu, ss, 1);
-        ss += __shfl_xor_sync(0xffffffffu, ss, 2);
-        ss += __shfl_xor_sync(0xffffffffu, ss, 4);
-        const float nrm = sqrtf(ss);
-        inv = nrm < 1e-20f ? 0.f : 1.f / nrm;
+      for (int i = 0; i < 8; ++i) {
+        const int r = r0 + rg + 4 * i;
+        raw[i] = make_uint4(0, 0, 0, 0);
+        if (r < cnt) raw[i] = ld_stream_16(src + (int64_t)r * g.stride_token);
       }
 #pragma unroll
-      for (int c = 0; c < 8; ++c) acc[c] = fmaf(v[c], inv, acc[c]);
+      for (int i = 0; i < 8; ++i) {
+        const uint32_t w[4] = {raw[i].x, raw[i].y, raw[i].z, raw[i].w};
+        float v[8];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          v[2 * c] = __uint_as_float(w[c] << 16);
+          v[2 * c + 1] = __uint_as_float(w[c] & 0xFFFF0000u);
+        }
+        float inv = 1.f;
+        if (cosine) {
+          float ss = 0.f;
+#pragma unroll
+          for (int c = 0; c < 8; ++c) ss = fmaf(v[c], v[c], ss);
+          ss += __shfl_xor_sync(0xffffffffu, ss, 1);
+          ss += __shfl_xor_sync(0xffffffffu, ss, 2);
+          ss += __shfl_xor_sync(0xffffffffu, ss, 4);
+          const float nrm = sqrtf(ss);
+          inv = nrm < 1e-20f ? 0.f : 1.f / nrm;
+        }
+#pragma unroll
+        for (int c = 0; c < 8; ++c) acc[c] = fmaf(v[c], inv, acc[c]);
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 8);
+      acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 16);
+    }
+    const float invc = 1.f / (float)cnt;
+    if (rg == 0) {
+      if (which == 0) {  // Qtilde row-major [H][NB][64]
+        float4 *dst = reinterpret_cast<float4 *>(qt + ((int64_t)h * g.NB + J) * 64 + sub * 8);
+        dst[0] = make_float4(acc[0] * invc, acc[1] * invc, acc[2] * invc, acc[3] * invc);
+        dst[1] = make_float4(acc[4] * invc, acc[5] * invc, acc[6] * invc, acc[7] * invc);
+      } else {  // Ktilde TRANSPOSED [H][64][NB]: the score kernels read it coalesced over J
+#pragma unroll
+        for (int c = 0; c < 8; ++c) ktT[((int64_t)h * 64 + sub * 8 + c) * g.NB + J] = acc[c] * invc;
+      }
     }
   }
-#pragma unroll
-  for (int c = 0; c < 8; ++c) {
-    acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 8);
-    acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 16);
-  }
-  const float invc = 1.f / (float)cnt;
-  if (rg == 0) {
-    if (which == 0) {  // Qtilde row-major [H][NB][64]
-      float4 *dst = reinterpret_cast<float4 *>(qt + ((int64_t)h * g.NB + J) * 64 + sub * 8);
-      dst[0] = make_float4(acc[0] * invc, acc[1] * invc, acc[2] * invc, acc[3] * invc);
-      dst[1] = make_float4(acc[4] * invc, acc[5] * invc, acc[6] * invc, acc[7] * invc);
-    } else {  // Ktilde TRANSPOSED [H][64][NB]: the score kernels read it coalesced over J
-#pragma unroll
-      for (int c = 0; c < 8; ++c) ktT[((int64_t)h * 64 + sub * 8 + c) * g.NB + J] = acc[c] * invc;
-    }
-  }
+  if (!probe) return;  // CTA-uniform
   if (want_part) {
     if (rg == 0) {
 #pragma unroll
-      for (int c = 0; c < 8; ++c) qsum[warp][sub * 8 + c] = acc[c];
+      for (int c = 0; c < 8; ++c) qsum[warp][sub * 8 + c] = acc[c];  // zero for warps past the last block
     }
     __syncthreads();
-    if (warp == 0) {  // warp 0 always owns a real block (J = 8c < NB)
+    if (warp == 0) {
 #pragma unroll
       for (int d = lane; d < 64; d += 32) {
         float t = 0.f;
@@ -250,152 +386,43 @@ __global__ void __launch_bounds__(256) pool_rowptr_kernel(const __nv_bfloat16 *_
       }
     }
   }
-}
-
-// ------------------------------------------------------------------------------------------------ warp-level top-n
-// Order-preserving key: larger float <-> larger key; -0 is folded onto +0 so that ties follow the float comparison.
-__device__ __forceinline__ uint32_t score_key(float s) {
-  uint32_t u = __float_as_uint(s);
-  if (u == 0x80000000u) u = 0u;
-  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
-}
-
-// One warp: keep the n largest of s[0..NB) under (score desc, index asc); write their indices ascending to out.
-// hist: 256 uint32 of shared memory private to the warp.  Radix-select the n-th largest key (4 passes of 8 bits),
-// then an ordered compaction: {key > tau} plus the first `need` (by index) of {key == tau}.
-__device__ inline void warp_topn_emit(const float *s, int NB, int n, int32_t *out, uint32_t *hist) {
-  const int lane = threadIdx.x & 31;
-  uint32_t prefix = 0, mask = 0;
-  int need = n;
-  for (int shift = 24; shift >= 0; shift -= 8) {
-    for (int i = lane; i < 256; i += 32) hist[i] = 0;
-    __syncwarp();
-    for (int j = lane; j < NB; j += 32) {
-      const uint32_t key = score_key(s[j]);
-      if ((key & mask) == prefix) atomicAdd(&hist[(key >> shift) & 255u], 1u);
-    }
-    __syncwarp();
-    // lane L owns buckets 255-8L .. 248-8L (descending); find the bucket where the running count reaches `need`
-    uint32_t loc[8], tot = 0;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) { loc[i] = hist[255 - 8 * lane - i]; tot += loc[i]; }
-    uint32_t inc = tot;
-#pragma unroll
-    for (int off = 1; off < 32; off <<= 1) {
-      uint32_t v = __shfl_up_sync(0xffffffffu, inc, off);
-      if (lane >= off) inc += v;
-    }
-    const uint32_t exc = inc - tot;
-    const uint32_t hit = __ballot_sync(0xffffffffu, inc >= (uint32_t)need);
-    const int src = __ffs(hit) - 1;
-    int bucket = 0, above = 0;
-    if (lane == src) {
-      uint32_t run = exc;
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        if (run + loc[i] >= (uint32_t)need) { bucket = 255 - 8 * lane - i; above = (int)run; break; }
-        run += loc[i];
-      }
-    }
-    bucket = __shfl_sync(0xffffffffu, bucket, src);
-    above = __shfl_sync(0xffffffffu, above, src);
-    need -= above;
-    prefix |= (uint32_t)bucket << shift;
-    mask |= 255u << shift;
-    __syncwarp();
-  }
-  const uint32_t tau = prefix;  // key of the n-th largest score; take `need` of the elements equal to it, lowest index first
-  int written = 0, eq_seen = 0;
-  const uint32_t lt = (1u << lane) - 1u;
-  for (int j0 = 0; j0 < NB; j0 += 32) {
-    const int j = j0 + lane;
-    const uint32_t key = j < NB ? score_key(s[j]) : 0u;
-    const bool gt = j < NB && key > tau, eq = j < NB && key == tau;
-    const uint32_t eqb = __ballot_sync(0xffffffffu, eq);
-    const bool take = gt || (eq && eq_seen + __popc(eqb & lt) < need);
-    const uint32_t tb = __ballot_sync(0xffffffffu, take);
-    if (take) out[written + __popc(tb & lt)] = j;
-    written += __popc(tb);
-    eq_seen += __popc(eqb);
-  }
-}
-
-// One warp: per-frame top-k (PER_FRAME scope): in every frame's candidate range keep the kf best; ascending output.
-__device__ inline void warp_per_frame_emit(const float *s, const SelGeom &g, int kf, int32_t *out) {
-  const int lane = threadIdx.x & 31;
-  int base = 0;
-  for (int f0 = 0; f0 < g.S; f0 += 32) {
-    const int f = f0 + lane;
-    int64_t lo = 0, hi = -1;
-    if (f < g.S) frame_candidates(g, f, lo, hi);
-    const int m = (int)i64max(0, hi - lo + 1);
-    const int keep = m < kf ? m : kf;
-    int inc = keep;
-#pragma unroll
-    for (int off = 1; off < 32; off <<= 1) {
-      int v = __shfl_up_sync(0xffffffffu, inc, off);
-      if (lane >= off) inc += v;
-    }
-    int pos = base + inc - keep;
-    for (int a = 0; a < m; ++a) {
-      const float sa = s[lo + a];
-      int rank = 0;
-      for (int b = 0; b < m; ++b) {
-        const float sb = s[lo + b];
-        rank += (sb > sa) || (sb == sa && b < a);
-      }
-      if (rank < kf) out[pos++] = (int32_t)(lo + a);
-    }
-    base += __shfl_sync(0xffffffffu, inc, 31);
-  }
-}
-
-// ------------------------------------------------------------------------------------------------ probe
-// grid (number of QUERY_PROBE heads), 1024 threads, dynamic smem: NB floats + 256 uint32.  qbar (16 row groups x 64 dims,
-// fixed summation order), probe scores, then warp 0 radix-selects.  Writes the head's shared list to probe_list[h][0..n).
-struct ProbeHeads { int32_t n; uint8_t head[SAF3R_MAX_HEADS]; };
-
-__global__ void __launch_bounds__(1024) probe_kernel(const float *__restrict__ qpart, const float *__restrict__ ktT,
-                                                     int32_t *__restrict__ probe_list, SelGeom g, HeadCfgArray cfg, ProbeHeads ph) {
-  const int h = ph.head[blockIdx.x];
-  extern __shared__ float sm[];
-  float *s = sm;
-  uint32_t *hist = reinterpret_cast<uint32_t *>(sm + g.NB);
-  __shared__ float part[16][64];
-  __shared__ float qb[64];
-  {
-    const int d = threadIdx.x & 63, grp = threadIdx.x >> 6;
-    const int nparts = (g.NB + 7) / 8;
-    const float *base = qpart + (int64_t)h * nparts * 64 + d;
-    float a0 = 0.f;
-    for (int c = grp; c < nparts; c += 16) a0 += base[(int64_t)c * 64];
-    part[grp][d] = a0;
-    __syncthreads();
-    if (threadIdx.x < 64) {
-      float t = 0.f;
-#pragma unroll
-      for (int i = 0; i < 16; ++i) t += part[i][threadIdx.x];
-      qb[threadIdx.x] = t / (float)g.N;
-    }
-    __syncthreads();
-  }
-  for (int J = threadIdx.x; J < g.NB; J += blockDim.x) {
-    const float *kc = ktT + (int64_t)h * 64 * g.NB + J;
-    float acc = 0.f;
-#pragma unroll 16
-    for (int d = 0; d < 64; ++d) acc = fmaf(qb[d], __ldg(kc + (int64_t)d * g.NB), acc);
-    s[J] = acc * 0.125f;
+  // last-CTA-done: every thread's global writes are fenced, then one thread takes a ticket
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const uint32_t t = atomicAdd(&done[h], 1u);
+    is_last = (t == 2u * (uint32_t)ctas_per_job - 1u);
+    if (is_last) done[h] = 0u;  // self-reset for the next call (all other CTAs of this head have already arrived)
   }
   __syncthreads();
-  if (threadIdx.x < 32) warp_topn_emit(s, g.NB, (int)i64min(cfg.c[h].keep_blocks, g.NB), probe_list + (int64_t)h * g.NB, hist);
+  if (!is_last) return;
+  __threadfence();
+  probe_head(qpart, ktT, probe_list, g, h, (int)i64min(cfg.c[h].keep_blocks, g.NB), probe_key, qsum, qb);
 }
 
 // ------------------------------------------------------------------------------------------------ select
-// grid (ceil(NB/R), H), 256 threads (8 warps), R <= 16 rows per CTA (Ktilde is re-read once per CTA, so more rows = less L2 traffic).  dynamic smem: R*NB floats (scores) + R*64 floats
-// (Qtilde rows) + 8*256 uint32 (histograms).
-__global__ void __launch_bounds__(256) select_kernel(const float *__restrict__ qt, const float *__restrict__ ktT,
-                                                     const int32_t *__restrict__ probe_list, const int64_t *__restrict__ row_ptr,
-                                                     int32_t *__restrict__ col_idx, SelGeom g, HeadCfgArray cfg, int R) {
+// grid (ceil(NB/R), H), 256 threads (8 warps), R = 16 rows (fewer when NB is large) per CTA.
+//   closed-form heads: lane-parallel emitters;  QUERY_PROBE heads: copy the head's probe list into every row;
+//   BLOCK_TOPK heads: score rows s[I][J] = Qtilde_I . Ktilde_J * c (fp32 FMA in the order d = 0..63, as packed
+//   row pairs; each thread owns two columns J and keeps 16 row accumulators for each) stored as order-preserving keys
+//   in shared memory, then one warp per row: bisection top-n or per-frame top-k.
+// dynamic smem: R*NB keys + 64*R floats (Qtilde rows, transposed so that four rows of one d are one 16-byte load).
+constexpr int kSelRows = 16;
+
+__device__ __forceinline__ uint64_t sel_pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ uint64_t sel_fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+
+__global__ void __launch_bounds__(256, 2) select_kernel(const float *__restrict__ qt, const float *__restrict__ ktT,
+                                                        const int32_t *__restrict__ probe_list, const int64_t *__restrict__ row_ptr,
+                                                        int32_t *__restrict__ col_idx, SelGeom g, HeadCfgArray cfg, int R) {
   const int h = blockIdx.y;
   const saf3r_head_cfg c = cfg.c[h];
   const int I0 = blockIdx.x * R;
@@ -436,38 +463,64 @@ __global__ void __launch_bounds__(256) select_kernel(const float *__restrict__ q
     return;
   }
 
-  float *scores = sm;                                   // [R][NB]
-  float *qrows = sm + (size_t)R * g.NB;                 // [R][64]
-  uint32_t *hist = reinterpret_cast<uint32_t *>(qrows + R * 64) + warp * 256;
-  for (int i = threadIdx.x; i < rows * 64; i += blockDim.x) qrows[i] = qt[((int64_t)h * g.NB + I0) * 64 + i];
+  uint32_t *keys = reinterpret_cast<uint32_t *>(sm);   // [R][NB]
+  float *qT = sm + (size_t)R * g.NB;                   // [64][kSelRows] (rows past `rows` are zero)
+  for (int i = threadIdx.x; i < 64 * kSelRows; i += blockDim.x) {
+    const int d = i / kSelRows, r = i % kSelRows;
+    qT[i] = r < rows ? qt[((int64_t)h * g.NB + I0 + r) * 64 + d] : 0.f;
+  }
   __syncthreads();
   const float cs = c.score_mode == SAF3R_SCORE_COSINE ? 1.f : 0.125f;
-  for (int J = threadIdx.x; J < g.NB; J += blockDim.x) {
-    float kv[64];
-    const float *kc = ktT + (int64_t)h * 64 * g.NB + J;
+  const float *kh = ktT + (int64_t)h * 64 * g.NB;
+  for (int J0 = threadIdx.x; J0 < g.NB; J0 += 512) {
+    const int J1 = J0 + 256;
+    const bool has1 = J1 < g.NB;
+    uint64_t a0[kSelRows / 2], a1[kSelRows / 2];
 #pragma unroll
-    for (int d = 0; d < 64; ++d) kv[d] = __ldg(kc + (int64_t)d * g.NB);
-    for (int r = 0; r < rows; ++r) {
-      const float4 *qr = reinterpret_cast<const float4 *>(qrows + r * 64);
-      float acc = 0.f;
+    for (int r = 0; r < kSelRows / 2; ++r) a0[r] = a1[r] = 0ull;
+#pragma unroll 2
+    for (int d0 = 0; d0 < 64; d0 += 8) {
+      float k0[8], k1[8];
 #pragma unroll
-      for (int d4 = 0; d4 < 16; ++d4) {
-        const float4 t = qr[d4];
-        acc = fmaf(t.x, kv[4 * d4], acc);
-        acc = fmaf(t.y, kv[4 * d4 + 1], acc);
-        acc = fmaf(t.z, kv[4 * d4 + 2], acc);
-        acc = fmaf(t.w, kv[4 * d4 + 3], acc);
+      for (int i = 0; i < 8; ++i) {
+        k0[i] = __ldg(kh + (int64_t)(d0 + i) * g.NB + J0);
+        k1[i] = has1 ? __ldg(kh + (int64_t)(d0 + i) * g.NB + J1) : 0.f;
       }
-      scores[(size_t)r * g.NB + J] = acc * cs;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const float4 *qr = reinterpret_cast<const float4 *>(qT + (d0 + i) * kSelRows);
+        const uint64_t kk0 = sel_pack2(k0[i], k0[i]), kk1 = sel_pack2(k1[i], k1[i]);
+#pragma unroll
+        for (int r4 = 0; r4 < kSelRows / 4; ++r4) {
+          const float4 t = qr[r4];
+          const uint64_t qa = sel_pack2(t.x, t.y), qb = sel_pack2(t.z, t.w);
+          a0[2 * r4] = sel_fma2(qa, kk0, a0[2 * r4]);
+          a0[2 * r4 + 1] = sel_fma2(qb, kk0, a0[2 * r4 + 1]);
+          a1[2 * r4] = sel_fma2(qa, kk1, a1[2 * r4]);
+          a1[2 * r4 + 1] = sel_fma2(qb, kk1, a1[2 * r4 + 1]);
+        }
+      }
+    }
+#pragma unroll
+    for (int r2 = 0; r2 < kSelRows / 2; ++r2) {
+      float lo, hi;
+      asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a0[r2]));
+      if (2 * r2 < rows) keys[(size_t)(2 * r2) * g.NB + J0] = score_key(lo * cs);
+      if (2 * r2 + 1 < rows) keys[(size_t)(2 * r2 + 1) * g.NB + J0] = score_key(hi * cs);
+      if (has1) {
+        asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a1[r2]));
+        if (2 * r2 < rows) keys[(size_t)(2 * r2) * g.NB + J1] = score_key(lo * cs);
+        if (2 * r2 + 1 < rows) keys[(size_t)(2 * r2 + 1) * g.NB + J1] = score_key(hi * cs);
+      }
     }
   }
   __syncthreads();
   for (int r = warp; r < rows; r += 8) {
     int32_t *out = col_idx + row_ptr[(int64_t)h * g.NB + I0 + r];
     if (c.topk_scope == SAF3R_SCOPE_GLOBAL)
-      warp_topn_emit(scores + (size_t)r * g.NB, g.NB, (int)i64min(c.keep_blocks, g.NB), out, hist);
+      warp_topn_bisect(keys + (size_t)r * g.NB, g.NB, (int)i64min(c.keep_blocks, g.NB), out);
     else
-      warp_per_frame_emit(scores + (size_t)r * g.NB, g, c.topk_per_frame, out);
+      warp_per_frame_emit(keys + (size_t)r * g.NB, g, c.topk_per_frame, out);
   }
 }
 
