@@ -263,6 +263,21 @@ def run_ours(args):
         sel_gbs = float(np.sum(sel_bytes)) / (float(np.sum(sel_ms)) * 1e-3) / 1e9
         result["select_roofline"] = {"bound": "hbm", "achieved": sel_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                      "frac": sel_gbs / peaks["hbm_gbs"], "note": "whole select call (pool+score+select) over the pool stage's algorithmic bytes"}
+        # stage split of the select call (untimed extra pass with saf3r_set_stage_timing): pool launch vs score+select launch
+        ctx.set_stage_timing(True)
+        pool_ms, ssel_ms = [], []
+        for i in range(2 * n_res):
+            d = dl[i % n_res]
+            ctx.select(d["q"], d["k"], shape, d["cfgs"], workspace=d["ws"], lists=d["lists"])
+            a, b = ctx.last_select_stage_ms()
+            if i >= n_res:
+                pool_ms.append(a)
+                ssel_ms.append(b)
+        ctx.set_stage_timing(False)
+        pool_gbs = float(np.sum([need[i] * sh.N * sh.D * 2 for i in range(n_res)])) / (float(np.sum(pool_ms)) * 1e-3) / 1e9
+        result["select_stages"] = {"pool_ms": float(np.mean(pool_ms)), "score_select_ms": float(np.mean(ssel_ms)),
+                                   "pool_gbs": pool_gbs, "pool_frac_of_hbm_peak": pool_gbs / peaks["hbm_gbs"],
+                                   "note": "pool launch = pooling + row_ptr + closed-form lists; score_select = probe + score + top-n + list copies; CUDA events inside saf3r_select"}
 
         if not args.skip_dense:
             d = dl[0]

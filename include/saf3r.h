@@ -131,6 +131,14 @@ saf3r_status saf3r_layer_host(saf3r_ctx *ctx, const void *q_host, const void *k_
 /* Number of kernels the library has launched on this context since creation (for bench.py's gpu_launches). */
 int64_t saf3r_launch_count(const saf3r_ctx *ctx);
 
+/* Measurement aid ("select ms split into pool and score+select stages").  When enabled, saf3r_select records
+ * CUDA events on its stream before the pool launch, between the two launches and after the select launch (three
+ * cudaEventRecord calls, no synchronisation).  saf3r_last_select_stage_ms blocks until the last timed saf3r_select has
+ * finished and returns the two stage durations in milliseconds: pool_ms = pooling (+ row_ptr, + the probe of QUERY_PROBE
+ * heads, which runs inside the pool launch), select_ms = score + select + list emission. */
+saf3r_status saf3r_set_stage_timing(saf3r_ctx *ctx, int enable);
+saf3r_status saf3r_last_select_stage_ms(saf3r_ctx *ctx, float *pool_ms, float *select_ms);
+
 #ifdef __cplusplus
 }
 #endif

@@ -25,7 +25,8 @@ SCOPE_GLOBAL, SCOPE_PER_FRAME = range(2)
 SCORE_DOT, SCORE_COSINE = range(2)
 
 EXPORTS = ("saf3r_create", "saf3r_destroy", "saf3r_last_error", "saf3r_query_sizes", "saf3r_select", "saf3r_sparse_attn",
-           "saf3r_dense_attn", "saf3r_layer_host_scratch_bytes", "saf3r_layer_host", "saf3r_launch_count")
+           "saf3r_dense_attn", "saf3r_layer_host_scratch_bytes", "saf3r_layer_host", "saf3r_launch_count",
+           "saf3r_set_stage_timing", "saf3r_last_select_stage_ms")
 
 
 class Saf3rError(RuntimeError):
@@ -74,6 +75,8 @@ def load_library():
         L.saf3r_layer_host.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), vp, C.c_size_t, vp, vp]
         L.saf3r_launch_count.argtypes = [vp]
         L.saf3r_launch_count.restype = i64
+        L.saf3r_set_stage_timing.argtypes = [vp, i32]
+        L.saf3r_last_select_stage_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         _lib = L
     return _lib
 
@@ -143,6 +146,15 @@ class Context:
 
     def launch_count(self) -> int:
         return int(self.lib.saf3r_launch_count(self.h))
+
+    # ---- saf3r_set_stage_timing / saf3r_last_select_stage_ms
+    def set_stage_timing(self, enable: bool):
+        self._check(self.lib.saf3r_set_stage_timing(self.h, int(enable)))
+
+    def last_select_stage_ms(self) -> tuple[float, float]:
+        a, b = C.c_float(), C.c_float()
+        self._check(self.lib.saf3r_last_select_stage_ms(self.h, C.byref(a), C.byref(b)))
+        return float(a.value), float(b.value)
 
     # ---- saf3r_query_sizes
     def query_sizes(self, shape: ShapeC, cfgs) -> tuple[int, int]:

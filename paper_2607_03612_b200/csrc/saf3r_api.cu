@@ -35,7 +35,9 @@ struct saf3r_ctx {
   std::string err;
   bool sticky_cuda = false;
   int64_t launches = 0;
-  uint32_t *done_dev = nullptr;  // [SAF3R_MAX_HEADS] last-CTA-done counters of the pool kernel; zero between calls
+  bool stage_timing = false;
+  cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};  // select: start, after the pool launch, after the select launch
+  bool ev_valid = false;
   std::vector<std::pair<MapKey, CUtensorMap>> maps;  // small LRU-less cache
   // per-head list totals of the lists saf3r_select last wrote into a given row_ptr buffer (scheduling hint only)
   struct LenHint { const int64_t *row_ptr; int32_t H, NB; int64_t len[SAF3R_MAX_HEADS]; };
@@ -122,7 +124,7 @@ static WsLayout ws_layout(const SelGeom &g) {
   WsLayout w;
   size_t off = 0;
   w.qt = off; off = align256(off + (size_t)g.H * g.NB * 64 * sizeof(float));
-  w.kt = off; off = align256(off + (size_t)g.H * g.NB * 64 * sizeof(float));
+  w.kt = off; off = align256(off + (size_t)g.H * kt_stride(g.NB) * 64 * sizeof(float));
   w.qpart = off; off = align256(off + (size_t)g.H * ((g.NB + 7) / 8) * 64 * sizeof(float));
   w.probe = off; off = align256(off + (size_t)g.H * g.NB * sizeof(int32_t));
   w.total = off;
@@ -178,9 +180,6 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
   e = cudaFuncSetAttribute(saf3r_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(pool_rowptr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-  if (e == cudaSuccess) e = cudaMalloc(&ctx->done_dev, SAF3R_MAX_HEADS * sizeof(uint32_t));
-  if (e == cudaSuccess) e = cudaMemset(ctx->done_dev, 0, SAF3R_MAX_HEADS * sizeof(uint32_t));
   if (e != cudaSuccess) {
     fprintf(stderr, "saf3r_create: cudaFuncSetAttribute failed: %s\n", cudaGetErrorString(e));
     delete ctx;
@@ -192,13 +191,33 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
 
 void saf3r_destroy(saf3r_ctx *ctx) {
   if (!ctx) return;
-  if (ctx->done_dev) cudaFree(ctx->done_dev);
+  for (auto &e : ctx->ev)
+    if (e) cudaEventDestroy(e);
   delete ctx;
 }
 
 const char *saf3r_last_error(const saf3r_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 
 int64_t saf3r_launch_count(const saf3r_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+saf3r_status saf3r_set_stage_timing(saf3r_ctx *ctx, int enable) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (enable && !ctx->ev[0]) {
+    for (auto &e : ctx->ev) CU_CHECK(cudaEventCreate(&e));
+  }
+  ctx->stage_timing = enable != 0;
+  ctx->ev_valid = false;
+  return SAF3R_OK;
+}
+
+saf3r_status saf3r_last_select_stage_ms(saf3r_ctx *ctx, float *pool_ms, float *select_ms) {
+  if (!ctx || !pool_ms || !select_ms) return SAF3R_ERR_INVALID_ARG;
+  if (!ctx->ev_valid) return fail(ctx, SAF3R_ERR_INVALID_ARG, "no timed saf3r_select call yet (saf3r_set_stage_timing)");
+  CU_CHECK(cudaEventSynchronize(ctx->ev[2]));
+  CU_CHECK(cudaEventElapsedTime(pool_ms, ctx->ev[0], ctx->ev[1]));
+  CU_CHECK(cudaEventElapsedTime(select_ms, ctx->ev[1], ctx->ev[2]));
+  return SAF3R_OK;
+}
 
 saf3r_status saf3r_query_sizes(const saf3r_shape *shape, const saf3r_head_cfg *cfg, int64_t *list_entries, size_t *workspace_bytes) {
   if (validate_shape(shape, false) || !cfg) return SAF3R_ERR_INVALID_ARG;
@@ -232,7 +251,7 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
   }
   cudaStream_t st = (cudaStream_t)stream_;
   uint8_t *wsb = (uint8_t *)ws;
-  float *qt = (float *)(wsb + w.qt), *kt = (float *)(wsb + w.kt) /* transposed [H][64][NB] */, *qpart = (float *)(wsb + w.qpart);
+  float *qt = (float *)(wsb + w.qt), *kt = (float *)(wsb + w.kt) , *qpart = (float *)(wsb + w.qpart);
   int32_t *probe = (int32_t *)(wsb + w.probe);
 
   HeadCfgArray ca;
@@ -241,6 +260,8 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
   memset(&jobs, 0, sizeof jobs);
   RowPtrPlan plan;
   memset(&plan, 0, sizeof plan);
+  HeadSets sets;
+  memset(&sets, 0, sizeof sets);
   bool any_block = false, any_probe = false;
   int64_t base = 0;
   for (int h = 0; h < g.H; ++h) {
@@ -248,6 +269,10 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
     any_block |= cfg[h].type == SAF3R_HEAD_BLOCK_TOPK;
     any_probe |= cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK;
     const bool per_row = cfg[h].type == SAF3R_HEAD_STATIC && cfg[h].static_mode != SAF3R_STATIC_ANCHOR;
+    if (cfg[h].type == SAF3R_HEAD_BLOCK_TOPK) sets.block[sets.n_block++] = (uint8_t)h;
+    else if (cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK) sets.probe[sets.n_probe++] = (uint8_t)h;
+    else if (per_row) sets.light[sets.n_light++] = (uint8_t)h;
+    else sets.emit[sets.n_emit++] = (uint8_t)h;
     plan.const_len[h] = per_row ? -1 : (int32_t)row_length(g, cfg[h], 0);
     plan.head_base[h] = base;
     base += hint.len[h];
@@ -266,27 +291,49 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
         ++jobs.n;
       }
     }
-  // launch 1: pooling (one warp per token block of every tensor a rule reads; the last CTA of a QUERY_PROBE head also runs
-  // its probe) + one row_ptr CTA per head
+  // launch 1: pooling (one warp per token block of every tensor a rule reads) + one row_ptr CTA per head + the lists of the
+  // constant-length closed-form heads
   const int pool_ctas = jobs.n * ((g.NB + 7) / 8);
-  const size_t pool_sm = any_probe ? (size_t)g.NB * 4 : 0;
-  if (pool_sm > 200 * 1024) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the probe stage");
-  pool_rowptr_kernel<<<pool_ctas + g.H, 256, pool_sm, st>>>((const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart, probe,
-                                                           lists->row_ptr, ctx->done_dev, g, jobs, plan, ca, pool_ctas);
+  const int light_chunks = (g.NB + kLightRows - 1) / kLightRows;
+  if (ctx->stage_timing) cudaEventRecord(ctx->ev[0], st);
+  pool_rowptr_kernel<<<pool_ctas + g.H + sets.n_emit * light_chunks, 256, 0, st>>>(
+      (const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart, lists->row_ptr, lists->col_idx, g, jobs, plan, ca, sets,
+      pool_ctas);
   ctx->launches += 1;
-  // launch 2: per-row emit / score + select.  R rows per CTA: 16, fewer when NB is large (two CTAs per SM if possible)
+  if (ctx->stage_timing) cudaEventRecord(ctx->ev[1], st);
+  // launch 2: probe CTAs, score + select CTAs (R rows each: 16, fewer when NB is large - two CTAs per SM if possible - or
+  // when the BLOCK_TOPK heads are few), light CTAs of the per-row-length STATIC heads
   int R = kSelRows;
   size_t sm = 0;
+  const size_t row = (size_t)kt_stride(g.NB) * 4;
   if (any_block) {
-    const size_t qbytes = 64 * kSelRows * 4, row = (size_t)g.NB * 4;
+    const size_t qbytes = 64 * kSelRows * 4;
     size_t budget = 108 * 1024 - qbytes;
     if (row > budget) budget = 220 * 1024 - qbytes;
     if (row > budget) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the select kernel");
     while ((size_t)R * row > budget) --R;
+    while (R > 8 && (int64_t)sets.n_block * ((g.NB + R - 1) / R) < 2 * (int64_t)ctx->sm_count) R = (R + 1) / 2;
     sm = (size_t)R * row + qbytes;
   }
-  select_kernel<<<dim3((g.NB + R - 1) / R, g.H), 256, sm, st>>>(qt, kt, probe, lists->row_ptr, lists->col_idx, g, ca, R);
-  ctx->launches += 1;
+  if (any_probe) {
+    if (row > 200 * 1024) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the probe stage");
+    if (sm < row) sm = row;
+  }
+  const int sel_ctas = sets.n_probe + sets.n_block * ((g.NB + R - 1) / R) + sets.n_light * light_chunks;
+  if (sel_ctas > 0) {
+    select_kernel<<<sel_ctas, 256, sm, st>>>(qt, kt, probe, lists->row_ptr, qpart, probe, lists->col_idx, g, ca, sets, R, 0);
+    ctx->launches += 1;
+  }
+  // launch 3: every row of a QUERY_PROBE head gets a copy of the head's probe list
+  if (sets.n_probe > 0) {
+    select_kernel<<<sets.n_probe * light_chunks, 256, 0, st>>>(qt, kt, probe, lists->row_ptr, qpart, probe, lists->col_idx, g, ca, sets,
+                                                              R, 1);
+    ctx->launches += 1;
+  }
+  if (ctx->stage_timing) {
+    cudaEventRecord(ctx->ev[2], st);
+    ctx->ev_valid = true;
+  }
   CU_CHECK(cudaGetLastError());
   hint.row_ptr = lists->row_ptr; hint.H = g.H; hint.NB = g.NB;
   bool found = false;

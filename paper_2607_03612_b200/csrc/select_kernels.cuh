@@ -22,6 +22,10 @@ struct HeadCfgArray {
   saf3r_head_cfg c[SAF3R_MAX_HEADS];
 };
 
+// Ktilde is stored TRANSPOSED, [H][64][NBp] with the row stride NBp = NB rounded up to 4, so that the score stage reads
+// four consecutive k-blocks of one dimension d as one aligned 16-byte load, coalesced across the warp.
+__host__ __device__ inline int64_t kt_stride(int32_t NB) { return ((int64_t)NB + 3) & ~(int64_t)3; }
+
 __host__ __device__ inline int64_t i64min(int64_t a, int64_t b) { return a < b ? a : b; }
 __host__ __device__ inline int64_t i64max(int64_t a, int64_t b) { return a > b ? a : b; }
 
@@ -129,17 +133,21 @@ __device__ __forceinline__ void warp_topn_bisect_impl(const uint32_t *key, int N
     }
   }
   auto count_ge = [&](uint32_t cand) -> int {
-    int c = 0;
+    int c0 = 0, c1 = 0;  // two chains; compare + predicated add = two instructions per key
     if (kRegs) {
 #pragma unroll
-      for (int i = 0; i < kKeysPerLaneReg; ++i) c += (kk[i] >= cand) ? 1 : 0;
+      for (int i = 0; i < kKeysPerLaneReg; i += 2) {
+        asm("{\n\t.reg .pred p;\n\tsetp.ge.u32 p, %1, %2;\n\t@p add.s32 %0, %0, 1;\n\t}" : "+r"(c0) : "r"(kk[i]), "r"(cand));
+        asm("{\n\t.reg .pred p;\n\tsetp.ge.u32 p, %1, %2;\n\t@p add.s32 %0, %0, 1;\n\t}" : "+r"(c1) : "r"(kk[i + 1]), "r"(cand));
+      }
     } else {
-      for (int j = lane; j < NB; j += 32) c += (key[j] >= cand) ? 1 : 0;
+      for (int j = lane; j < NB; j += 32) c0 += (key[j] >= cand) ? 1 : 0;
     }
-    return __reduce_add_sync(0xffffffffu, c);
+    return __reduce_add_sync(0xffffffffu, c0 + c1);
   };
   uint32_t prefix = 0;
   bool exact = false;
+#pragma unroll 1
   for (int bit = 31; bit >= 0; --bit) {
     const uint32_t cand = prefix | (1u << bit);
     const int c = count_ge(cand);
@@ -161,6 +169,17 @@ __device__ __forceinline__ void warp_topn_bisect_impl(const uint32_t *key, int N
   }
   int written = 0, eq_seen = 0;
   const uint32_t lt = (1u << lane) - 1u;
+  if (kRegs && need == 0) {  // common case: no ties at the cut; keys still in registers (padding keys are 0 <= tau)
+#pragma unroll
+    for (int i = 0; i < kKeysPerLaneReg; ++i) {
+      const bool take = kk[i] > tau;
+      const uint32_t tb = __ballot_sync(0xffffffffu, take);
+      int32_t *dst = out + written + __popc(tb & lt);
+      asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u32 [%0], %1;\n\t}" ::"l"(dst), "r"(lane + 32 * i), "r"((uint32_t)take) : "memory");
+      written += __popc(tb);
+    }
+    return;
+  }
   for (int j0 = 0; j0 < NB; j0 += 32) {
     const int j = j0 + lane;
     const uint32_t kv = j < NB ? key[j] : 0u;
@@ -208,6 +227,54 @@ __device__ inline void warp_per_frame_emit(const uint32_t *key, const SelGeom &g
   }
 }
 
+// ------------------------------------------------------------------------------------------------ light rows
+// One warp writes the list of q-block I of a head whose rule needs no scores of its own: closed forms (DENSE,
+// UNIFORM_STRIDE, STATIC) or a copy of the head's probe list (QUERY_PROBE_TOPK).
+__device__ __forceinline__ void emit_light_row(const SelGeom &g, const saf3r_head_cfg &c, int h, int64_t I, int32_t *out,
+                                               const int32_t *probe_list) {
+  const int lane = threadIdx.x & 31;
+  if (c.type == SAF3R_HEAD_QUERY_PROBE_TOPK) {
+    const int n = (int)i64min(c.keep_blocks, g.NB);
+    for (int i = lane; i < n; i += 32) out[i] = probe_list[(int64_t)h * g.NB + i];
+  } else if (c.type == SAF3R_HEAD_DENSE) {
+    for (int J = lane; J < g.NB; J += 32) out[J] = J;
+  } else if (c.type == SAF3R_HEAD_UNIFORM_STRIDE && c.stride >= 1) {
+    const int n = (g.NB - c.offset + c.stride - 1) / c.stride;
+    for (int i = lane; i < n; i += 32) out[i] = c.offset + i * c.stride;
+  } else if (c.type == SAF3R_HEAD_UNIFORM_STRIDE) {  // keep_blocks form (n <= NB, so the indices are distinct)
+    if ((uint64_t)g.NB * (uint64_t)c.keep_blocks < 0x100000000ull) {  // 32-bit division (the 64-bit one is emulated)
+      const uint32_t nb = (uint32_t)g.NB, kb = (uint32_t)c.keep_blocks;
+      for (uint32_t i = lane; i < kb; i += 32) out[i] = (int32_t)((i * nb) / kb);
+    } else {
+      for (int i = lane; i < c.keep_blocks; i += 32) out[i] = (int32_t)(((int64_t)i * g.NB) / c.keep_blocks);
+    }
+  } else if (c.type == SAF3R_HEAD_STATIC && c.static_mode != SAF3R_STATIC_POSITION_BAND) {  // one contiguous range
+    int64_t lo, hi;
+    if (c.static_mode == SAF3R_STATIC_ANCHOR) {
+      lo = ((int64_t)c.anchor_frame * g.T) / g.B;
+      hi = (((int64_t)c.anchor_frame + 1) * g.T - 1) / g.B;
+    } else {
+      const int64_t t0 = I * g.B, t1 = i64min(t0 + g.B, g.N);
+      lo = ((t0 / g.T) * g.T) / g.B;
+      hi = (((t1 - 1) / g.T + 1) * g.T - 1) / g.B;
+    }
+    for (int64_t J = lo + lane; J <= hi; J += 32) out[J - lo] = (int32_t)J;
+  } else if (lane == 0) {
+    int64_t w = 0;
+    closed_form_row(g, c, I, [&](int64_t J) { out[w++] = (int32_t)J; });
+  }
+}
+constexpr int kLightRows = 32;  // rows per CTA of the light emitters (8 warps x 4 rows)
+
+// Which heads each launch serves (host-built).
+struct HeadSets {
+  int32_t n_emit, n_light, n_block, n_probe;
+  uint8_t emit[SAF3R_MAX_HEADS];   // launch 1: closed-form heads whose rows all have the same length (no dependence at all)
+  uint8_t light[SAF3R_MAX_HEADS];  // launch 2: per-row-length STATIC heads (need row_ptr)
+  uint8_t block[SAF3R_MAX_HEADS];  // launch 2: BLOCK_TOPK heads (score + top-n)
+  uint8_t probe[SAF3R_MAX_HEADS];  // launch 2: QUERY_PROBE heads, one probe CTA each; launch 3: copy of the probe list into every row
+};
+
 // ------------------------------------------------------------------------------------------------ pool + row_ptr + probe
 // One launch, two kinds of CTA (256 threads):
 //   blockIdx.x <  pool_ctas : 8 warps, ONE WARP PER TOKEN BLOCK.  job j = (tensor, head) pairs that the head's rule reads
@@ -215,11 +282,11 @@ __device__ inline void warp_per_frame_emit(const uint32_t *key, const SelGeom &g
 //                            streams its block's B x 128 B with 16-byte loads (lane = 16-byte chunk (l&7) of rows
 //                            (l>>3) + 4i, eight loads in flight), accumulates in fp32, folds the four row groups with
 //                            shuffles and writes the 64-float mean.
-//                            The LAST pool CTA of a QUERY_PROBE head to finish (device counter, no waiting) runs the
-//                            head's probe: qbar = (1/N) sum_t q_t from the per-CTA token sums,
-//                            p[J] = qbar . Ktilde_J / sqrt(D), top-n -> probe_list[h][0..n).
-//   blockIdx.x >= pool_ctas : one CTA per head writes that head's row_ptr entries: head_base + I*len for heads whose
+//                            The Q job of a QUERY_PROBE head also writes its CTA's token sum (for qbar).
+//   next H CTAs             : one CTA per head writes that head's row_ptr entries: head_base + I*len for heads whose
 //                            rows all have the same length, a block scan of the closed-form lengths otherwise.
+//   remaining CTAs          : the lists of the closed-form heads whose rows all have the same length (DENSE, UNIFORM_STRIDE,
+//                            STATIC/ANCHOR): 32 rows per CTA, written under the pooling's HBM time.
 struct PoolJobs {
   int32_t n;                            // number of (tensor, head) jobs
   uint8_t head[2 * SAF3R_MAX_HEADS];
@@ -238,26 +305,39 @@ __device__ __forceinline__ uint4 ld_stream_16(const void *p) {
   return r;
 }
 
-// Probe of one QUERY_PROBE head, run by the whole CTA (256 threads) once the head's Qtilde partial sums and Ktilde are
-// complete in global memory (they were written by other CTAs of this launch: read them with ld.cg).
-__device__ __noinline__ void probe_head(const float *qpart, const float *ktT, int32_t *probe_list, const SelGeom &g, int h, int n,
+// Probe of one QUERY_PROBE head, run by a whole CTA (256 threads) of the select launch: qbar = (1/N) sum_t q_t from the
+// per-CTA token sums of the pool launch, p[J] = qbar . Ktilde_J / sqrt(D), top-n -> probe_list[h][0..n).
+__device__ inline void probe_head(const float *qpart, const float *kt, int32_t *probe_list, const SelGeom &g, int h, int n,
                                   uint32_t *key /* dynamic smem, NB */, float (*part)[64], float *qb) {
   const int nparts = (g.NB + 7) / 8;
   {
     const int d = threadIdx.x & 63, grp = threadIdx.x >> 6;
     const float *base = qpart + (int64_t)h * nparts * 64 + d;
     float a0 = 0.f;
-    for (int c = grp; c < nparts; c += 4) a0 += __ldcg(base + (int64_t)c * 64);
+    for (int c0 = grp; c0 < nparts; c0 += 32) {  // eight loads in flight, summed in a fixed order
+      float t[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) t[i] = (c0 + 4 * i < nparts) ? __ldcg(base + (int64_t)(c0 + 4 * i) * 64) : 0.f;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) a0 += t[i];
+    }
     part[grp][d] = a0;
     __syncthreads();
     if (threadIdx.x < 64) qb[threadIdx.x] = ((part[0][threadIdx.x] + part[1][threadIdx.x]) + (part[2][threadIdx.x] + part[3][threadIdx.x])) / (float)g.N;
     __syncthreads();
   }
+  const int64_t ld = kt_stride(g.NB);
   for (int J = threadIdx.x; J < g.NB; J += 256) {
-    const float *kc = ktT + (int64_t)h * 64 * g.NB + J;
+    const float *kc = kt + (int64_t)h * 64 * ld + J;
     float acc = 0.f;
-#pragma unroll 16
-    for (int d = 0; d < 64; ++d) acc = fmaf(qb[d], __ldcg(kc + (int64_t)d * g.NB), acc);
+#pragma unroll
+    for (int d0 = 0; d0 < 64; d0 += 16) {
+      float t[16];
+#pragma unroll
+      for (int i = 0; i < 16; ++i) t[i] = __ldcg(kc + (int64_t)(d0 + i) * ld);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) acc = fmaf(qb[d0 + i], t[i], acc);
+    }
     key[J] = score_key(acc * 0.125f);
   }
   __syncthreads();
@@ -265,10 +345,20 @@ __device__ __noinline__ void probe_head(const float *qpart, const float *ktT, in
 }
 
 __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
-                                                          float *__restrict__ qt, float *__restrict__ ktT, float *__restrict__ qpart,
-                                                          int32_t *__restrict__ probe_list, int64_t *__restrict__ row_ptr,
-                                                          uint32_t *__restrict__ done /* ctx-owned [H], zero between calls */,
-                                                          SelGeom g, PoolJobs jobs, RowPtrPlan plan, HeadCfgArray cfg, int pool_ctas) {
+                                                          float *__restrict__ qt, float *__restrict__ kt, float *__restrict__ qpart,
+                                                          int64_t *__restrict__ row_ptr, int32_t *__restrict__ col_idx, SelGeom g, PoolJobs jobs, RowPtrPlan plan,
+                                                          HeadCfgArray cfg, HeadSets sets, int pool_ctas) {
+  if ((int)blockIdx.x >= pool_ctas + g.H) {
+    // ---------------------------------------------------------------- lists of a constant-length closed-form head
+    const int chunks = (g.NB + kLightRows - 1) / kLightRows;
+    const int e = (int)blockIdx.x - pool_ctas - g.H;
+    const int h = sets.emit[e / chunks];
+    const int I0 = (e % chunks) * kLightRows;
+    const int warp = threadIdx.x >> 5;
+    for (int r = warp; r < kLightRows && I0 + r < g.NB; r += 8)
+      emit_light_row(g, cfg.c[h], h, I0 + r, col_idx + plan.head_base[h] + (int64_t)(I0 + r) * plan.const_len[h], nullptr);
+    return;
+  }
   if ((int)blockIdx.x >= pool_ctas) {
     // ---------------------------------------------------------------- row_ptr of one head
     const int h = blockIdx.x - pool_ctas;
@@ -301,10 +391,7 @@ __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16
   }
   // ------------------------------------------------------------------ pool: one warp per token block
   // CTA c of a job covers blocks 8c .. 8c+7 (jobs are padded to a multiple of 8 blocks, so a CTA never straddles jobs)
-  extern __shared__ uint32_t probe_key[];  // NB keys, used only by the last CTA of a QUERY_PROBE head
   __shared__ float qsum[8][64];
-  __shared__ float qb[64];
-  __shared__ int is_last;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ctas_per_job = (g.NB + 7) / 8;
   const int job = blockIdx.x / ctas_per_job, cta_in_job = blockIdx.x % ctas_per_job;
@@ -363,46 +450,35 @@ __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16
         float4 *dst = reinterpret_cast<float4 *>(qt + ((int64_t)h * g.NB + J) * 64 + sub * 8);
         dst[0] = make_float4(acc[0] * invc, acc[1] * invc, acc[2] * invc, acc[3] * invc);
         dst[1] = make_float4(acc[4] * invc, acc[5] * invc, acc[6] * invc, acc[7] * invc);
-      } else {  // Ktilde TRANSPOSED [H][64][NB]: the score kernels read it coalesced over J
+      } else {  // Ktilde transposed [H][64][NBp]
+        const int64_t ld = kt_stride(g.NB);
 #pragma unroll
-        for (int c = 0; c < 8; ++c) ktT[((int64_t)h * 64 + sub * 8 + c) * g.NB + J] = acc[c] * invc;
+        for (int c = 0; c < 8; ++c) kt[((int64_t)h * 64 + sub * 8 + c) * ld + J] = acc[c] * invc;
       }
     }
   }
-  if (!probe) return;  // CTA-uniform
-  if (want_part) {
-    if (rg == 0) {
+  if (!want_part) return;  // CTA-uniform
+  if (rg == 0) {
 #pragma unroll
-      for (int c = 0; c < 8; ++c) qsum[warp][sub * 8 + c] = acc[c];  // zero for warps past the last block
-    }
-    __syncthreads();
-    if (warp == 0) {
-#pragma unroll
-      for (int d = lane; d < 64; d += 32) {
-        float t = 0.f;
-#pragma unroll
-        for (int w = 0; w < 8; ++w) t += qsum[w][d];
-        qpart[((int64_t)h * ctas_per_job + cta_in_job) * 64 + d] = t;
-      }
-    }
-  }
-  // last-CTA-done: every thread's global writes are fenced, then one thread takes a ticket
-  __threadfence();
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    const uint32_t t = atomicAdd(&done[h], 1u);
-    is_last = (t == 2u * (uint32_t)ctas_per_job - 1u);
-    if (is_last) done[h] = 0u;  // self-reset for the next call (all other CTAs of this head have already arrived)
+    for (int c = 0; c < 8; ++c) qsum[warp][sub * 8 + c] = acc[c];  // zero for warps past the last block
   }
   __syncthreads();
-  if (!is_last) return;
-  __threadfence();
-  probe_head(qpart, ktT, probe_list, g, h, (int)i64min(cfg.c[h].keep_blocks, g.NB), probe_key, qsum, qb);
+  if (warp == 0) {
+#pragma unroll
+    for (int d = lane; d < 64; d += 32) {
+      float t = 0.f;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) t += qsum[w][d];
+      qpart[((int64_t)h * ctas_per_job + cta_in_job) * 64 + d] = t;
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ select
-// grid (ceil(NB/R), H), 256 threads (8 warps), R = 16 rows (fewer when NB is large) per CTA.
-//   closed-form heads: lane-parallel emitters;  QUERY_PROBE heads: copy the head's probe list into every row;
+// 1-D grid, 256 threads (8 warps).  phase 0: one probe CTA per QUERY_PROBE head, then n_block * ceil(NB/R) heavy CTAs
+// (R = 16 rows, fewer when NB is large or the BLOCK_TOPK heads are few), then light CTAs (32 rows each) for the per-row-length
+// STATIC heads.  phase 1 (a second, small launch, only if there are QUERY_PROBE heads): light CTAs copy each head's probe
+// list into every row.
 //   BLOCK_TOPK heads: score rows s[I][J] = Qtilde_I . Ktilde_J * c (fp32 FMA in the order d = 0..63, as packed
 //   row pairs; each thread owns two columns J and keeps 16 row accumulators for each) stored as order-preserving keys
 //   in shared memory, then one warp per row: bisection top-n or per-frame top-k.
@@ -420,107 +496,129 @@ __device__ __forceinline__ uint64_t sel_fma2(uint64_t a, uint64_t b, uint64_t c)
   return d;
 }
 
-__global__ void __launch_bounds__(256, 2) select_kernel(const float *__restrict__ qt, const float *__restrict__ ktT,
-                                                        const int32_t *__restrict__ probe_list, const int64_t *__restrict__ row_ptr,
-                                                        int32_t *__restrict__ col_idx, SelGeom g, HeadCfgArray cfg, int R) {
-  const int h = blockIdx.y;
-  const saf3r_head_cfg c = cfg.c[h];
-  const int I0 = blockIdx.x * R;
-  const int rows = (int)i64min(R, g.NB - I0);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  extern __shared__ float sm[];
-
-  if (c.type != SAF3R_HEAD_BLOCK_TOPK) {
-    for (int r = warp; r < rows; r += 8) {
-      const int64_t I = I0 + r;
-      int32_t *out = col_idx + row_ptr[(int64_t)h * g.NB + I];
-      if (c.type == SAF3R_HEAD_QUERY_PROBE_TOPK) {
-        const int n = (int)i64min(c.keep_blocks, g.NB);
-        for (int i = lane; i < n; i += 32) out[i] = probe_list[(int64_t)h * g.NB + i];
-      } else if (c.type == SAF3R_HEAD_DENSE) {
-        for (int J = lane; J < g.NB; J += 32) out[J] = J;
-      } else if (c.type == SAF3R_HEAD_UNIFORM_STRIDE && c.stride >= 1) {
-        const int n = (g.NB - c.offset + c.stride - 1) / c.stride;
-        for (int i = lane; i < n; i += 32) out[i] = c.offset + i * c.stride;
-      } else if (c.type == SAF3R_HEAD_UNIFORM_STRIDE) {  // keep_blocks form (n <= NB, so the indices are distinct)
-        for (int i = lane; i < c.keep_blocks; i += 32) out[i] = (int32_t)(((int64_t)i * g.NB) / c.keep_blocks);
-      } else if (c.type == SAF3R_HEAD_STATIC && c.static_mode != SAF3R_STATIC_POSITION_BAND) {  // one contiguous range
-        int64_t lo, hi;
-        if (c.static_mode == SAF3R_STATIC_ANCHOR) {
-          lo = ((int64_t)c.anchor_frame * g.T) / g.B;
-          hi = (((int64_t)c.anchor_frame + 1) * g.T - 1) / g.B;
-        } else {
-          const int64_t t0 = I * g.B, t1 = i64min(t0 + g.B, g.N);
-          lo = ((t0 / g.T) * g.T) / g.B;
-          hi = (((t1 - 1) / g.T + 1) * g.T - 1) / g.B;
-        }
-        for (int64_t J = lo + lane; J <= hi; J += 32) out[J - lo] = (int32_t)J;
-      } else if (lane == 0) {
-        int64_t w = 0;
-        closed_form_row(g, c, I, [&](int64_t J) { out[w++] = (int32_t)J; });
-      }
-    }
-    return;
-  }
-
-  uint32_t *keys = reinterpret_cast<uint32_t *>(sm);   // [R][NB]
-  float *qT = sm + (size_t)R * g.NB;                   // [64][kSelRows] (rows past `rows` are zero)
-  for (int i = threadIdx.x; i < 64 * kSelRows; i += blockDim.x) {
-    const int d = i / kSelRows, r = i % kSelRows;
+// Score rows I0 .. I0+rows-1 (rows <= RT) of head h against every k-block: keys[r][J] = key(Qtilde_{I0+r} . Ktilde_J * cs).
+// Groups of 1024 columns: each thread owns four consecutive columns (one 16-byte load of Ktilde^T per d, coalesced across
+// the warp) and RT rows, 4*RT accumulators as packed row pairs.  The columns left over (< 1024) are spread over all threads
+// as (row, four columns) tasks.  Every sum runs in the order d = 0..63 with fp32 FMAs, so both paths give the same bits.
+template <int RT>
+__device__ __forceinline__ void score_rows(const float *__restrict__ qt, const float *__restrict__ kt, uint32_t *keys, float *qT,
+                                           const SelGeom &g, int h, int I0, int rows, float cs) {
+  for (int i = threadIdx.x; i < 64 * RT; i += blockDim.x) {
+    const int d = i / RT, r = i % RT;
     qT[i] = r < rows ? qt[((int64_t)h * g.NB + I0 + r) * 64 + d] : 0.f;
   }
   __syncthreads();
-  const float cs = c.score_mode == SAF3R_SCORE_COSINE ? 1.f : 0.125f;
-  const float *kh = ktT + (int64_t)h * 64 * g.NB;
-  for (int J0 = threadIdx.x; J0 < g.NB; J0 += 512) {
-    const int J1 = J0 + 256;
-    const bool has1 = J1 < g.NB;
-    uint64_t a0[kSelRows / 2], a1[kSelRows / 2];
+  const int64_t ld = kt_stride(g.NB);
+  const float *kh = kt + (int64_t)h * 64 * ld;
+  int Jb = 0;
+  for (; Jb + 1024 <= g.NB; Jb += 1024) {
+    const int J = Jb + 4 * (int)threadIdx.x;
+    uint64_t a[4][RT / 2];
 #pragma unroll
-    for (int r = 0; r < kSelRows / 2; ++r) a0[r] = a1[r] = 0ull;
-#pragma unroll 2
-    for (int d0 = 0; d0 < 64; d0 += 8) {
-      float k0[8], k1[8];
+    for (int c = 0; c < 4; ++c)
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        k0[i] = __ldg(kh + (int64_t)(d0 + i) * g.NB + J0);
-        k1[i] = has1 ? __ldg(kh + (int64_t)(d0 + i) * g.NB + J1) : 0.f;
-      }
+      for (int r = 0; r < RT / 2; ++r) a[c][r] = 0ull;
+    const float *kp = kh + J;
+#pragma unroll 4
+    for (int d = 0; d < 64; ++d) {
+      const float4 kv = __ldg(reinterpret_cast<const float4 *>(kp + (int64_t)d * ld));
+      const uint64_t k0 = sel_pack2(kv.x, kv.x), k1 = sel_pack2(kv.y, kv.y), k2 = sel_pack2(kv.z, kv.z), k3 = sel_pack2(kv.w, kv.w);
+      const float4 *qr = reinterpret_cast<const float4 *>(qT + d * RT);
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const float4 *qr = reinterpret_cast<const float4 *>(qT + (d0 + i) * kSelRows);
-        const uint64_t kk0 = sel_pack2(k0[i], k0[i]), kk1 = sel_pack2(k1[i], k1[i]);
-#pragma unroll
-        for (int r4 = 0; r4 < kSelRows / 4; ++r4) {
-          const float4 t = qr[r4];
-          const uint64_t qa = sel_pack2(t.x, t.y), qb = sel_pack2(t.z, t.w);
-          a0[2 * r4] = sel_fma2(qa, kk0, a0[2 * r4]);
-          a0[2 * r4 + 1] = sel_fma2(qb, kk0, a0[2 * r4 + 1]);
-          a1[2 * r4] = sel_fma2(qa, kk1, a1[2 * r4]);
-          a1[2 * r4 + 1] = sel_fma2(qb, kk1, a1[2 * r4 + 1]);
-        }
+      for (int r4 = 0; r4 < RT / 4; ++r4) {
+        const float4 t = qr[r4];
+        const uint64_t qa = sel_pack2(t.x, t.y), qb = sel_pack2(t.z, t.w);
+        a[0][2 * r4] = sel_fma2(qa, k0, a[0][2 * r4]);
+        a[0][2 * r4 + 1] = sel_fma2(qb, k0, a[0][2 * r4 + 1]);
+        a[1][2 * r4] = sel_fma2(qa, k1, a[1][2 * r4]);
+        a[1][2 * r4 + 1] = sel_fma2(qb, k1, a[1][2 * r4 + 1]);
+        a[2][2 * r4] = sel_fma2(qa, k2, a[2][2 * r4]);
+        a[2][2 * r4 + 1] = sel_fma2(qb, k2, a[2][2 * r4 + 1]);
+        a[3][2 * r4] = sel_fma2(qa, k3, a[3][2 * r4]);
+        a[3][2 * r4 + 1] = sel_fma2(qb, k3, a[3][2 * r4 + 1]);
       }
     }
 #pragma unroll
-    for (int r2 = 0; r2 < kSelRows / 2; ++r2) {
-      float lo, hi;
-      asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a0[r2]));
-      if (2 * r2 < rows) keys[(size_t)(2 * r2) * g.NB + J0] = score_key(lo * cs);
-      if (2 * r2 + 1 < rows) keys[(size_t)(2 * r2 + 1) * g.NB + J0] = score_key(hi * cs);
-      if (has1) {
-        asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a1[r2]));
-        if (2 * r2 < rows) keys[(size_t)(2 * r2) * g.NB + J1] = score_key(lo * cs);
-        if (2 * r2 + 1 < rows) keys[(size_t)(2 * r2 + 1) * g.NB + J1] = score_key(hi * cs);
-      }
+    for (int r2 = 0; r2 < RT / 2; ++r2) {
+      float lo[4], hi[4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) asm("mov.b64 {%0, %1}, %2;" : "=f"(lo[c]), "=f"(hi[c]) : "l"(a[c][r2]));
+      if (2 * r2 < rows)
+        *reinterpret_cast<uint4 *>(keys + (size_t)(2 * r2) * ld + J) =
+            make_uint4(score_key(lo[0] * cs), score_key(lo[1] * cs), score_key(lo[2] * cs), score_key(lo[3] * cs));
+      if (2 * r2 + 1 < rows)
+        *reinterpret_cast<uint4 *>(keys + (size_t)(2 * r2 + 1) * ld + J) =
+            make_uint4(score_key(hi[0] * cs), score_key(hi[1] * cs), score_key(hi[2] * cs), score_key(hi[3] * cs));
     }
   }
+  // left-over columns: (row, column quad) tasks; the padded columns NB..NBp-1 of Ktilde^T are never written, so their
+  // scores are computed from garbage and stored into the row's padding, which nothing reads
+  const int quads = (int)((ld - Jb) / 4);
+  for (int idx = threadIdx.x; idx < quads * rows; idx += blockDim.x) {
+    const int r = idx / quads, J = Jb + 4 * (idx % quads);
+    const float *kp = kh + J;
+    float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll 8
+    for (int d = 0; d < 64; ++d) {
+      const float4 kv = __ldg(reinterpret_cast<const float4 *>(kp + (int64_t)d * ld));
+      const float qv = qT[d * RT + r];
+      a0 = fmaf(qv, kv.x, a0);
+      a1 = fmaf(qv, kv.y, a1);
+      a2 = fmaf(qv, kv.z, a2);
+      a3 = fmaf(qv, kv.w, a3);
+    }
+    *reinterpret_cast<uint4 *>(keys + (size_t)r * ld + J) =
+        make_uint4(score_key(a0 * cs), score_key(a1 * cs), score_key(a2 * cs), score_key(a3 * cs));
+  }
+}
+
+__global__ void __launch_bounds__(256, 2) select_kernel(const float *__restrict__ qt, const float *__restrict__ kt,
+                                                        const int32_t *__restrict__ probe_list, const int64_t *__restrict__ row_ptr,
+                                                        const float *__restrict__ qpart, int32_t *__restrict__ probe_out,
+                                                        int32_t *__restrict__ col_idx, SelGeom g, HeadCfgArray cfg, HeadSets sets, int R,
+                                                        int phase) {
+  const int warp = threadIdx.x >> 5;
+  extern __shared__ float sm[];
+  __shared__ float part[4][64];
+  __shared__ float qb[64];
+  const int strips = (g.NB + R - 1) / R;
+  const int probe_ctas = phase == 0 ? sets.n_probe : 0;
+  const int heavy_ctas = phase == 0 ? sets.n_block * strips : 0;
+  if ((int)blockIdx.x < probe_ctas) {
+    const int h = sets.probe[blockIdx.x];
+    probe_head(qpart, kt, probe_out, g, h, (int)i64min(cfg.c[h].keep_blocks, g.NB), reinterpret_cast<uint32_t *>(sm), part, qb);
+    return;
+  }
+  const int bid = (int)blockIdx.x - probe_ctas;
+  if (bid >= heavy_ctas) {
+    // light CTAs come last in launch order, 32 rows each: per-row-length STATIC heads (phase 0), QUERY_PROBE heads (phase 1)
+    const int chunks = (g.NB + kLightRows - 1) / kLightRows;
+    const int e = bid - heavy_ctas;
+    const int h = phase == 0 ? sets.light[e / chunks] : sets.probe[e / chunks];
+    const int I0 = (e % chunks) * kLightRows;
+    for (int r = warp; r < kLightRows && I0 + r < g.NB; r += 8)
+      emit_light_row(g, cfg.c[h], h, I0 + r, col_idx + row_ptr[(int64_t)h * g.NB + I0 + r], probe_list);
+    return;
+  }
+  const int h = sets.block[bid / strips];
+  const saf3r_head_cfg c = cfg.c[h];
+  const int I0 = (bid % strips) * R;
+  const int rows = (int)i64min(R, g.NB - I0);
+
+  uint32_t *keys = reinterpret_cast<uint32_t *>(sm);   // [R][NBp]
+  const int64_t ld = kt_stride(g.NB);                  // key rows are padded like Ktilde^T
+  float *qT = sm + (size_t)R * ld;                     // [64][RT] (rows past `rows` are zero)
+  const float cs = c.score_mode == SAF3R_SCORE_COSINE ? 1.f : 0.125f;
+  if (R <= 4) score_rows<4>(qt, kt, keys, qT, g, h, I0, rows, cs);
+  else if (R <= 8) score_rows<8>(qt, kt, keys, qT, g, h, I0, rows, cs);
+  else score_rows<kSelRows>(qt, kt, keys, qT, g, h, I0, rows, cs);
   __syncthreads();
   for (int r = warp; r < rows; r += 8) {
     int32_t *out = col_idx + row_ptr[(int64_t)h * g.NB + I0 + r];
     if (c.topk_scope == SAF3R_SCOPE_GLOBAL)
-      warp_topn_bisect(keys + (size_t)r * g.NB, g.NB, (int)i64min(c.keep_blocks, g.NB), out);
+      warp_topn_bisect(keys + (size_t)r * ld, g.NB, (int)i64min(c.keep_blocks, g.NB), out);
     else
-      warp_per_frame_emit(keys + (size_t)r * g.NB, g, c.topk_per_frame, out);
+      warp_per_frame_emit(keys + (size_t)r * ld, g, c.topk_per_frame, out);
   }
 }
 
