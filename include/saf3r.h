@@ -31,7 +31,9 @@
 extern "C" {
 #endif
 
+#ifndef SAF3R_MAX_HEADS
 #define SAF3R_MAX_HEADS 64 /* per call; a batch folds into the head dimension */
+#endif
 
 typedef struct saf3r_ctx saf3r_ctx; /* opaque; owns its tensor-map cache, a tiny device scratch and the error string */
 

@@ -321,13 +321,7 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
   }
   const int sel_ctas = sets.n_probe + sets.n_block * ((g.NB + R - 1) / R) + sets.n_light * light_chunks;
   if (sel_ctas > 0) {
-    select_kernel<<<sel_ctas, 256, sm, st>>>(qt, kt, probe, lists->row_ptr, qpart, probe, lists->col_idx, g, ca, sets, R, 0);
-    ctx->launches += 1;
-  }
-  // launch 3: every row of a QUERY_PROBE head gets a copy of the head's probe list
-  if (sets.n_probe > 0) {
-    select_kernel<<<sets.n_probe * light_chunks, 256, 0, st>>>(qt, kt, probe, lists->row_ptr, qpart, probe, lists->col_idx, g, ca, sets,
-                                                              R, 1);
+    select_kernel<<<sel_ctas, 256, sm, st>>>(qt, kt, probe, lists->row_ptr, qpart, probe, lists->col_idx, g, ca, sets, R);
     ctx->launches += 1;
   }
   if (ctx->stage_timing) {

@@ -272,7 +272,7 @@ struct HeadSets {
   uint8_t emit[SAF3R_MAX_HEADS];   // launch 1: closed-form heads whose rows all have the same length (no dependence at all)
   uint8_t light[SAF3R_MAX_HEADS];  // launch 2: per-row-length STATIC heads (need row_ptr)
   uint8_t block[SAF3R_MAX_HEADS];  // launch 2: BLOCK_TOPK heads (score + top-n)
-  uint8_t probe[SAF3R_MAX_HEADS];  // launch 2: QUERY_PROBE heads, one probe CTA each; launch 3: copy of the probe list into every row
+  uint8_t probe[SAF3R_MAX_HEADS];  // launch 2: QUERY_PROBE heads, one probe CTA each (probe + the head's lists)
 };
 
 // ------------------------------------------------------------------------------------------------ pool + row_ptr + probe
@@ -307,8 +307,8 @@ __device__ __forceinline__ uint4 ld_stream_16(const void *p) {
 
 // Probe of one QUERY_PROBE head, run by a whole CTA (256 threads) of the select launch: qbar = (1/N) sum_t q_t from the
 // per-CTA token sums of the pool launch, p[J] = qbar . Ktilde_J / sqrt(D), top-n -> probe_list[h][0..n).
-__device__ inline void probe_head(const float *qpart, const float *kt, int32_t *probe_list, const SelGeom &g, int h, int n,
-                                  uint32_t *key /* dynamic smem, NB */, float (*part)[64], float *qb) {
+__device__ inline void probe_head(const float *qpart, const float *kt, int32_t *probe_list, int32_t *head_lists, const SelGeom &g,
+                                  int h, int n, uint32_t *key /* dynamic smem, NB */, float (*part)[64], float *qb) {
   const int nparts = (g.NB + 7) / 8;
   {
     const int d = threadIdx.x & 63, grp = threadIdx.x >> 6;
@@ -342,6 +342,20 @@ __device__ inline void probe_head(const float *qpart, const float *kt, int32_t *
   }
   __syncthreads();
   if (threadIdx.x < 32) warp_topn_bisect(key, g.NB, n, probe_list + (int64_t)h * g.NB);
+  __syncthreads();
+  // every q-block of the head gets the same list: its NB rows of n entries are contiguous in col_idx, so the region is the
+  // list repeated NB times; written here with coalesced stores while the score CTAs of the launch are still busy
+  int32_t *list = reinterpret_cast<int32_t *>(key);
+  for (int i = threadIdx.x; i < n; i += 256) list[i] = __ldcg(probe_list + (int64_t)h * g.NB + i);  // this CTA's own global writes
+  __syncthreads();
+  const int64_t total = (int64_t)g.NB * n;
+  int m = (int)(threadIdx.x % (unsigned)n);
+  const int step = 256 % n;
+  for (int64_t idx = threadIdx.x; idx < total; idx += 256) {
+    head_lists[idx] = list[m];
+    m += step;
+    if (m >= n) m -= n;
+  }
 }
 
 __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
@@ -475,10 +489,9 @@ __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16
 }
 
 // ------------------------------------------------------------------------------------------------ select
-// 1-D grid, 256 threads (8 warps).  phase 0: one probe CTA per QUERY_PROBE head, then n_block * ceil(NB/R) heavy CTAs
-// (R = 16 rows, fewer when NB is large or the BLOCK_TOPK heads are few), then light CTAs (32 rows each) for the per-row-length
-// STATIC heads.  phase 1 (a second, small launch, only if there are QUERY_PROBE heads): light CTAs copy each head's probe
-// list into every row.
+// 1-D grid, 256 threads (8 warps): one probe CTA per QUERY_PROBE head (probe, top-n, and the head's lists), then
+// n_block * ceil(NB/R) heavy CTAs (R = 16 rows, fewer when NB is large or the BLOCK_TOPK heads are few), then light CTAs
+// (32 rows each) for the per-row-length STATIC heads.
 //   BLOCK_TOPK heads: score rows s[I][J] = Qtilde_I . Ktilde_J * c (fp32 FMA in the order d = 0..63, as packed
 //   row pairs; each thread owns two columns J and keeps 16 row accumulators for each) stored as order-preserving keys
 //   in shared memory, then one warp per row: bisection top-n or per-frame top-k.
@@ -575,26 +588,26 @@ __device__ __forceinline__ void score_rows(const float *__restrict__ qt, const f
 __global__ void __launch_bounds__(256, 2) select_kernel(const float *__restrict__ qt, const float *__restrict__ kt,
                                                         const int32_t *__restrict__ probe_list, const int64_t *__restrict__ row_ptr,
                                                         const float *__restrict__ qpart, int32_t *__restrict__ probe_out,
-                                                        int32_t *__restrict__ col_idx, SelGeom g, HeadCfgArray cfg, HeadSets sets, int R,
-                                                        int phase) {
+                                                        int32_t *__restrict__ col_idx, SelGeom g, HeadCfgArray cfg, HeadSets sets, int R) {
   const int warp = threadIdx.x >> 5;
   extern __shared__ float sm[];
   __shared__ float part[4][64];
   __shared__ float qb[64];
   const int strips = (g.NB + R - 1) / R;
-  const int probe_ctas = phase == 0 ? sets.n_probe : 0;
-  const int heavy_ctas = phase == 0 ? sets.n_block * strips : 0;
+  const int probe_ctas = sets.n_probe;
+  const int heavy_ctas = sets.n_block * strips;
   if ((int)blockIdx.x < probe_ctas) {
     const int h = sets.probe[blockIdx.x];
-    probe_head(qpart, kt, probe_out, g, h, (int)i64min(cfg.c[h].keep_blocks, g.NB), reinterpret_cast<uint32_t *>(sm), part, qb);
+    probe_head(qpart, kt, probe_out, col_idx + row_ptr[(int64_t)h * g.NB], g, h, (int)i64min(cfg.c[h].keep_blocks, g.NB),
+               reinterpret_cast<uint32_t *>(sm), part, qb);
     return;
   }
   const int bid = (int)blockIdx.x - probe_ctas;
   if (bid >= heavy_ctas) {
-    // light CTAs come last in launch order, 32 rows each: per-row-length STATIC heads (phase 0), QUERY_PROBE heads (phase 1)
+    // light CTAs come last in launch order, 32 rows each: per-row-length STATIC heads
     const int chunks = (g.NB + kLightRows - 1) / kLightRows;
     const int e = bid - heavy_ctas;
-    const int h = phase == 0 ? sets.light[e / chunks] : sets.probe[e / chunks];
+    const int h = sets.light[e / chunks];
     const int I0 = (e % chunks) * kLightRows;
     for (int r = warp; r < kLightRows && I0 + r < g.NB; r += 8)
       emit_light_row(g, cfg.c[h], h, I0 + r, col_idx + row_ptr[(int64_t)h * g.NB + I0 + r], probe_list);
