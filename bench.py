@@ -46,36 +46,58 @@ def shape_for(name: str) -> sy.Shape:
     return {"c2": sy.shape_c2, "c3": sy.shape_c3, "c4": sy.shape_c4, "c5": sy.shape_c5}[name]()
 
 
-def make_layers(name: str, count: int):
+def make_layers(name: str, count: int, gen: str | None = None, ratio: float | None = None):
     sh = shape_for(name)
     layers = []
     for l in range(count):
-        if name == "c3":
+        if name == "c3" and gen is None:
             layers.append(sy.config_c3_layer(l, sh=sh))
         else:
-            gens, cfgs = sy.mixed_heads(sh)
-            layers.append(sy.make_layer(sh, gens, cfgs, seed={"c2": 2, "c4": 4, "c5": 5}[name] * 1000 + l, layer=l))
+            gens, cfgs = sy.sweep_heads(sh, gen, ratio) if gen is not None else sy.mixed_heads(sh)
+            layers.append(sy.make_layer(sh, gens, cfgs, seed={"c2": 2, "c3": 3, "c4": 4, "c5": 5}[name] * 1000 + l, layer=l))
     return layers
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    """Samples SM clock / throttle reasons / power during the timed region (NVML every 20 ms; nvidia-smi as a fallback)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
         self.index, self.rows, self.stop, self.t = index, [], threading.Event(), None
+        self.nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nvml = pynvml
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(index)
+        except Exception:
+            self.nvml = None
+
+    def _sample_nvml(self):
+        n = self.nvml
+        sm = n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM)
+        mx = n.nvmlDeviceGetMaxClockInfo(self.handle, n.NVML_CLOCK_SM)
+        pw = n.nvmlDeviceGetPowerUsage(self.handle) / 1000.0
+        r = n.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle)
+        flag = lambda b: "Active" if (r & b) else "Not Active"
+        return [str(sm), str(mx), f"{pw:.1f}", flag(n.nvmlClocksThrottleReasonHwSlowdown),
+                flag(n.nvmlClocksThrottleReasonHwThermalSlowdown), flag(n.nvmlClocksThrottleReasonSwThermalSlowdown),
+                flag(n.nvmlClocksThrottleReasonSwPowerCap)]
 
     def _run(self):
         while not self.stop.is_set():
             try:
-                o = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
-                                   capture_output=True, text=True, timeout=5).stdout.strip()
-                if o:
-                    self.rows.append([x.strip() for x in o.split(",")])
+                if self.nvml is not None:
+                    self.rows.append(self._sample_nvml())
+                else:
+                    o = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                       capture_output=True, text=True, timeout=5).stdout.strip()
+                    if o:
+                        self.rows.append([x.strip() for x in o.split(",")])
             except Exception:
                 pass
-            self.stop.wait(0.2)
+            self.stop.wait(0.02 if self.nvml is not None else 0.2)
 
     def __enter__(self):
         self.t = threading.Thread(target=self._run, daemon=True)
@@ -89,10 +111,11 @@ class ClockSampler:
     def summary(self):
         sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
         mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        pw = [float(r[2]) for r in self.rows if len(r) > 2 and r[2].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = sorted({n for r in self.rows if len(r) >= 7 for n, v in zip(names, r[3:7]) if v.lower().startswith("active")})
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
-                "samples": len(sm)}
+                "samples": len(sm), "power_w_max": max(pw) if pw else None, "source": "nvml" if self.nvml is not None else "nvidia-smi"}
 
 
 def cpu_oracle_layer_ms(L: sy.Layer, qblocks_per_head: int, one_per_type: bool = False):
@@ -147,10 +170,12 @@ def run_reference(args):
     }))
 
 
-def workload_name(cfg: str, sh: sy.Shape) -> str:
-    return (f"{cfg.upper()}: one global-attention layer, S={sh.S} frames x T={sh.T} tokens, N={sh.N}, H={sh.H}, D={sh.D}, "
-            f"block {sh.B}, seeded per-layer mix of head types (uniform-stride / frame-local / same-position block top-k / "
-            f"sink query-probe) and sparsity")
+def workload_name(cfg: str, sh: sy.Shape, gen: str | None = None, ratio: float | None = None) -> str:
+    base = f"{cfg.upper()}: one global-attention layer, S={sh.S} frames x T={sh.T} tokens, N={sh.N}, H={sh.H}, D={sh.D}, block {sh.B}, "
+    if gen is not None:
+        return base + f"all heads of generator '{gen}' at kept-block ratio {ratio:g}"
+    return base + ("seeded per-layer mix of head types (uniform-stride / frame-local / same-position block top-k / "
+                   "sink query-probe) and sparsity")
 
 
 def run_ours(args):
@@ -168,7 +193,7 @@ def run_ours(args):
     peaks = load_peaks()
     sh = shape_for(args.config)
     n_res = min(args.resident_layers, args.steps)
-    layers = make_layers(args.config, n_res)
+    layers = make_layers(args.config, n_res, args.gen, args.ratio)
     ctx = sf.Context(local)
     shape = sf.make_shape(sh.S, sh.T, sh.H, sh.D, sh.B)
     stream = torch.cuda.current_stream()
@@ -217,10 +242,8 @@ def run_ours(args):
         barrier()
     launches = ctx.launch_count() - launches0
     total_ms = t_beg.elapsed_time(t_end)
-    if world > 1:
-        t = torch.tensor([total_ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    from paper_2607_03612_b200.sharding import max_over_ranks
+    total_ms = max_over_ranks(total_ms, dev)                     # device timing, MAX over ranks
     sel_ms = [e[0].elapsed_time(e[1]) for e in evs]
     att_ms = [e[1].elapsed_time(e[2]) for e in evs]
 
@@ -237,13 +260,15 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
         "data": "synthetic",
-        "config": {"workload": workload_name(args.config, sh), "resident_layers": n_res,
+        "config": {"workload": workload_name(args.config, sh, args.gen, args.ratio), "resident_layers": n_res,
                    "l2": "inputs (844 MB of Q/K/V per layer at C3) exceed the 126 MB L2; layers rotate" if args.config != "c2"
                    else "inputs 270 MB/layer exceed L2; layers rotate",
                    "kept_pair_ratio": float(np.mean(pairs)) / (sh.H * sh.NB * sh.NB)},
         "gpu_launches": int(launches),
         "select_ms": float(np.mean(sel_ms)), "sparse_attn_ms": float(np.mean(att_ms)),
         "executed_tflops": exec_tflops, "dense_equiv_tflops": dense_flop * args.steps / (total_ms * 1e-3) / 1e12,
+        "footprint_bytes": {"qkv_out": 4 * sh.H * sh.N * sh.D * 2, "lists": int(max(pairs)) * 4 + (sh.H * sh.NB + 1) * 8,
+                            "select_workspace": int(dl[0]["ws_bytes"])},
     }
 
     if rank == 0:
@@ -255,6 +280,7 @@ def run_ours(args):
             traffic = json.load(open(tp)).get("saf3r_attn_kernel_bytes_per_launch")
         result["roofline"] = {"bound": "tensor", "achieved": exec_tflops, "peak": peaks["tflops_sustained"], "unit": "TFLOP/s",
                               "frac": exec_tflops / peaks["tflops_sustained"], "traffic": traffic,
+                              "traffic_note": "ncu dram bytes of the layer-0 launch (profiles/traffic.json); achieved is the mean over the resident layers",
                               "kernel": "saf3r_attn_kernel", "peak_source": f"{peaks['source']} sustained bf16 (kernel timed inside a long step)",
                               "frac_of_burst": exec_tflops / peaks["tflops_burst"]}
         # selection pass against HBM: algorithmic bytes = Q and/or K of the heads whose rule reads them
@@ -331,6 +357,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c3", choices=["c2", "c3", "c4", "c5"])
     ap.add_argument("--resident-layers", type=int, default=4)
+    ap.add_argument("--gen", default=None, choices=[sy.GEN_UNIFORM, sy.GEN_SAME_POSITION, sy.GEN_SINK],
+                    help="sparsity sweep (C4): all heads of this generator type")
+    ap.add_argument("--ratio", type=float, default=None, help="sparsity sweep: kept-block ratio, e.g. 0.10")
     ap.add_argument("--dense-reps", type=int, default=2)
     ap.add_argument("--skip-dense", action="store_true")
     ap.add_argument("--skip-e2e", action="store_true")

@@ -227,3 +227,106 @@ def test_c2_dense_sampled_rows(env):
         check_attention(out[h].cpu().numpy(), ref, f"C2 dense head {h}")
         ref, _ = orc.attn_dense(L.q[h], L.k[h], L.v[h], sh.N - 64, sh.N)
         check_attention(out[h].cpu().numpy(), ref, f"C2 dense tail head {h}")
+
+
+# ------------------------------------------------------------------------------------------------ C3 (metric point), full size
+def test_c3_full_size_lists_and_sampled_attention(env):
+    """BASELINE.json's metric configuration (S=100, N=137400, NB=1074) in the launch configuration bench.py times:
+    lists of all 16 heads against the oracle (near-tie rule), attention on sampled q-blocks per head evaluated by the
+    oracle on the GPU's own lists (protocol iii), bf16 output path included."""
+    sf, ctx, torch = env
+    L = sy.config_c3_layer(0)
+    sh = L.shape
+    q, k, v = upload(L)
+    shape = c_shape(sf, sh)
+    lists = ctx.select(q, k, shape, L.cfgs)
+    out = ctx.sparse_attn(q, k, v, shape, lists, out_fp32=True)
+    out_bf = ctx.sparse_attn(q, k, v, shape, lists)
+    torch.cuda.synchronize()
+    hls = oracle_lists(L)
+    rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
+    stats = compare_lists(L, rp, col, hls)
+    print("C3 near-ties:", stats)
+    assert stats["tie_floored"] <= 1e-3 * stats["entries"]
+    rng = np.random.default_rng(3)
+    for h in range(sh.H):
+        qb = np.unique(np.concatenate([rng.choice(sh.NB, 1, replace=False), [sh.NB - 1]])).astype(np.int64)
+        r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
+        ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, r - r[0], col[r[0]:r[-1]], qb, want_lse=False)
+        check_attention(out[h].cpu().numpy(), ref, f"C3 head {h} ({L.gens[h]})")
+        m = ~np.isnan(ref)
+        assert np.abs(out_bf[h].float().cpu().numpy()[m] - ref[m]).max() <= 3e-2    # bf16 store adds its own rounding
+
+
+# ------------------------------------------------------------------------------------------------ top-n edge cases
+def test_select_planted_exact_ties(env):
+    """Identical K blocks give bit-identical scores: the cut must fall on the lower index (total order: score desc,
+    index asc), for the probe row and for every block-top-k row, with no near-tie excuse needed."""
+    sf, ctx, torch = env
+    gens = [sy.GEN_SAME_POSITION, sy.GEN_SINK, sy.GEN_UNIFORM]
+    cfgs = [sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=6),
+            sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=5),
+            sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=2)]
+    L = small_layer(6, 16, 3, 64, gens, cfgs, seed=21)          # T = 261, N = 1566, NB = 25
+    B = 64
+    for h in range(3):                                           # copy k-block 3 over k-blocks 7, 11, 12 and block 5 over 20
+        for dst, src in ((7, 3), (11, 3), (12, 3), (20, 5)):
+            L.k[h][dst * B:(dst + 1) * B] = L.k[h][src * B:(src + 1) * B]
+    q, k, _ = upload(L)
+    lists = ctx.select(q, k, c_shape(sf, L.shape), L.cfgs)
+    torch.cuda.synchronize()
+    rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
+    hls = oracle_lists(L)
+    for h, hl in enumerate(hls):
+        r = rp[h * L.shape.NB:(h + 1) * L.shape.NB + 1]
+        assert np.array_equal(r - r[0], hl.row_ptr)
+        assert np.array_equal(col[r[0]:r[-1]], hl.col_idx), f"head {h}: exact ties must be broken by the lower index"
+        if hl.scores is not None:                                # the planted ties really are exact in the oracle
+            assert np.all(hl.scores[:, 7] == hl.scores[:, 3]) and np.all(hl.scores[:, 12] == hl.scores[:, 3])
+
+
+def test_select_large_nb_paths(env):
+    """NB = 1160 > 1152: the top-n bisection reads its keys from shared memory (no register cache) and the score stage
+    runs its 1024-column main pass plus a left-over pass; n = NB keeps everything (degenerate cut)."""
+    sf, ctx, torch = env
+    gens = [sy.GEN_SAME_POSITION, sy.GEN_SINK, sy.GEN_SAME_POSITION, sy.GEN_UNIFORM]
+    sh = sy.Shape(S=54, G=37, H=4, D=64, B=64)                   # N = 74196, NB = 1160, tail 20
+    assert sh.NB == 1160
+    cfgs = [sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=97),
+            sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=54),
+            sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=2, score_mode=sy.SCORE_COSINE),
+            sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=sh.NB)]
+    L = sy.make_layer(sh, gens, cfgs, seed=22)
+    q, k, v = upload(L)
+    shape = c_shape(sf, sh)
+    lists = ctx.select(q, k, shape, L.cfgs)
+    out = ctx.sparse_attn(q, k, v, shape, lists, out_fp32=True)
+    torch.cuda.synchronize()
+    rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
+    stats = compare_lists(L, rp, col, oracle_lists(L))
+    print("NB=1160 near-ties:", stats)
+    assert stats["tie_floored"] <= 1e-3 * stats["entries"]
+    for h in (0, 1):
+        qb = np.array([3, sh.NB - 1], np.int64)
+        r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
+        ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, r - r[0], col[r[0]:r[-1]], qb, want_lse=False)
+        check_attention(out[h].cpu().numpy(), ref, f"NB=1160 head {h}")
+
+
+def test_select_is_deterministic_and_reusable(env):
+    """Two select calls into the same buffers give identical lists (no atomics, no run-to-run order dependence), and the
+    stage-timing aid does not change them."""
+    sf, ctx, torch = env
+    L = sy.config_c2()
+    q, k, _ = upload(L)
+    shape = c_shape(sf, L.shape)
+    lists = ctx.select(q, k, shape, L.cfgs)
+    torch.cuda.synchronize()
+    a = (lists.row_ptr.clone(), lists.col_idx.clone())
+    ctx.set_stage_timing(True)
+    lists.col_idx.zero_()
+    ctx.select(q, k, shape, L.cfgs, lists=lists)
+    pool_ms, sel_ms = ctx.last_select_stage_ms()
+    ctx.set_stage_timing(False)
+    assert pool_ms > 0 and sel_ms > 0
+    assert torch.equal(a[0], lists.row_ptr) and torch.equal(a[1], lists.col_idx)
