@@ -51,7 +51,10 @@ typedef enum {
   SAF3R_HEAD_UNIFORM_STRIDE = 1,   /* "Uniform Sampling Kernel", PAPER.md:L102 (scanning heads; also c_base, L106) */
   SAF3R_HEAD_STATIC = 2,           /* "Static Kernel", PAPER.md:L96 (position heads) */
   SAF3R_HEAD_QUERY_PROBE_TOPK = 3, /* "Query-Probe Top-K Kernel", PAPER.md:L98, L122-124 (vertical-line heads) */
-  SAF3R_HEAD_BLOCK_TOPK = 4        /* block-wise similarity Top-K, PAPER.md:L100, L126 (correspondence heads) */
+  SAF3R_HEAD_BLOCK_TOPK = 4,       /* block-wise similarity Top-K, PAPER.md:L100, L126 (correspondence heads) */
+  SAF3R_HEAD_CACHED = 5            /* reuse the lists of head `offset` of an index cache computed once per sequence
+                                      ("the indices are cached and reused by all subsequent ... kernels");
+                                      only valid in saf3r_select_cached */
 } saf3r_head_type;
 typedef enum { SAF3R_STATIC_ANCHOR = 0, SAF3R_STATIC_FRAME_LOCAL = 1, SAF3R_STATIC_POSITION_BAND = 2 } saf3r_static_mode;
 typedef enum { SAF3R_SCOPE_GLOBAL = 0, SAF3R_SCOPE_PER_FRAME = 1 } saf3r_topk_scope;
@@ -68,6 +71,8 @@ typedef enum { SAF3R_SCORE_DOT = 0, SAF3R_SCORE_COSINE = 1 } saf3r_score_mode;
  *   BLOCK_TOPK       s[I][J] = Qtilde_I . Ktilde_J * c (c = 1/sqrt(D) for DOT; COSINE pools L2-normalised tokens, c = 1);
  *                    GLOBAL: top-`keep_blocks` of the row; PER_FRAME: top-`topk_per_frame` inside each frame's
  *                    candidate blocks {J : floor(J*B/T) = g}, union over frames g.
+ *   CACHED           the rows of head `offset` of the cache passed to saf3r_select_cached, copied; keep_blocks / topk_scope /
+ *                    topk_per_frame must repeat the rule the cache head was built with (they fix the list lengths)
  *   Top-n uses the total order (score descending, then index ascending). */
 typedef struct {
   int32_t type;
@@ -108,6 +113,16 @@ saf3r_status saf3r_query_sizes(const saf3r_shape *shape, const saf3r_head_cfg *c
 saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const saf3r_shape *shape,
                           const saf3r_head_cfg *cfg_host, void *workspace_dev, size_t workspace_bytes,
                           saf3r_lists *out_lists, void *cuda_stream);
+
+/* Step 1 with an index cache: `cache` holds the lists of `cache_heads` BLOCK_TOPK heads
+ * computed ONCE per sequence by an ordinary saf3r_select call on a caller-supplied feature tensor (q = k = features,
+ * SAF3R_SCORE_COSINE reproduces the paper's cosine similarity of patch features at block level).  Heads of type
+ * SAF3R_HEAD_CACHED copy their rows from cache head `offset`; all other heads behave as in saf3r_select, so a layer whose
+ * correspondence heads are CACHED pools and scores only for its QUERY_PROBE heads.  The cache must have been built for the
+ * same (num_frames, tokens_per_frame, block); it is only read.  cache == NULL makes this identical to saf3r_select. */
+saf3r_status saf3r_select_cached(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const saf3r_shape *shape,
+                                 const saf3r_head_cfg *cfg_host, const saf3r_lists *cache, int32_t cache_heads,
+                                 void *workspace_dev, size_t workspace_bytes, saf3r_lists *out_lists, void *cuda_stream);
 
 /* Step 2: o_i = sum_j softmax_j(q_i.k_j/sqrt(D)) v_j over j in the blocks of list(h, blk(i)), j < N.
  * out_dev: bf16 (out_is_fp32 = 0) or fp32 (1), same [H][N][D] strides as q.  lse_dev_or_null: fp32 [H][N] contiguous,

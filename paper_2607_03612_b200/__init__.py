@@ -19,14 +19,14 @@ MAX_HEADS = 64
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CAPACITY, ERR_CUDA = range(5)
 _STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "CAPACITY", 4: "CUDA"}
 
-HEAD_DENSE, HEAD_UNIFORM_STRIDE, HEAD_STATIC, HEAD_QUERY_PROBE_TOPK, HEAD_BLOCK_TOPK = range(5)
+HEAD_DENSE, HEAD_UNIFORM_STRIDE, HEAD_STATIC, HEAD_QUERY_PROBE_TOPK, HEAD_BLOCK_TOPK, HEAD_CACHED = range(6)
 STATIC_ANCHOR, STATIC_FRAME_LOCAL, STATIC_POSITION_BAND = range(3)
 SCOPE_GLOBAL, SCOPE_PER_FRAME = range(2)
 SCORE_DOT, SCORE_COSINE = range(2)
 
 EXPORTS = ("saf3r_create", "saf3r_destroy", "saf3r_last_error", "saf3r_query_sizes", "saf3r_select", "saf3r_sparse_attn",
            "saf3r_dense_attn", "saf3r_layer_host_scratch_bytes", "saf3r_layer_host", "saf3r_launch_count",
-           "saf3r_set_stage_timing", "saf3r_last_select_stage_ms")
+           "saf3r_set_stage_timing", "saf3r_last_select_stage_ms", "saf3r_select_cached")
 
 
 class Saf3rError(RuntimeError):
@@ -69,6 +69,8 @@ def load_library():
         L.saf3r_last_error.restype = C.c_char_p
         L.saf3r_query_sizes.argtypes = [C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(i64), C.POINTER(C.c_size_t)]
         L.saf3r_select.argtypes = [vp, vp, vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), vp, C.c_size_t, C.POINTER(ListsC), vp]
+        L.saf3r_select_cached.argtypes = [vp, vp, vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(ListsC), C.c_int32, vp,
+                                          C.c_size_t, C.POINTER(ListsC), vp]
         L.saf3r_sparse_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(ListsC), vp, i32, vp, vp]
         L.saf3r_dense_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), vp, i32, vp, vp]
         L.saf3r_layer_host_scratch_bytes.argtypes = [C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(C.c_size_t)]
@@ -160,8 +162,11 @@ class Context:
     def query_sizes(self, shape: ShapeC, cfgs) -> tuple[int, int]:
         return query_sizes(shape, cfgs)
 
-    # ---- saf3r_select
-    def select(self, q, k, shape: ShapeC, cfgs, workspace=None, lists: Lists | None = None, stream=None) -> Lists:
+    # ---- saf3r_select / saf3r_select_cached
+    def select(self, q, k, shape: ShapeC, cfgs, workspace=None, lists: Lists | None = None, stream=None,
+               cache: Lists | None = None, cache_heads: int = 0) -> Lists:
+        """cache: lists of `cache_heads` heads built once per sequence (an ordinary select on features); heads of type
+        HEAD_CACHED copy their rows from cache head cfg['offset'] (saf3r_select_cached)."""
         import torch
         arr = make_cfgs(cfgs)
         entries, ws_bytes = query_sizes(shape, arr)
@@ -174,8 +179,14 @@ class Context:
             lists = Lists(torch.empty(shape.num_heads * NB + 1, dtype=torch.int64, device=dev),
                           torch.empty(max(entries, 1), dtype=torch.int32, device=dev))
         lc = lists.c()
-        self._check(self.lib.saf3r_select(self.h, q.data_ptr(), k.data_ptr(), C.byref(shape), arr, workspace.data_ptr(),
-                                          workspace.numel() * workspace.element_size(), C.byref(lc), _stream_ptr(stream)))
+        if cache is not None:
+            cc = cache.c()
+            self._check(self.lib.saf3r_select_cached(self.h, q.data_ptr(), k.data_ptr(), C.byref(shape), arr, C.byref(cc),
+                                                     int(cache_heads), workspace.data_ptr(),
+                                                     workspace.numel() * workspace.element_size(), C.byref(lc), _stream_ptr(stream)))
+        else:
+            self._check(self.lib.saf3r_select(self.h, q.data_ptr(), k.data_ptr(), C.byref(shape), arr, workspace.data_ptr(),
+                                              workspace.numel() * workspace.element_size(), C.byref(lc), _stream_ptr(stream)))
         return lists
 
     # ---- saf3r_sparse_attn / saf3r_dense_attn

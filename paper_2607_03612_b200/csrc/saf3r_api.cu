@@ -84,11 +84,20 @@ static SelGeom make_geom(const saf3r_shape *s) {
   g.stride_head = s->stride_head; g.stride_token = s->stride_token;
   return g;
 }
-static const char *validate_cfg(const SelGeom &g, const saf3r_head_cfg *cfg) {
+static const char *validate_cfg(const SelGeom &g, const saf3r_head_cfg *cfg, int cache_heads = 0) {
   if (!cfg) return "cfg is null";
   for (int h = 0; h < g.H; ++h) {
     const saf3r_head_cfg &c = cfg[h];
     switch (c.type) {
+      case SAF3R_HEAD_CACHED:
+        if (cache_heads <= 0) return "CACHED head outside saf3r_select_cached / saf3r_query_sizes, or without a cache";
+        if (c.offset < 0 || c.offset >= cache_heads) return "CACHED: offset must name a head of the cache";
+        if (c.topk_scope == SAF3R_SCOPE_GLOBAL) {
+          if (c.keep_blocks < 1 || c.keep_blocks > g.NB) return "CACHED/GLOBAL: need 1 <= keep_blocks <= NB";
+        } else if (c.topk_scope == SAF3R_SCOPE_PER_FRAME) {
+          if (c.topk_per_frame < 1) return "CACHED/PER_FRAME: topk_per_frame must be >= 1";
+        } else return "CACHED: bad topk_scope";
+        break;
       case SAF3R_HEAD_DENSE: break;
       case SAF3R_HEAD_UNIFORM_STRIDE:
         if (c.stride < 0) return "UNIFORM_STRIDE: stride must be >= 0";
@@ -223,20 +232,25 @@ saf3r_status saf3r_query_sizes(const saf3r_shape *shape, const saf3r_head_cfg *c
   if (validate_shape(shape, false) || !cfg) return SAF3R_ERR_INVALID_ARG;
   if (unsupported_shape(shape)) return SAF3R_ERR_UNSUPPORTED;
   const SelGeom g = make_geom(shape);
-  if (validate_cfg(g, cfg)) return SAF3R_ERR_INVALID_ARG;
+  if (validate_cfg(g, cfg, SAF3R_MAX_HEADS)) return SAF3R_ERR_INVALID_ARG;  // CACHED heads: lengths are closed forms too
   if (list_entries) *list_entries = total_entries(g, cfg);
   if (workspace_bytes) *workspace_bytes = ws_layout(g).total;
   return SAF3R_OK;
 }
 
-saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const saf3r_shape *shape, const saf3r_head_cfg *cfg,
-                          void *ws, size_t ws_bytes, saf3r_lists *lists, void *stream_) {
+}  // extern "C"
+
+static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, const saf3r_shape *shape, const saf3r_head_cfg *cfg,
+                                const saf3r_lists *cache, int cache_heads, void *ws, size_t ws_bytes, saf3r_lists *lists,
+                                void *stream_) {
   if (!ctx) return SAF3R_ERR_INVALID_ARG;
   if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
   if (const char *m = validate_shape(shape, true)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
   if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
   const SelGeom g = make_geom(shape);
-  if (const char *m = validate_cfg(g, cfg)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (cache && (!cache->row_ptr || !cache->col_idx || cache_heads < 1 || cache_heads > SAF3R_MAX_HEADS))
+    return fail(ctx, SAF3R_ERR_INVALID_ARG, "cache has null arrays or a bad head count");
+  if (const char *m = validate_cfg(g, cfg, cache ? cache_heads : 0)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
   if (!q || !k || !ws || !lists || !lists->row_ptr || !lists->col_idx) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
   if (((uintptr_t)q | (uintptr_t)k) & 15) return fail(ctx, SAF3R_ERR_INVALID_ARG, "q/k must be 16-byte aligned");
   const WsLayout w = ws_layout(g);
@@ -269,7 +283,8 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
     any_block |= cfg[h].type == SAF3R_HEAD_BLOCK_TOPK;
     any_probe |= cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK;
     const bool per_row = cfg[h].type == SAF3R_HEAD_STATIC && cfg[h].static_mode != SAF3R_STATIC_ANCHOR;
-    if (cfg[h].type == SAF3R_HEAD_BLOCK_TOPK) sets.block[sets.n_block++] = (uint8_t)h;
+    if (cfg[h].type == SAF3R_HEAD_CACHED) sets.cached[sets.n_cached++] = (uint8_t)h;
+    else if (cfg[h].type == SAF3R_HEAD_BLOCK_TOPK) sets.block[sets.n_block++] = (uint8_t)h;
     else if (cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK) sets.probe[sets.n_probe++] = (uint8_t)h;
     else if (per_row) sets.light[sets.n_light++] = (uint8_t)h;
     else sets.emit[sets.n_emit++] = (uint8_t)h;
@@ -293,12 +308,13 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
     }
   // launch 1: pooling (one warp per token block of every tensor a rule reads) + one row_ptr CTA per head + the lists of the
   // constant-length closed-form heads
-  const int pool_ctas = jobs.n * ((g.NB + 7) / 8);
+  const int pool_tasks = jobs.n * ((g.NB + 7) / 8);
+  const int pool_ctas = pool_tasks < 4 * ctx->sm_count ? pool_tasks : 4 * ctx->sm_count;  // persistent: 4 CTAs per SM
   const int light_chunks = (g.NB + kLightRows - 1) / kLightRows;
   if (ctx->stage_timing) cudaEventRecord(ctx->ev[0], st);
   pool_rowptr_kernel<<<pool_ctas + g.H + sets.n_emit * light_chunks, 256, 0, st>>>(
       (const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart, lists->row_ptr, lists->col_idx, g, jobs, plan, ca, sets,
-      pool_ctas);
+      pool_ctas, pool_tasks);
   ctx->launches += 1;
   if (ctx->stage_timing) cudaEventRecord(ctx->ev[1], st);
   // launch 2: probe CTAs, score + select CTAs (R rows each: 16, fewer when NB is large - two CTAs per SM if possible - or
@@ -319,9 +335,10 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
     if (row > 200 * 1024) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the probe stage");
     if (sm < row) sm = row;
   }
-  const int sel_ctas = sets.n_probe + sets.n_block * ((g.NB + R - 1) / R) + sets.n_light * light_chunks;
+  const int sel_ctas = sets.n_probe + sets.n_block * ((g.NB + R - 1) / R) + (sets.n_light + sets.n_cached) * light_chunks;
   if (sel_ctas > 0) {
-    select_kernel<<<sel_ctas, 256, sm, st>>>(qt, kt, probe, lists->row_ptr, qpart, probe, lists->col_idx, g, ca, sets, R);
+    select_kernel<<<sel_ctas, 256, sm, st>>>(qt, kt, probe, lists->row_ptr, qpart, probe, lists->col_idx,
+                                             cache ? cache->row_ptr : nullptr, cache ? cache->col_idx : nullptr, g, ca, sets, R);
     ctx->launches += 1;
   }
   if (ctx->stage_timing) {
@@ -339,6 +356,21 @@ saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const sa
   }
   return SAF3R_OK;
 }
+
+extern "C" {
+
+saf3r_status saf3r_select(saf3r_ctx *ctx, const void *q, const void *k, const saf3r_shape *shape, const saf3r_head_cfg *cfg,
+                          void *ws, size_t ws_bytes, saf3r_lists *lists, void *stream) {
+  return select_impl(ctx, q, k, shape, cfg, nullptr, 0, ws, ws_bytes, lists, stream);
+}
+
+saf3r_status saf3r_select_cached(saf3r_ctx *ctx, const void *q, const void *k, const saf3r_shape *shape, const saf3r_head_cfg *cfg,
+                                 const saf3r_lists *cache, int32_t cache_heads, void *ws, size_t ws_bytes, saf3r_lists *lists,
+                                 void *stream) {
+  return select_impl(ctx, q, k, shape, cfg, cache, cache ? cache_heads : 0, ws, ws_bytes, lists, stream);
+}
+
+}  // extern "C"
 
 static saf3r_status get_map(saf3r_ctx *ctx, const void *ptr, const SelGeom &g, CUtensorMap *out) {
   MapKey key{ptr, g.N, g.stride_head, g.stride_token, g.H, g.B};
@@ -415,6 +447,8 @@ static saf3r_status attn_common(saf3r_ctx *ctx, const void *q, const void *k, co
   CU_CHECK(cudaGetLastError());
   return SAF3R_OK;
 }
+
+extern "C" {
 
 saf3r_status saf3r_sparse_attn(saf3r_ctx *ctx, const void *q, const void *k, const void *v, const saf3r_shape *shape,
                                const saf3r_lists *lists, void *out, int out_is_fp32, float *lse, void *stream) {

@@ -90,9 +90,10 @@ __host__ __device__ inline int64_t closed_form_row(const SelGeom &g, const saf3r
 
 // List length of a row (any head type); a closed form of (shape, cfg).
 __host__ __device__ inline int64_t row_length(const SelGeom &g, const saf3r_head_cfg &c, int64_t I) {
-  if (c.type == SAF3R_HEAD_QUERY_PROBE_TOPK || (c.type == SAF3R_HEAD_BLOCK_TOPK && c.topk_scope == SAF3R_SCOPE_GLOBAL))
+  const bool topk = c.type == SAF3R_HEAD_BLOCK_TOPK || c.type == SAF3R_HEAD_CACHED;  // CACHED repeats its source head's rule
+  if (c.type == SAF3R_HEAD_QUERY_PROBE_TOPK || (topk && c.topk_scope == SAF3R_SCOPE_GLOBAL))
     return i64min(c.keep_blocks, g.NB);
-  if (c.type == SAF3R_HEAD_BLOCK_TOPK) {
+  if (topk) {
     int64_t cnt = 0;
     for (int64_t f = 0; f < g.S; ++f) {
       int64_t lo, hi;
@@ -268,7 +269,8 @@ constexpr int kLightRows = 32;  // rows per CTA of the light emitters (8 warps x
 
 // Which heads each launch serves (host-built).
 struct HeadSets {
-  int32_t n_emit, n_light, n_block, n_probe;
+  int32_t n_emit, n_light, n_block, n_probe, n_cached;
+  uint8_t cached[SAF3R_MAX_HEADS];  // launch 2: CACHED heads (rows copied from the index cache)
   uint8_t emit[SAF3R_MAX_HEADS];   // launch 1: closed-form heads whose rows all have the same length (no dependence at all)
   uint8_t light[SAF3R_MAX_HEADS];  // launch 2: per-row-length STATIC heads (need row_ptr)
   uint8_t block[SAF3R_MAX_HEADS];  // launch 2: BLOCK_TOPK heads (score + top-n)
@@ -361,7 +363,7 @@ __device__ inline void probe_head(const float *qpart, const float *kt, int32_t *
 __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
                                                           float *__restrict__ qt, float *__restrict__ kt, float *__restrict__ qpart,
                                                           int64_t *__restrict__ row_ptr, int32_t *__restrict__ col_idx, SelGeom g, PoolJobs jobs, RowPtrPlan plan,
-                                                          HeadCfgArray cfg, HeadSets sets, int pool_ctas) {
+                                                          HeadCfgArray cfg, HeadSets sets, int pool_ctas, int pool_tasks) {
   if ((int)blockIdx.x >= pool_ctas + g.H) {
     // ---------------------------------------------------------------- lists of a constant-length closed-form head
     const int chunks = (g.NB + kLightRows - 1) / kLightRows;
@@ -405,10 +407,13 @@ __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16
   }
   // ------------------------------------------------------------------ pool: one warp per token block
   // CTA c of a job covers blocks 8c .. 8c+7 (jobs are padded to a multiple of 8 blocks, so a CTA never straddles jobs)
+  // The pool CTAs are persistent: pool_ctas <= 4 per SM of them stride over the pool_tasks (job, 8 blocks) tasks, so that
+  // all of them end together instead of leaving a partial last wave.
   __shared__ float qsum[8][64];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ctas_per_job = (g.NB + 7) / 8;
-  const int job = blockIdx.x / ctas_per_job, cta_in_job = blockIdx.x % ctas_per_job;
+  for (int task = blockIdx.x; task < pool_tasks; task += pool_ctas) {
+  const int job = task / ctas_per_job, cta_in_job = task % ctas_per_job;
   const int J = cta_in_job * 8 + warp;
   const int h = jobs.head[job], which = jobs.which[job];
   const bool probe = jobs.probe[job] != 0;
@@ -471,7 +476,7 @@ __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16
       }
     }
   }
-  if (!want_part) return;  // CTA-uniform
+  if (!want_part) continue;  // CTA-uniform
   if (rg == 0) {
 #pragma unroll
     for (int c = 0; c < 8; ++c) qsum[warp][sub * 8 + c] = acc[c];  // zero for warps past the last block
@@ -485,6 +490,8 @@ __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16
       for (int w = 0; w < 8; ++w) t += qsum[w][d];
       qpart[((int64_t)h * ctas_per_job + cta_in_job) * 64 + d] = t;
     }
+  }
+  __syncthreads();  // qsum is reused by this CTA's next task
   }
 }
 
@@ -588,7 +595,9 @@ __device__ __forceinline__ void score_rows(const float *__restrict__ qt, const f
 __global__ void __launch_bounds__(256, 2) select_kernel(const float *__restrict__ qt, const float *__restrict__ kt,
                                                         const int32_t *__restrict__ probe_list, const int64_t *__restrict__ row_ptr,
                                                         const float *__restrict__ qpart, int32_t *__restrict__ probe_out,
-                                                        int32_t *__restrict__ col_idx, SelGeom g, HeadCfgArray cfg, HeadSets sets, int R) {
+                                                        int32_t *__restrict__ col_idx, const int64_t *__restrict__ cache_row_ptr,
+                                                        const int32_t *__restrict__ cache_col_idx, SelGeom g, HeadCfgArray cfg,
+                                                        HeadSets sets, int R) {
   const int warp = threadIdx.x >> 5;
   extern __shared__ float sm[];
   __shared__ float part[4][64];
@@ -604,11 +613,23 @@ __global__ void __launch_bounds__(256, 2) select_kernel(const float *__restrict_
   }
   const int bid = (int)blockIdx.x - probe_ctas;
   if (bid >= heavy_ctas) {
-    // light CTAs come last in launch order, 32 rows each: per-row-length STATIC heads
+    // light CTAs come last in launch order, 32 rows each: per-row-length STATIC heads, then CACHED heads
     const int chunks = (g.NB + kLightRows - 1) / kLightRows;
     const int e = bid - heavy_ctas;
-    const int h = sets.light[e / chunks];
     const int I0 = (e % chunks) * kLightRows;
+    if (e / chunks >= sets.n_light) {
+      const int h = sets.cached[e / chunks - sets.n_light];
+      const int src = cfg.c[h].offset;
+      const int lane = threadIdx.x & 31;
+      for (int r = warp; r < kLightRows && I0 + r < g.NB; r += 8) {
+        const int64_t a = cache_row_ptr[(int64_t)src * g.NB + I0 + r], b = cache_row_ptr[(int64_t)src * g.NB + I0 + r + 1];
+        const int64_t o = row_ptr[(int64_t)h * g.NB + I0 + r], cap = row_ptr[(int64_t)h * g.NB + I0 + r + 1] - o;
+        const int64_t n = i64min(b - a, cap);  // equal when cfg repeats the source rule; never write past the row
+        for (int64_t i = lane; i < n; i += 32) col_idx[o + i] = cache_col_idx[a + i];
+      }
+      return;
+    }
+    const int h = sets.light[e / chunks];
     for (int r = warp; r < kLightRows && I0 + r < g.NB; r += 8)
       emit_light_row(g, cfg.c[h], h, I0 + r, col_idx + row_ptr[(int64_t)h * g.NB + I0 + r], probe_list);
     return;

@@ -21,7 +21,7 @@ from dataclasses import dataclass, field
 import numpy as np
 
 # enum values (restated here as data, see include/saf3r.h for the CUDA side and oracle/saf3r_oracle.c for the oracle)
-HEAD_DENSE, HEAD_UNIFORM_STRIDE, HEAD_STATIC, HEAD_QUERY_PROBE_TOPK, HEAD_BLOCK_TOPK = range(5)
+HEAD_DENSE, HEAD_UNIFORM_STRIDE, HEAD_STATIC, HEAD_QUERY_PROBE_TOPK, HEAD_BLOCK_TOPK, HEAD_CACHED = range(6)
 STATIC_ANCHOR, STATIC_FRAME_LOCAL, STATIC_POSITION_BAND = range(3)
 SCOPE_GLOBAL, SCOPE_PER_FRAME = range(2)
 SCORE_DOT, SCORE_COSINE = range(2)
@@ -252,3 +252,9 @@ def sweep_heads(sh: Shape, gen: str, ratio: float):
     else:
         raise ValueError(gen)
     return [gen] * sh.H, [dict(c) for _ in range(sh.H)]
+
+
+def make_features(sh: Shape, seed: int) -> np.ndarray:
+    """[N][D] bf16 bits: per-sequence patch features standing in for the encoder's last-block output (PAPER.md:L126 uses DINO
+    features; none exist here): the same-position code of every token + N(0, 0.1) noise, shared by all layers."""
+    return make_head(GEN_SAME_POSITION, sh, seed, layer=9999, head=0)[0]

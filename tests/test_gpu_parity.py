@@ -330,3 +330,60 @@ def test_select_is_deterministic_and_reusable(env):
     ctx.set_stage_timing(False)
     assert pool_ms > 0 and sel_ms > 0
     assert torch.equal(a[0], lists.row_ptr) and torch.equal(a[1], lists.col_idx)
+
+
+# ------------------------------------------------------------------------------------------------ index cache + stack (NEXT-1)
+def test_index_cache_and_graph_stack(env):
+    """similarity Top-K lists computed once per sequence from features and reused by the correspondence heads
+    of every layer.  CACHED heads must equal the ORACLE's block top-k on the features (cosine), the other heads of each
+    layer must equal the oracle on that layer's q/k, and the CUDA-graph replay of the stack must equal the eager run."""
+    sf, ctx, torch = env
+    from paper_2607_03612_b200.stack import GlobalStack, cached_cfgs
+    sh = sy.Shape(S=5, G=17, H=4, D=64, B=64)                    # T = 294, N = 1470, NB = 23
+    shape = c_shape(sf, sh)
+    cache_cfgs = [sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=1, score_mode=sy.SCORE_COSINE),
+                  sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=5, score_mode=sy.SCORE_COSINE)]
+    gens = [sy.GEN_SINK, sy.GEN_SAME_POSITION, sy.GEN_FRAME_LOCAL, sy.GEN_SAME_POSITION]
+    base = [sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=5), cache_cfgs[0],
+            sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_FRAME_LOCAL), cache_cfgs[1]]
+    layers = [sy.make_layer(sh, gens, base, seed=30 + l, layer=l) for l in range(3)]
+    layer_cfgs = [cached_cfgs(base, cache_cfgs, {1: 0, 3: 1}) for _ in layers]
+    assert layer_cfgs[0][1]["type"] == sy.HEAD_CACHED
+    feat = sy.make_features(sh, seed=7)
+    fdev = to_dev(np.stack([feat, feat]))
+    st = GlobalStack(ctx, shape, layer_cfgs, cache_cfgs)
+    st.bind([upload(L) for L in layers])
+    st.build_cache(fdev)
+    outs = [o.clone() for o in st.run()]
+    torch.cuda.synchronize()
+    # oracle: cache lists from the features
+    ocache = [orc.select_head(feat, feat, sh.S, sh.T, sh.B, orc.make_cfg(**c), want_scores=True) for c in cache_cfgs]
+    for l, L in enumerate(layers):
+        rp, col = st.lists[l].row_ptr.cpu().numpy(), st.lists[l].col_idx.cpu().numpy()
+        hls = []
+        for h in range(sh.H):
+            if layer_cfgs[l][h]["type"] == sy.HEAD_CACHED:
+                hls.append(ocache[layer_cfgs[l][h]["offset"]])
+            else:
+                hls.append(orc.select_head(L.q[h], L.k[h], sh.S, sh.T, sh.B, orc.make_cfg(**base[h]), want_scores=True))
+        for h, hl in enumerate(hls):
+            r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
+            assert np.array_equal(r - r[0], hl.row_ptr), f"layer {l} head {h}: row_ptr"
+            assert np.array_equal(col[r[0]:r[-1]], hl.col_idx), f"layer {l} head {h}: lists"
+            ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, hl.row_ptr, hl.col_idx)
+            assert np.abs(outs[l][h].float().cpu().numpy() - ref).max() <= 3e-2     # bf16 output
+    # the same stack as one CUDA graph
+    for o in st.out:
+        o.zero_()
+    st.capture()
+    for o in st.out:
+        o.zero_()
+    st.replay()
+    torch.cuda.synchronize()
+    for a, b in zip(outs, st.out):
+        assert torch.equal(a, b)
+    # CACHED heads are rejected without a cache
+    q, k, _ = upload(layers[0])
+    with pytest.raises(sf.Saf3rError) as ei:
+        ctx.select(q, k, shape, layer_cfgs[0])
+    assert ei.value.status == sf.ERR_INVALID_ARG
