@@ -349,6 +349,96 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_stack(args):
+    """the whole global-attention stack (default 24 layers) with the per-sequence index
+    cache and as one CUDA graph.  Prints one JSON line (an extra, not the contract line)."""
+    import torch
+    import paper_2607_03612_b200 as sf
+    from paper_2607_03612_b200.stack import GlobalStack, cached_cfgs
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(0)
+    sh = shape_for(args.config)
+    ctx = sf.Context(0)
+    shape = sf.make_shape(sh.S, sh.T, sh.H, sh.D, sh.B)
+    n_res = min(args.resident_layers, args.layers)
+    res = [sy.config_c3_layer(l, sh=sh) for l in range(n_res)]          # resident Q/K/V sets (each >> L2), cycled
+    up = lambda x: torch.from_numpy(x.view(np.int16)).to(dev).view(torch.bfloat16)
+    qkv_res = [(up(L.q), up(L.k), up(L.v)) for L in res]
+    out_res = [torch.empty_like(q) for q, _, _ in qkv_res]
+    # per-layer rules: the C3 recipe; the stack with a cache turns the same-position heads into CACHED heads
+    cache_cfgs = [sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=1, score_mode=sy.SCORE_COSINE),
+                  sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=max(1, round(0.1 * sh.NB)),
+                         score_mode=sy.SCORE_COSINE)]
+    plain, cached = [], []
+    for l in range(args.layers):
+        gens = res[l % n_res].gens                                       # head types follow the resident data
+        _, cfgs, _ = sy.stack_layer_heads(sh, l % n_res)
+        plain.append(cfgs)
+        cached.append(cached_cfgs(cfgs, cache_cfgs, {h: h % 2 for h, g in enumerate(gens) if g == sy.GEN_SAME_POSITION}))
+    feat = up(np.stack([sy.make_features(sh, seed=77)] * 2))
+    qkv = [qkv_res[l % n_res] for l in range(args.layers)]
+    out = [out_res[l % n_res] for l in range(args.layers)]
+
+    def timed(fn, reps):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    def select_only_graph(st):
+        """The stack's select calls alone, captured as a CUDA graph, so that the GPU time is measured and not the host time of
+        24 back-to-back Python calls (select is far shorter than a host call sequence when no attention kernel hides it)."""
+        n_cache = len(st.cache_cfgs) if st.cache_cfgs else 0
+        side = torch.cuda.Stream()
+
+        def go():
+            for (q, k, v), cfgs, lists in zip(st.qkv, st.layer_cfgs, st.lists):
+                ctx.select(q, k, shape, cfgs, workspace=st.ws, lists=lists, cache=st.cache, cache_heads=n_cache, stream=side)
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            go()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            go()
+        return g
+
+    res_out = {}
+    st0 = GlobalStack(ctx, shape, plain)
+    st0.bind(qkv, out)
+    res_out["eager_no_cache_ms"] = timed(st0.run, args.steps)
+    g0 = select_only_graph(st0)
+    res_out["select_no_cache_ms_per_layer"] = timed(g0.replay, args.steps) / args.layers
+    pairs0 = sum(sf.query_sizes(shape, c)[0] for c in plain)
+    del g0, st0
+    st1 = GlobalStack(ctx, shape, cached, cache_cfgs)
+    st1.bind(qkv, out)
+    res_out["cache_build_ms"] = timed(lambda: st1.build_cache(feat), args.steps)
+    res_out["eager_cached_ms"] = timed(st1.run, args.steps)
+    g1 = select_only_graph(st1)
+    res_out["select_cached_ms_per_layer"] = timed(g1.replay, args.steps) / args.layers
+    st1.capture()
+    res_out["graph_cached_ms"] = timed(st1.replay, args.steps)
+    pairs1 = sum(sf.query_sizes(shape, c)[0] for c in cached)
+    flop = lambda p: 4.0 * sh.B * sh.B * sh.D * p
+    print(json.dumps({
+        "metric": "global_attn_stack_ms", "unit": "ms/stack", "value": res_out["graph_cached_ms"], "n_gpus": 1, "steps": args.steps,
+        "layers": args.layers, "data": "synthetic", "dtype": "bf16",
+        "config": {"workload": f"{args.config.upper()} stack: {args.layers} global layers, S={sh.S}, N={sh.N}, H={sh.H}, block {sh.B}; "
+                               f"{n_res} resident Q/K/V sets cycled; index cache = 2 rules (per-frame top-1, global 10 %) on synthetic features"},
+        **res_out,
+        "kept_pair_ratio_no_cache": pairs0 / (args.layers * sh.H * sh.NB * sh.NB),
+        "kept_pair_ratio_cached": pairs1 / (args.layers * sh.H * sh.NB * sh.NB),
+        "executed_tflops_no_cache_incl_select": flop(pairs0) / (res_out["eager_no_cache_ms"] * 1e-3) / 1e12,
+        "executed_tflops_graph_cached_incl_select": flop(pairs1) / (res_out["graph_cached_ms"] * 1e-3) / 1e12,
+    }))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -364,8 +454,12 @@ def main():
     ap.add_argument("--skip-dense", action="store_true")
     ap.add_argument("--skip-e2e", action="store_true")
     ap.add_argument("--skip-cpu", action="store_true")
+    ap.add_argument("--stack", action="store_true", help="time the whole stack with the index cache and as one CUDA graph")
+    ap.add_argument("--layers", type=int, default=24)
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.stack:
+        run_stack(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
