@@ -387,3 +387,32 @@ def test_index_cache_and_graph_stack(env):
     with pytest.raises(sf.Saf3rError) as ei:
         ctx.select(q, k, shape, layer_cfgs[0])
     assert ei.value.status == sf.ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------------------------------------ offline head profiling (NEXT-3)
+def test_offline_profiling_recovers_planted_head_types(env):
+    """NMSE (Eq. 1) between dense mode and each candidate, greedy substitution under Omega(c) <= Omega(c_base)
+    (Eq. 2).  On synthetic heads with planted structure the search must return the matching kernel for the frame-local,
+    sink and same-position heads, never do worse than the baseline, and its NMSE must agree with the oracle's Eq. 1."""
+    sf, ctx, torch = env
+    from paper_2607_03612_b200 import profiling
+    sh = sy.Shape(S=8, G=16, H=4, D=64, B=64)                    # T = 261, N = 2088, NB = 33
+    gens = [sy.GEN_UNIFORM, sy.GEN_FRAME_LOCAL, sy.GEN_SAME_POSITION, sy.GEN_SINK]
+    L = sy.make_layer(sh, gens, [sy.cfg(type=sy.HEAD_DENSE)] * 4, seed=41)
+    shape = c_shape(sf, sh)
+    q, k, v = upload(L)
+    prof = profiling.profile_heads(ctx, [(q, k, v)], shape, sigma=0.70)   # n_base = 10: the stride set misses the sink blocks
+    for h, p in enumerate(prof):
+        print(gens[h], {kk: vv for kk, vv in p.cfg.items() if vv}, f"E*={p.nmse:.3e} E_base={p.nmse_base:.3e}", p.cost, p.cost_base)
+        assert p.nmse <= p.nmse_base and p.cost <= p.cost_base   # Eq. 2
+    assert prof[1].cfg["type"] == sy.HEAD_STATIC and prof[1].cfg["static_mode"] == sy.STATIC_FRAME_LOCAL
+    assert prof[2].cfg["type"] == sy.HEAD_BLOCK_TOPK
+    assert prof[3].cfg["type"] in (sy.HEAD_QUERY_PROBE_TOPK, sy.HEAD_BLOCK_TOPK)    # sink blocks: probe or block top-k both find them
+    assert prof[1].nmse < 1e-3 and prof[3].nmse < 0.05 and prof[2].nmse < 0.5 * prof[2].nmse_base
+    assert prof[1].cost < prof[1].cost_base                      # structured heads end up sparser than the baseline
+    # Eq. 1 against the oracle for the chosen configuration of head 2
+    h = 2
+    hl = orc.select_head(L.q[h], L.k[h], sh.S, sh.T, sh.B, orc.make_cfg(**prof[h].cfg))
+    o_sp, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, hl.row_ptr, hl.col_idx, want_lse=False)
+    o_full, _ = orc.attn_dense(L.q[h], L.k[h], L.v[h])
+    assert abs(orc.nmse(o_full, o_sp) - prof[h].nmse) <= 1e-3 + 0.05 * prof[h].nmse
