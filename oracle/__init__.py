@@ -54,6 +54,8 @@ def lib():
         L.orc_select_head.restype = i64
         L.orc_attn_lists.argtypes = [vp, vp, vp, i64, i32, i32, vp, vp, vp, i64, vp, vp]
         L.orc_attn_dense.argtypes = [vp, vp, vp, i64, i32, i64, i64, vp, vp]
+        L.orc_attn_tokens.argtypes = [vp, vp, vp, i64, i32, vp, i64, i64, i64, vp, vp]
+        L.orc_token_probe.argtypes = [vp, vp, i64, i32, vp]
         L.orc_nmse.argtypes = [vp, vp, i64]
         L.orc_nmse.restype = dbl
         L.orc_num_threads.restype = i32
@@ -167,6 +169,36 @@ def attn_dense(q_bits, k_bits, v_bits, i0: int = 0, i1: int | None = None):
     lse = np.full((N,), np.nan, np.float32)
     lib().orc_attn_dense(_p(q), _p(k), _p(v), N, D, i0, i1, _p(out), _p(lse))
     return out, lse
+
+
+def attn_tokens(q_bits, k_bits, v_bits, idx, i0: int = 0, i1: int | None = None):
+    """Every query of rows [i0, i1) attends the same key-token set idx (ascending); returns (out [N][D], lse [N]), other rows NaN."""
+    q, k, v = _u16(q_bits), _u16(k_bits), _u16(v_bits)
+    N, D = q.shape
+    i1 = N if i1 is None else i1
+    idx = np.ascontiguousarray(idx, np.int64)
+    out = np.full((N, D), np.nan, np.float32)
+    lse = np.full((N,), np.nan, np.float32)
+    pad = idx if idx.size else np.zeros((1,), np.int64)
+    lib().orc_attn_tokens(_p(q), _p(k), _p(v), N, D, _p(pad), idx.size, i0, i1, _p(out), _p(lse))
+    return out, lse
+
+
+def token_probe(q_bits, k_bits) -> np.ndarray:
+    """p[j] = qbar . k_j / sqrt(D) for every key token."""
+    q, k = _u16(q_bits), _u16(k_bits)
+    N, D = q.shape
+    p = np.empty((N,), np.float32)
+    lib().orc_token_probe(_p(q), _p(k), N, D, _p(p))
+    return p
+
+
+def token_probe_topk(q_bits, k_bits, K: int):
+    """Query-Probe Top-K at token level: the K key tokens with the largest probe score (score desc, index asc), ascending.
+    Returns (idx int64 [K], scores fp32 [N])."""
+    p = token_probe(q_bits, k_bits)
+    keep = topn(p, K, use_sort=True)
+    return keep.astype(np.int64), p
 
 
 def nmse(o_full: np.ndarray, o_sparse: np.ndarray) -> float:

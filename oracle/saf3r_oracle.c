@@ -356,6 +356,58 @@ void orc_attn_dense(const uint16_t *q, const uint16_t *k, const uint16_t *v, int
   }
 }
 
+/* ---- token-granular variants: the paper's own, token-level definitions of two kernels ------------
+ * O4-token: every query attends the SAME explicit key-token set idx[0..n) (ascending, unique).
+ *   Uniform Sampling Kernel: "selects key positions with a fixed stride": idx = {o + i*s}.
+ *   Query-Probe Top-K Kernel: "all queries attend only to these keys".
+ * o_i = sum_{j in idx} softmax_j(q_i.k_j / sqrt(D)) v_j;  n == 0 -> o_i = 0, lse_i = -inf.  Rows [i0, i1). */
+void orc_attn_tokens(const uint16_t *q, const uint16_t *k, const uint16_t *v, int64_t N, int32_t D, const int64_t *idx,
+                     int64_t n, int64_t i0, int64_t i1, float *out, float *lse) {
+  const double inv_sqrt_d = 1.0 / sqrt((double)D);
+  (void)N;
+#pragma omp parallel for schedule(dynamic, 8)
+  for (int64_t i = i0; i < i1; ++i) {
+    if (n == 0) {
+      for (int d = 0; d < D; ++d) out[i * D + d] = 0.f;
+      if (lse) lse[i] = -INFINITY;
+      continue;
+    }
+    double *z = (double *)malloc(sizeof(double) * (size_t)n);
+    double zmax = -INFINITY;
+    for (int64_t t = 0; t < n; ++t) {
+      const int64_t j = idx[t];
+      double dot = 0.0;
+      for (int d = 0; d < D; ++d) dot += (double)bf16_to_f32(q[i * D + d]) * (double)bf16_to_f32(k[j * D + d]);
+      z[t] = dot * inv_sqrt_d;
+      if (z[t] > zmax) zmax = z[t];
+    }
+    double denom = 0.0;
+    for (int64_t t = 0; t < n; ++t) { z[t] = exp(z[t] - zmax); denom += z[t]; }
+    for (int d = 0; d < D; ++d) {
+      double o = 0.0;
+      for (int64_t t = 0; t < n; ++t) o += z[t] * (double)bf16_to_f32(v[idx[t] * D + d]);
+      out[i * D + d] = (float)(o / denom);
+    }
+    if (lse) lse[i] = (float)(zmax + log(denom));
+    free(z);
+  }
+}
+
+/* Token-level query probe: p[j] = qbar . k_j / sqrt(D) for every key token j, qbar = (1/N) sum_i q_i (double
+ * accumulation, stored fp32 like every other score of this oracle). */
+void orc_token_probe(const uint16_t *q, const uint16_t *k, int64_t N, int32_t D, float *p) {
+  float *qbar = (float *)malloc(sizeof(float) * (size_t)D);
+  orc_mean_query(q, N, D, qbar);
+  const double inv_sqrt_d = 1.0 / sqrt((double)D);
+#pragma omp parallel for schedule(static)
+  for (int64_t j = 0; j < N; ++j) {
+    double dot = 0.0;
+    for (int d = 0; d < D; ++d) dot += (double)qbar[d] * (double)bf16_to_f32(k[j * D + d]);
+    p[j] = (float)(dot * inv_sqrt_d);
+  }
+  free(qbar);
+}
+
 /* O5  NMSE, Eq. 1 (one sample): ||O_full - O_sparse||_2^2 / ||O_full||_2^2. */
 double orc_nmse(const float *o_full, const float *o_sparse, int64_t count) {
   double num = 0.0, den = 0.0;

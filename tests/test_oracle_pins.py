@@ -381,3 +381,99 @@ def test_p13_nmse():
     exp = ((a.astype(np.float64) - b) ** 2).sum() / (a.astype(np.float64) ** 2).sum()
     assert abs(orc.nmse(a, b) - exp) <= 1e-12
     assert abs(orc.nmse(a, np.zeros_like(a)) - 1.0) <= 1e-12       # dropping the head entirely ("Skip")
+
+
+# ------------------------------------------------------------------------------------------------ P14-P16: token-granular variants
+def _rand_bits(rng, shape, scale=1.0):
+    return sy.f32_to_bf16_bits((rng.standard_normal(shape) * scale).astype(np.float32))
+
+
+def test_p14_attn_tokens_bruteforce_and_reductions():
+    """O4-token against what fixes it: numpy float64 brute force with an explicit key mask; idx = all tokens == the
+    separately coded dense function; idx = the tokens of a block list == the block-list function; empty set convention;
+    and the library routine torch SDPA with a boolean mask."""
+    rng = np.random.default_rng(14)
+    N, D = 75, 16
+    q, k, v = _rand_bits(rng, (N, D), 1.5), _rand_bits(rng, (N, D), 1.5), _rand_bits(rng, (N, D))
+    qf, kf, vf = (sy.bf16_bits_to_f32(x).astype(np.float64) for x in (q, k, v))
+    idx = np.array(sorted(rng.choice(N, 17, replace=False)), np.int64)
+    out, lse = orc.attn_tokens(q, k, v, idx)
+    z = qf @ kf[idx].T / np.sqrt(D)
+    w = np.exp(z - z.max(1, keepdims=True))
+    ref = (w / w.sum(1, keepdims=True)) @ vf[idx]
+    assert np.abs(out - ref).max() <= 1e-6
+    assert np.abs(lse - (z.max(1) + np.log(w.sum(1)))).max() <= 1e-5
+    # all tokens == dense
+    o_all, l_all = orc.attn_tokens(q, k, v, np.arange(N))
+    o_d, l_d = orc.attn_dense(q, k, v)
+    assert np.abs(o_all - o_d).max() <= 1e-6 and np.abs(l_all - l_d).max() <= 1e-6
+    # tokens of a block list == block-list attention (B = 8, blocks {1, 4, 9 (tail)})
+    B, blocks = 8, [1, 4, 9]
+    tok = np.concatenate([np.arange(b * B, min((b + 1) * B, N)) for b in blocks])
+    NB = (N + B - 1) // B
+    rp = np.arange(NB + 1, dtype=np.int64) * len(blocks)
+    col = np.tile(np.array(blocks, np.int32), NB)
+    o_b, _ = orc.attn_lists(q, k, v, B, rp, col)
+    o_t, _ = orc.attn_tokens(q, k, v, tok)
+    assert np.abs(o_b - o_t).max() <= 1e-6
+    # empty set, and a sub-range of rows
+    o_e, l_e = orc.attn_tokens(q, k, v, np.zeros(0, np.int64))
+    assert np.all(o_e == 0) and np.all(np.isneginf(l_e))
+    o_r, _ = orc.attn_tokens(q, k, v, idx, 10, 20)
+    assert np.isnan(o_r[:10]).all() and np.isnan(o_r[20:]).all() and np.abs(o_r[10:20] - ref[10:20]).max() <= 1e-6
+    # library routine
+    import torch
+    mask = torch.zeros(N, N, dtype=torch.bool)
+    mask[:, torch.from_numpy(idx)] = True
+    sd = torch.nn.functional.scaled_dot_product_attention(torch.from_numpy(qf)[None], torch.from_numpy(kf)[None],
+                                                          torch.from_numpy(vf)[None], attn_mask=mask)[0].numpy()
+    assert np.abs(out - sd).max() <= 1e-6
+
+
+def test_p15_token_stride_closed_form():
+    """Uniform sampling at token level: keys {o + i*s}; count ceil((N-o)/s) = the 1/s of PAPER.md:L241 (s = 32
+    -> 3.1 %, s = 64 -> 1.6 %); s = 1 is dense; attending a strided set == dense attention over the sub-sampled K/V arrays."""
+    rng = np.random.default_rng(15)
+    N, D = 203, 8
+    q, k, v = _rand_bits(rng, (N, D)), _rand_bits(rng, (N, D)), _rand_bits(rng, (N, D))
+    for s, o in ((1, 0), (3, 0), (3, 2), (32, 5), (64, 0)):
+        idx = np.arange(o, N, s)
+        assert len(idx) == -(-(N - o) // s)
+        out, _ = orc.attn_tokens(q, k, v, idx)
+        if s == 1:
+            assert np.abs(out - orc.attn_dense(q, k, v)[0]).max() <= 1e-6
+        # same numbers from the dense function on the sub-sampled keys (queries padded / truncated to the same count)
+        ks, vs = np.ascontiguousarray(k[o::s]), np.ascontiguousarray(v[o::s])
+        m = len(ks)
+        qs = np.ascontiguousarray(np.concatenate([q, q])[:m]) if m <= 2 * N else None
+        d, _ = orc.attn_dense(qs, ks, vs)
+        take = min(m, N)
+        assert np.abs(out[:take] - d[:take]).max() <= 1e-6
+    # the paper's printed ratio (tests/golden/paper_key_fractions.txt, PAPER.md:L259): stride 32 keeps 16x the keys of K = 2 per
+    # frame at T = 1024 tokens per frame, with the token-level count of this function
+    vals = dict(l.split() for l in open(os.path.join(GOLD, "paper_key_fractions.txt")) if l.strip() and not l.startswith("#"))
+    T = 1024
+    assert len(np.arange(0, 8 * T, 32)) / (8 * 2) == float(vals["stride32_vs_k2_sparsity_ratio"])
+
+
+def test_p16_token_probe_is_column_mean_of_scores_and_topk_order():
+    """the probe equals the column-wise average of S = QK^T/sqrt(D) (numpy float64) and induces the same
+    ranking; the top-K set follows the total order (score desc, index asc) - checked against numpy's stable argsort with
+    planted exact ties (duplicated key rows)."""
+    rng = np.random.default_rng(16)
+    N, D, K = 120, 16, 9
+    q, k = _rand_bits(rng, (N, D)), _rand_bits(rng, (N, D))
+    k[40] = k[7]
+    k[41] = k[7]
+    k[99] = k[7]
+    qf, kf = sy.bf16_bits_to_f32(q).astype(np.float64), sy.bf16_bits_to_f32(k).astype(np.float64)
+    col_mean = (qf @ kf.T / np.sqrt(D)).mean(0)
+    idx, p = orc.token_probe_topk(q, k, K)
+    assert np.abs(p - col_mean).max() <= 1e-6
+    assert p[40] == p[7] == p[41] == p[99]
+    order = np.argsort(-p.astype(np.float64), kind="stable")     # score desc, index asc
+    assert np.array_equal(idx, np.sort(order[:K]))
+    # a cut that falls inside the tie group takes the lower indices
+    rank7 = int(np.nonzero(order == 7)[0][0])
+    idx2, _ = orc.token_probe_topk(q, k, rank7 + 2)
+    assert 7 in idx2 and 40 in idx2 and 41 not in idx2 and 99 not in idx2
