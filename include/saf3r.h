@@ -148,6 +148,31 @@ saf3r_status saf3r_layer_host(saf3r_ctx *ctx, const void *q_host, const void *k_
 /* Number of kernels the library has launched on this context since creation (for bench.py's gpu_launches). */
 int64_t saf3r_launch_count(const saf3r_ctx *ctx);
 
+/* ---- Token-granular variants: the paper's own token-level definitions ---------------------------------
+ * All of them run the dense mode of the attention kernel over a key/value token set that differs from the query's.
+ *
+ * saf3r_token_stride_attn: Uniform Sampling Kernel at token level, "selects key positions with a fixed stride"
+ *   (s = 32, 64 in Tab. 6/7, L241): every query attends the key tokens {offset + i*stride < N}.  No gather: K and
+ *   V are read through a strided TMA view.  stride >= 1, 0 <= offset < min(stride, N).  One launch.
+ * saf3r_token_probe_select: Query-Probe Top-K at token level: qbar = (1/N) sum_i q_i,
+ *   p[j] = qbar . k_j / sqrt(D) for every key token j, the K tokens with the largest p (score desc, index asc) written
+ *   ascending to idx_dev[h][0..K) (int32, [H][K]).  1 <= K <= N, the same K for every head of the call.  Four launches.
+ * saf3r_token_set_attn: every query of head h attends the key tokens idx_dev[h][0..K) (ascending, unique, < N; the output of
+ *   saf3r_token_probe_select or any caller-made set): gathers those K/V rows into the workspace and runs the dense mode over
+ *   them.  Two launches.
+ * saf3r_token_query_sizes: workspace bytes of the two calls above (host only). */
+saf3r_status saf3r_token_stride_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const void *v_dev,
+                                     const saf3r_shape *shape, int32_t stride, int32_t offset, void *out_dev, int out_is_fp32,
+                                     float *lse_dev_or_null, void *cuda_stream);
+saf3r_status saf3r_token_query_sizes(const saf3r_shape *shape, int32_t K, size_t *select_workspace_bytes,
+                                     size_t *attn_workspace_bytes);
+saf3r_status saf3r_token_probe_select(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const saf3r_shape *shape, int32_t K,
+                                      void *workspace_dev, size_t workspace_bytes, int32_t *idx_dev, void *cuda_stream);
+saf3r_status saf3r_token_set_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const void *v_dev,
+                                  const saf3r_shape *shape, const int32_t *idx_dev, int32_t K, void *workspace_dev,
+                                  size_t workspace_bytes, void *out_dev, int out_is_fp32, float *lse_dev_or_null,
+                                  void *cuda_stream);
+
 /* Measurement aid ("select ms split into pool and score+select stages").  When enabled, saf3r_select records
  * CUDA events on its stream before the pool launch, between the two launches and after the select launch (three
  * cudaEventRecord calls, no synchronisation).  saf3r_last_select_stage_ms blocks until the last timed saf3r_select has

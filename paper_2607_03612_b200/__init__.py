@@ -26,7 +26,8 @@ SCORE_DOT, SCORE_COSINE = range(2)
 
 EXPORTS = ("saf3r_create", "saf3r_destroy", "saf3r_last_error", "saf3r_query_sizes", "saf3r_select", "saf3r_sparse_attn",
            "saf3r_dense_attn", "saf3r_layer_host_scratch_bytes", "saf3r_layer_host", "saf3r_launch_count",
-           "saf3r_set_stage_timing", "saf3r_last_select_stage_ms", "saf3r_select_cached")
+           "saf3r_set_stage_timing", "saf3r_last_select_stage_ms", "saf3r_select_cached", "saf3r_token_stride_attn",
+           "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn")
 
 
 class Saf3rError(RuntimeError):
@@ -71,6 +72,10 @@ def load_library():
         L.saf3r_select.argtypes = [vp, vp, vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), vp, C.c_size_t, C.POINTER(ListsC), vp]
         L.saf3r_select_cached.argtypes = [vp, vp, vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(ListsC), C.c_int32, vp,
                                           C.c_size_t, C.POINTER(ListsC), vp]
+        L.saf3r_token_stride_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.c_int32, C.c_int32, vp, i32, vp, vp]
+        L.saf3r_token_query_sizes.argtypes = [C.POINTER(ShapeC), C.c_int32, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
+        L.saf3r_token_probe_select.argtypes = [vp, vp, vp, C.POINTER(ShapeC), C.c_int32, vp, C.c_size_t, vp, vp]
+        L.saf3r_token_set_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), vp, C.c_int32, vp, C.c_size_t, vp, i32, vp, vp]
         L.saf3r_sparse_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(ListsC), vp, i32, vp, vp]
         L.saf3r_dense_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), vp, i32, vp, vp]
         L.saf3r_layer_host_scratch_bytes.argtypes = [C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(C.c_size_t)]
@@ -213,6 +218,47 @@ class Context:
         self._check(st)
         return (out, lse) if want_lse else out
 
+    # ---- token-granular variants: saf3r_token_stride_attn / saf3r_token_probe_select / saf3r_token_set_attn
+    def _out_lse(self, q, shape, out, out_fp32, want_lse):
+        import torch
+        if out is None:
+            out = torch.empty(q.shape, dtype=torch.float32 if out_fp32 else torch.bfloat16, device=q.device)
+        N = shape.num_frames * shape.tokens_per_frame
+        lse = torch.empty((shape.num_heads, N), dtype=torch.float32, device=q.device) if want_lse else None
+        return out, lse
+
+    def token_stride_attn(self, q, k, v, shape: ShapeC, stride: int, offset: int = 0, out=None, out_fp32=False, want_lse=False,
+                          stream=None):
+        out, lse = self._out_lse(q, shape, out, out_fp32, want_lse)
+        self._check(self.lib.saf3r_token_stride_attn(self.h, q.data_ptr(), k.data_ptr(), v.data_ptr(), C.byref(shape), int(stride),
+                                                     int(offset), out.data_ptr(), int(out_fp32),
+                                                     lse.data_ptr() if lse is not None else None, _stream_ptr(stream)))
+        return (out, lse) if want_lse else out
+
+    def token_probe_select(self, q, k, shape: ShapeC, K: int, workspace=None, idx=None, stream=None):
+        """Returns idx int32 [H][K] (device): the K key tokens with the largest probe score per head, ascending."""
+        import torch
+        sel_ws, _ = token_query_sizes(shape, K)
+        if workspace is None:
+            workspace = torch.empty(sel_ws, dtype=torch.uint8, device=q.device)
+        if idx is None:
+            idx = torch.empty((shape.num_heads, K), dtype=torch.int32, device=q.device)
+        self._check(self.lib.saf3r_token_probe_select(self.h, q.data_ptr(), k.data_ptr(), C.byref(shape), int(K), workspace.data_ptr(),
+                                                      workspace.numel(), idx.data_ptr(), _stream_ptr(stream)))
+        return idx
+
+    def token_set_attn(self, q, k, v, shape: ShapeC, idx, workspace=None, out=None, out_fp32=False, want_lse=False, stream=None):
+        import torch
+        K = int(idx.shape[1])
+        _, att_ws = token_query_sizes(shape, K)
+        if workspace is None:
+            workspace = torch.empty(att_ws, dtype=torch.uint8, device=q.device)
+        out, lse = self._out_lse(q, shape, out, out_fp32, want_lse)
+        self._check(self.lib.saf3r_token_set_attn(self.h, q.data_ptr(), k.data_ptr(), v.data_ptr(), C.byref(shape), idx.data_ptr(), K,
+                                                  workspace.data_ptr(), workspace.numel(), out.data_ptr(), int(out_fp32),
+                                                  lse.data_ptr() if lse is not None else None, _stream_ptr(stream)))
+        return (out, lse) if want_lse else out
+
     # ---- saf3r_layer_host
     def layer_host_scratch_bytes(self, shape: ShapeC, cfgs) -> int:
         arr = make_cfgs(cfgs)
@@ -228,6 +274,16 @@ class Context:
                                               arr, scratch.data_ptr(), scratch.numel() * scratch.element_size(),
                                               out_host.data_ptr(), _stream_ptr(stream)))
         return out_host
+
+
+def token_query_sizes(shape: ShapeC, K: int) -> tuple[int, int]:
+    """Host-only: (select workspace bytes, attention workspace bytes) of the token-granular calls."""
+    L = load_library()
+    a, b = C.c_size_t(), C.c_size_t()
+    st = L.saf3r_token_query_sizes(C.byref(shape), int(K), C.byref(a), C.byref(b))
+    if st != OK:
+        raise Saf3rError(st, "saf3r_token_query_sizes rejected (shape, K)")
+    return int(a.value), int(b.value)
 
 
 def query_sizes(shape: ShapeC, cfgs) -> tuple[int, int]:

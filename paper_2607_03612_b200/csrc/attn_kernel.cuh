@@ -31,7 +31,8 @@ struct AttnParams {
   void *out;
   float *lse;  // [H][N] or nullptr
   int64_t out_stride_head, out_stride_token;
-  int32_t N, NB, H;
+  int32_t N, NB, H;      // query tokens / q-blocks / heads
+  int32_t N_kv, NB_kv;  // key/value tokens / k-blocks (== N, NB except in the token-granular variants)
   int32_t out_fp32;
   float scale_log2;  // (1/sqrt(D)) * log2(e)
   uint8_t head_order[SAF3R_MAX_HEADS];  // blockIdx.y -> head, longest lists first
@@ -75,14 +76,14 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
   const uint32_t tS = tmem + lane_off + C0, tO = tmem + lane_off + kTmemO + 32 * kHalf, tP = tmem + lane_off + kTmemP + C0 / 2;
   float *smax = reinterpret_cast<float *>(smem + L::kMax);
   float *ssum = reinterpret_cast<float *>(smem + L::kSum);
-  const int tail = p.N - (p.NB - 1) * B;  // valid keys in the last k-block
+  const int tail = p.N_kv - (p.NB_kv - 1) * B;  // valid keys in the last k-block
   const int64_t tok = (int64_t)I * B + r;
   const bool row_valid = (r < B) && (tok < p.N);
   const float c = p.scale_log2;
   const float lazy_raw = kLazyLog2 / c;
   float m = -INFINITY, l = 0.f;
-  const int J_last = (n_ent > 0) ? (p.row_ptr ? p.col_idx[e0 + n_ent - 1] : p.NB - 1) : -1;
-  const bool last_is_tail = (J_last == p.NB - 1) && (tail < B);
+  const int J_last = (n_ent > 0) ? (p.row_ptr ? p.col_idx[e0 + n_ent - 1] : p.NB_kv - 1) : -1;
+  const bool last_is_tail = (J_last == p.NB_kv - 1) && (tail < B);
 
   for (int e = 0; e < n_ent; ++e) {
     uint32_t v[NC];
@@ -229,7 +230,7 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::kBar + 120);
 
   int64_t e0 = 0;
-  int n_ent = p.NB;
+  int n_ent = p.NB_kv;
   if (p.row_ptr != nullptr) {
     const int64_t r = (int64_t)h * p.NB + I;
     e0 = p.row_ptr[r];

@@ -12,6 +12,7 @@
 #include "saf3r.h"
 #include "attn_kernel.cuh"
 #include "select_kernels.cuh"
+#include "token_kernels.cuh"
 
 using namespace saf3r;
 
@@ -398,8 +399,13 @@ static saf3r_status get_map(saf3r_ctx *ctx, const void *ptr, const SelGeom &g, C
   return SAF3R_OK;
 }
 
+struct KvGeom {  // key/value token set that differs from the query's (token-granular variants); n == 0: same as q
+  int64_t n, stride_head, stride_token;
+};
+
 static saf3r_status attn_common(saf3r_ctx *ctx, const void *q, const void *k, const void *v, const saf3r_shape *shape,
-                                const saf3r_lists *lists, void *out, int out_is_fp32, float *lse, void *stream_) {
+                                const saf3r_lists *lists, void *out, int out_is_fp32, float *lse, void *stream_,
+                                const KvGeom *kv = nullptr) {
   if (!ctx) return SAF3R_ERR_INVALID_ARG;
   if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
   if (const char *m = validate_shape(shape, true)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
@@ -408,11 +414,21 @@ static saf3r_status attn_common(saf3r_ctx *ctx, const void *q, const void *k, co
   if (((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) return fail(ctx, SAF3R_ERR_INVALID_ARG, "q/k/v/out must be 16-byte aligned");
   if (lists && (!lists->row_ptr || !lists->col_idx)) return fail(ctx, SAF3R_ERR_INVALID_ARG, "lists has null arrays");
   const SelGeom g = make_geom(shape);
+  SelGeom gk = g;
+  if (kv) {
+    if (kv->n < 1 || kv->n > 0x7FFFFFFFll - 256) return fail(ctx, SAF3R_ERR_INVALID_ARG, "n_kv out of range");
+    if (kv->stride_token < shape->head_dim || kv->stride_token % 8 || kv->stride_head % 8)
+      return fail(ctx, SAF3R_ERR_INVALID_ARG, "kv strides must be multiples of 8 elements and kv_stride_token >= head_dim");
+    gk.N = kv->n;
+    gk.NB = (int32_t)((kv->n + g.B - 1) / g.B);
+    gk.stride_head = kv->stride_head;
+    gk.stride_token = kv->stride_token;
+  }
   CUtensorMap mq, mk, mv;
   saf3r_status s;
   if ((s = get_map(ctx, q, g, &mq)) != SAF3R_OK) return s;
-  if ((s = get_map(ctx, k, g, &mk)) != SAF3R_OK) return s;
-  if ((s = get_map(ctx, v, g, &mv)) != SAF3R_OK) return s;
+  if ((s = get_map(ctx, k, gk, &mk)) != SAF3R_OK) return s;
+  if ((s = get_map(ctx, v, gk, &mv)) != SAF3R_OK) return s;
   AttnParams p;
   p.row_ptr = lists ? lists->row_ptr : nullptr;
   p.col_idx = lists ? lists->col_idx : nullptr;
@@ -421,6 +437,7 @@ static saf3r_status attn_common(saf3r_ctx *ctx, const void *q, const void *k, co
   p.out_stride_head = shape->stride_head;
   p.out_stride_token = shape->stride_token;
   p.N = (int32_t)g.N; p.NB = g.NB; p.H = g.H;
+  p.N_kv = (int32_t)gk.N; p.NB_kv = gk.NB;
   p.out_fp32 = out_is_fp32 ? 1 : 0;
   p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)shape->head_dim));
   // heads with the longest lists first (list lengths are per-head nearly uniform; dense mode: identity)
@@ -459,6 +476,96 @@ saf3r_status saf3r_sparse_attn(saf3r_ctx *ctx, const void *q, const void *k, con
 saf3r_status saf3r_dense_attn(saf3r_ctx *ctx, const void *q, const void *k, const void *v, const saf3r_shape *shape, void *out,
                               int out_is_fp32, float *lse, void *stream) {
   return attn_common(ctx, q, k, v, shape, nullptr, out, out_is_fp32, lse, stream);
+}
+
+// ------------------------------------------------------------------------------------------------ token-granular variants
+saf3r_status saf3r_token_stride_attn(saf3r_ctx *ctx, const void *q, const void *k, const void *v, const saf3r_shape *shape,
+                                     int32_t stride, int32_t offset, void *out, int out_is_fp32, float *lse, void *stream) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (const char *m = validate_shape(shape, true)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  const int64_t N = (int64_t)shape->num_frames * shape->tokens_per_frame;
+  if (stride < 1 || offset < 0 || offset >= stride || offset >= N)
+    return fail(ctx, SAF3R_ERR_INVALID_ARG, "token stride: need stride >= 1 and 0 <= offset < min(stride, N)");
+  if (!k || !v) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  const KvGeom kv{(N - offset + stride - 1) / stride, shape->stride_head, shape->stride_token * (int64_t)stride};
+  const __nv_bfloat16 *k0 = (const __nv_bfloat16 *)k + (int64_t)offset * shape->stride_token;
+  const __nv_bfloat16 *v0 = (const __nv_bfloat16 *)v + (int64_t)offset * shape->stride_token;
+  return attn_common(ctx, q, k0, v0, shape, nullptr, out, out_is_fp32, lse, stream, &kv);
+}
+
+struct TokWs {
+  size_t part, keys, select_total, kc, vc, attn_total;
+  int n_chunks;
+};
+static TokWs tok_ws(const SelGeom &g, int K) {
+  TokWs w;
+  w.n_chunks = (int)((g.N + kTokChunk - 1) / kTokChunk);
+  size_t off = 0;
+  w.part = off; off = align256(off + (size_t)g.H * w.n_chunks * 64 * sizeof(float));
+  w.keys = off; off = align256(off + (size_t)g.H * g.N * sizeof(uint32_t));
+  w.select_total = off;
+  off = 0;
+  w.kc = off; off = align256(off + (size_t)g.H * K * 64 * 2);
+  w.vc = off; off = align256(off + (size_t)g.H * K * 64 * 2);
+  w.attn_total = off;
+  return w;
+}
+
+saf3r_status saf3r_token_query_sizes(const saf3r_shape *shape, int32_t K, size_t *select_ws, size_t *attn_ws) {
+  if (validate_shape(shape, false)) return SAF3R_ERR_INVALID_ARG;
+  if (unsupported_shape(shape)) return SAF3R_ERR_UNSUPPORTED;
+  const SelGeom g = make_geom(shape);
+  if (K < 1 || K > g.N) return SAF3R_ERR_INVALID_ARG;
+  const TokWs w = tok_ws(g, K);
+  if (select_ws) *select_ws = w.select_total;
+  if (attn_ws) *attn_ws = w.attn_total;
+  return SAF3R_OK;
+}
+
+saf3r_status saf3r_token_probe_select(saf3r_ctx *ctx, const void *q, const void *k, const saf3r_shape *shape, int32_t K, void *ws,
+                                      size_t ws_bytes, int32_t *idx, void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_shape(shape, true)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  const SelGeom g = make_geom(shape);
+  if (K < 1 || K > g.N) return fail(ctx, SAF3R_ERR_INVALID_ARG, "token probe: need 1 <= K <= N");
+  if (!q || !k || !ws || !idx) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  if (((uintptr_t)q | (uintptr_t)k) & 15) return fail(ctx, SAF3R_ERR_INVALID_ARG, "q/k must be 16-byte aligned");
+  const TokWs w = tok_ws(g, K);
+  if (ws_bytes < w.select_total) return fail(ctx, SAF3R_ERR_CAPACITY, "workspace too small (saf3r_token_query_sizes)");
+  cudaStream_t st = (cudaStream_t)stream_;
+  float *part = (float *)((uint8_t *)ws + w.part);
+  uint32_t *keys = (uint32_t *)((uint8_t *)ws + w.keys);
+  token_qsum_kernel<<<dim3(w.n_chunks, g.H), 256, 0, st>>>((const __nv_bfloat16 *)q, part, g);
+  token_probe_kernel<<<dim3((unsigned)((g.N + kTokTile - 1) / kTokTile), g.H), 256, 0, st>>>((const __nv_bfloat16 *)k, part, keys, g,
+                                                                                           w.n_chunks);
+  token_topk_kernel<<<g.H, 1024, 0, st>>>(keys, idx, g.N, K);
+  ctx->launches += 3;
+  CU_CHECK(cudaGetLastError());
+  return SAF3R_OK;
+}
+
+saf3r_status saf3r_token_set_attn(saf3r_ctx *ctx, const void *q, const void *k, const void *v, const saf3r_shape *shape,
+                                  const int32_t *idx, int32_t K, void *ws, size_t ws_bytes, void *out, int out_is_fp32, float *lse,
+                                  void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_shape(shape, true)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  const SelGeom g = make_geom(shape);
+  if (K < 1 || K > g.N) return fail(ctx, SAF3R_ERR_INVALID_ARG, "token set: need 1 <= K <= N");
+  if (!q || !k || !v || !ws || !idx || !out) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  if (((uintptr_t)k | (uintptr_t)v | (uintptr_t)ws) & 15) return fail(ctx, SAF3R_ERR_INVALID_ARG, "k/v/workspace must be 16-byte aligned");
+  const TokWs w = tok_ws(g, K);
+  if (ws_bytes < w.attn_total) return fail(ctx, SAF3R_ERR_CAPACITY, "workspace too small (saf3r_token_query_sizes)");
+  cudaStream_t st = (cudaStream_t)stream_;
+  __nv_bfloat16 *kc = (__nv_bfloat16 *)((uint8_t *)ws + w.kc), *vc = (__nv_bfloat16 *)((uint8_t *)ws + w.vc);
+  token_gather_kernel<<<dim3((K + 31) / 32, g.H, 2), 256, 0, st>>>((const __nv_bfloat16 *)k, (const __nv_bfloat16 *)v, idx, kc, vc, g, K);
+  ctx->launches += 1;
+  CU_CHECK(cudaGetLastError());
+  const KvGeom kv{K, (int64_t)K * 64, 64};
+  return attn_common(ctx, q, kc, vc, shape, nullptr, out, out_is_fp32, lse, stream_, &kv);
 }
 
 struct HostLayout {

@@ -1,0 +1,198 @@
+// Token-granular variants: the paper's own token-level definitions of two of its kernels.
+//   Uniform Sampling Kernel: every s-th key token -> no kernel of its own: a strided TMA view of K/V fed to the
+//       dense mode of saf3r_attn_kernel (saf3r_token_stride_attn in saf3r_api.cu).
+//   Query-Probe Top-K Kernel: qbar = (1/N) sum_i q_i, p[j] = qbar . k_j / sqrt(D) for every key TOKEN,
+//       top-K tokens shared by all queries:
+//         token_qsum_kernel    per-chunk token sums of Q (HBM stream)
+//         token_probe_kernel   qbar from the chunk sums (fixed order), p[j] as order-preserving keys (HBM stream of K)
+//         token_topk_kernel    one CTA per head: 4x8-bit radix select of the K-th largest key over N keys (per-warp private
+//                              histograms), then an ordered block compaction -> ascending token indices, ties by lower index
+//         token_gather_kernel  K/V rows of the selected tokens -> compact [H][K][64] tiles for the dense mode of the attention
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "select_kernels.cuh"
+
+namespace saf3r {
+
+constexpr int kTokChunk = 2048;  // tokens per CTA of the Q-sum pass
+constexpr int kTokTile = 1024;   // tokens per CTA of the probe pass
+
+__device__ __forceinline__ void bf16x8_to_f32(const uint4 &raw, float (&v)[8]) {
+  const uint32_t w[4] = {raw.x, raw.y, raw.z, raw.w};
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    v[2 * c] = __uint_as_float(w[c] << 16);
+    v[2 * c + 1] = __uint_as_float(w[c] & 0xFFFF0000u);
+  }
+}
+
+// grid (ceil(N / kTokChunk), H), 256 threads: lane group of 8 threads = one token row (16 B each), 32 rows per step.
+__global__ void __launch_bounds__(256) token_qsum_kernel(const __nv_bfloat16 *__restrict__ q, float *__restrict__ part, SelGeom g) {
+  const int h = blockIdx.y, chunk = blockIdx.x;
+  const int sub = threadIdx.x & 7, row = threadIdx.x >> 3;
+  const int64_t t0 = (int64_t)chunk * kTokChunk;
+  const int cnt = (int)i64min(kTokChunk, g.N - t0);
+  const __nv_bfloat16 *src = q + (int64_t)h * g.stride_head + t0 * g.stride_token + sub * 8;
+  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  for (int r0 = 0; r0 < kTokChunk; r0 += 32 * 8) {
+    uint4 raw[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int r = r0 + row + 32 * i;
+      raw[i] = make_uint4(0, 0, 0, 0);
+      if (r < cnt) raw[i] = ld_stream_16(src + (int64_t)r * g.stride_token);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      float v[8];
+      bf16x8_to_f32(raw[i], v);
+#pragma unroll
+      for (int c = 0; c < 8; ++c) acc[c] += v[c];
+    }
+  }
+  __shared__ float red[32][64];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) red[row][sub * 8 + c] = acc[c];
+  __syncthreads();
+  if (threadIdx.x < 64) {
+    float t = 0.f;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) t += red[r][threadIdx.x];
+    part[((int64_t)h * gridDim.x + chunk) * 64 + threadIdx.x] = t;
+  }
+}
+
+// grid (ceil(N / kTokTile), H), 256 threads.  keys[h][j] = order-preserving key of p[j] = qbar . k_j / sqrt(D).
+__global__ void __launch_bounds__(256) token_probe_kernel(const __nv_bfloat16 *__restrict__ k, const float *__restrict__ part,
+                                                          uint32_t *__restrict__ keys, SelGeom g, int n_chunks) {
+  const int h = blockIdx.y;
+  __shared__ float qb[64];
+  if (threadIdx.x < 64) {
+    float t = 0.f;
+    for (int c = 0; c < n_chunks; ++c) t += part[((int64_t)h * n_chunks + c) * 64 + threadIdx.x];  // fixed order
+    qb[threadIdx.x] = t / (float)g.N;
+  }
+  __syncthreads();
+  const int sub = threadIdx.x & 7, row = threadIdx.x >> 3;
+  float qv[8];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) qv[c] = qb[sub * 8 + c];
+  const int64_t t0 = (int64_t)blockIdx.x * kTokTile;
+  const int cnt = (int)i64min(kTokTile, g.N - t0);
+  const __nv_bfloat16 *src = k + (int64_t)h * g.stride_head + t0 * g.stride_token + sub * 8;
+  for (int r0 = 0; r0 < kTokTile; r0 += 32 * 8) {
+    uint4 raw[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int r = r0 + row + 32 * i;
+      raw[i] = make_uint4(0, 0, 0, 0);
+      if (r < cnt) raw[i] = ld_stream_16(src + (int64_t)r * g.stride_token);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      float v[8];
+      bf16x8_to_f32(raw[i], v);
+      float d = 0.f;
+#pragma unroll
+      for (int c = 0; c < 8; ++c) d = fmaf(qv[c], v[c], d);
+      d += __shfl_xor_sync(0xffffffffu, d, 1);
+      d += __shfl_xor_sync(0xffffffffu, d, 2);
+      d += __shfl_xor_sync(0xffffffffu, d, 4);
+      const int r = r0 + row + 32 * i;
+      if (sub == 0 && r < cnt) keys[(int64_t)h * g.N + t0 + r] = score_key(d * 0.125f);
+    }
+  }
+}
+
+// grid (H), 1024 threads.  idx[h][0..K): the K tokens with the largest keys, ascending; ties at the cut by lower index.
+__global__ void __launch_bounds__(1024) token_topk_kernel(const uint32_t *__restrict__ keys, int32_t *__restrict__ idx, int64_t N, int K) {
+  const int h = blockIdx.x;
+  const uint32_t *key = keys + (int64_t)h * N;
+  int32_t *out = idx + (int64_t)h * K;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  __shared__ uint32_t hist[32][256];  // one private histogram per warp
+  __shared__ uint32_t tot[256];
+  __shared__ uint32_t s_prefix, s_need;
+  __shared__ int wtake[32], weq[32];
+  uint32_t prefix = 0, mask = 0;
+  int need = K;
+  for (int shift = 24; shift >= 0; shift -= 8) {
+    for (int i = threadIdx.x; i < 32 * 256; i += 1024) (&hist[0][0])[i] = 0;
+    __syncthreads();
+    for (int64_t j = threadIdx.x; j < N; j += 1024) {
+      const uint32_t kv = key[j];
+      if ((kv & mask) == prefix) atomicAdd(&hist[warp][(kv >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    if (threadIdx.x < 256) {
+      uint32_t t = 0;
+#pragma unroll
+      for (int w = 0; w < 32; ++w) t += hist[w][threadIdx.x];
+      tot[threadIdx.x] = t;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {  // 256 bins from the top: find the bin in which the running count reaches `need`
+      uint32_t run = 0;
+      int b = 255;
+      for (; b > 0; --b) {
+        if (run + tot[b] >= (uint32_t)need) break;
+        run += tot[b];
+      }
+      s_prefix = prefix | ((uint32_t)b << shift);
+      s_need = (uint32_t)need - run;
+    }
+    __syncthreads();
+    prefix = s_prefix;
+    need = (int)s_need;
+    mask |= 255u << shift;
+    __syncthreads();
+  }
+  const uint32_t tau = prefix;  // K-th largest key; take all keys above it and the first `need` (by index) equal to it
+  int written = 0, eq_seen = 0;
+  const uint32_t lt = (1u << lane) - 1u;
+  for (int64_t j0 = 0; j0 < N; j0 += 1024) {
+    const int64_t j = j0 + threadIdx.x;
+    const uint32_t kv = j < N ? key[j] : 0u;
+    const bool gt = j < N && kv > tau, eq = j < N && kv == tau;
+    const uint32_t eqb = __ballot_sync(0xffffffffu, eq);
+    if (lane == 0) weq[warp] = __popc(eqb);
+    __syncthreads();
+    int eq_before = eq_seen, eq_total = 0;
+    for (int w = 0; w < 32; ++w) {
+      if (w < warp) eq_before += weq[w];
+      eq_total += weq[w];
+    }
+    const bool take = gt || (eq && eq_before + __popc(eqb & lt) < need);
+    const uint32_t tb = __ballot_sync(0xffffffffu, take);
+    if (lane == 0) wtake[warp] = __popc(tb);
+    __syncthreads();
+    int before = written, total = 0;
+    for (int w = 0; w < 32; ++w) {
+      if (w < warp) before += wtake[w];
+      total += wtake[w];
+    }
+    if (take) out[before + __popc(tb & lt)] = (int32_t)j;
+    written += total;
+    eq_seen += eq_total;
+    __syncthreads();
+  }
+}
+
+// grid (ceil(K / 32), H, 2): rows idx[h][i] of K (z = 0) / V (z = 1) -> compact [H][K][64] bf16.
+__global__ void __launch_bounds__(256) token_gather_kernel(const __nv_bfloat16 *__restrict__ k, const __nv_bfloat16 *__restrict__ v,
+                                                           const int32_t *__restrict__ idx, __nv_bfloat16 *__restrict__ kc,
+                                                           __nv_bfloat16 *__restrict__ vc, SelGeom g, int K) {
+  const int h = blockIdx.y;
+  const int sub = threadIdx.x & 7, row = threadIdx.x >> 3;
+  const int i = blockIdx.x * 32 + row;
+  if (i >= K) return;
+  const int64_t t = idx[(int64_t)h * K + i];
+  const __nv_bfloat16 *src = (blockIdx.z ? v : k) + (int64_t)h * g.stride_head + t * g.stride_token + sub * 8;
+  __nv_bfloat16 *dst = (blockIdx.z ? vc : kc) + ((int64_t)h * K + i) * 64 + sub * 8;
+  *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
+}
+
+}  // namespace saf3r
