@@ -439,6 +439,62 @@ def run_stack(args):
     }))
 
 
+def run_token(args):
+    """the paper's token-level uniform stride and query-probe top-K kernels on one layer; one JSON line each
+    (an extra, not the contract line)."""
+    import torch
+    import paper_2607_03612_b200 as sf
+    dev = torch.device("cuda:0")
+    sh = shape_for(args.config)
+    ctx = sf.Context(0)
+    shape = sf.make_shape(sh.S, sh.T, sh.H, sh.D, sh.B)
+    L = sy.config_c3_layer(0, sh=sh)
+    up = lambda x: torch.from_numpy(x.view(np.int16)).to(dev).view(torch.bfloat16)
+    q, k, v = up(L.q), up(L.k), up(L.v)
+    out = torch.empty_like(q)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def timed(fn, reps):
+        fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            flush.zero_()                                           # L2 flush between timed iterations
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return float(np.mean(ts))
+
+    peaks = load_peaks()
+    dense_ms = timed(lambda: ctx.dense_attn(q, k, v, shape, out=out), 2)
+    lines = []
+    for s in args.strides:
+        n_kv = -(-sh.N // s)
+        ms = timed(lambda: ctx.token_stride_attn(q, k, v, shape, s, 0, out=out), args.steps)
+        tf = 4.0 * sh.N * (-(-n_kv // sh.B) * sh.B) * sh.D * sh.H / (ms * 1e-3) / 1e12
+        lines.append({"variant": f"token stride s={s}", "kept_keys": n_kv / sh.N, "ms": ms, "executed_tflops": tf,
+                      "frac_of_sustained_peak": tf / peaks["tflops_sustained"], "speedup_vs_own_dense": dense_ms / ms})
+    for K in args.topks:
+        sel_ws, att_ws = sf.token_query_sizes(shape, K)
+        ws1 = torch.empty(sel_ws, dtype=torch.uint8, device=dev)
+        ws2 = torch.empty(att_ws, dtype=torch.uint8, device=dev)
+        idx = torch.empty((sh.H, K), dtype=torch.int32, device=dev)
+        sel = timed(lambda: ctx.token_probe_select(q, k, shape, K, workspace=ws1, idx=idx), args.steps)
+        att = timed(lambda: ctx.token_set_attn(q, k, v, shape, idx, workspace=ws2, out=out), args.steps)
+        tf = 4.0 * sh.N * (-(-K // sh.B) * sh.B) * sh.D * sh.H / (att * 1e-3) / 1e12
+        sel_gbs = 2.0 * sh.H * sh.N * sh.D * 2 / (sel * 1e-3) / 1e9  # Q once (qbar) + K once (probe)
+        lines.append({"variant": f"token query-probe top-K K={K}", "kept_keys": K / sh.N, "select_ms": sel, "attn_ms": att,
+                      "ms": sel + att, "executed_tflops": tf, "frac_of_sustained_peak": tf / peaks["tflops_sustained"],
+                      "select_gbs": sel_gbs, "select_frac_of_hbm_peak": sel_gbs / peaks["hbm_gbs"],
+                      "speedup_vs_own_dense": dense_ms / (sel + att)})
+    print(json.dumps({"metric": "token_variant_layer_ms", "unit": "ms/layer", "data": "synthetic", "dtype": "bf16", "n_gpus": 1,
+                      "steps": args.steps, "config": {"workload": workload_name(args.config, sh), "l2": "256 MB flush between timed iterations"},
+                      "dense_attn_ms": dense_ms, "variants": lines}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -456,8 +512,13 @@ def main():
     ap.add_argument("--skip-cpu", action="store_true")
     ap.add_argument("--stack", action="store_true", help="time the whole stack with the index cache and as one CUDA graph")
     ap.add_argument("--layers", type=int, default=24)
+    ap.add_argument("--token", action="store_true", help="time the token-granular variants (NEXT-2) on one layer")
+    ap.add_argument("--strides", type=int, nargs="*", default=[8, 32, 64])
+    ap.add_argument("--topks", type=int, nargs="*", default=[1024, 4096, 16384])
     args = ap.parse_args()
-    if args.stack:
+    if args.token:
+        run_token(args)
+    elif args.stack:
         run_stack(args)
     elif args.impl == "reference":
         run_reference(args)
