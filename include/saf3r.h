@@ -137,8 +137,10 @@ saf3r_status saf3r_dense_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_d
                               void *cuda_stream);
 
 /* End-to-end convenience for HOST buffers (one global-attention layer): copies q/k/v (contiguous [H][N][D] bf16, ideally
- * pinned) to the device scratch, runs select + sparse_attn, copies the bf16 output back to out_host, all on
- * `cuda_stream`; returns after enqueueing (synchronise the stream before reading out_host).
+ * pinned) to the device scratch, runs select + sparse_attn, copies the bf16 output back to out_host; returns after
+ * enqueueing (synchronise `cuda_stream` before reading out_host).  The work is pipelined over up to eight groups of heads
+ * on context-owned side streams that are forked from and joined back to `cuda_stream` with events, so that the copies of
+ * one group overlap the compute of another; to `cuda_stream` it behaves like one ordered operation.
  * scratch_dev must hold saf3r_layer_host_scratch_bytes(...) bytes; shape strides are ignored (contiguous). */
 saf3r_status saf3r_layer_host_scratch_bytes(const saf3r_shape *shape, const saf3r_head_cfg *cfg_host, size_t *bytes);
 saf3r_status saf3r_layer_host(saf3r_ctx *ctx, const void *q_host, const void *k_host, const void *v_host,

@@ -36,6 +36,8 @@ struct saf3r_ctx {
   std::string err;
   bool sticky_cuda = false;
   int64_t launches = 0;
+  cudaStream_t side[3] = {nullptr, nullptr, nullptr};  // saf3r_layer_host: head-group pipeline (created on first use)
+  cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
   bool stage_timing = false;
   cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};  // select: start, after the pool launch, after the select launch
   bool ev_valid = false;
@@ -202,6 +204,11 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
 void saf3r_destroy(saf3r_ctx *ctx) {
   if (!ctx) return;
   for (auto &e : ctx->ev)
+    if (e) cudaEventDestroy(e);
+  for (auto &sd : ctx->side)
+    if (sd) cudaStreamDestroy(sd);
+  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  for (auto &e : ctx->ev_join)
     if (e) cudaEventDestroy(e);
   delete ctx;
 }
@@ -568,10 +575,21 @@ saf3r_status saf3r_token_set_attn(saf3r_ctx *ctx, const void *q, const void *k, 
   return attn_common(ctx, q, kc, vc, shape, nullptr, out, out_is_fp32, lse, stream_, &kv);
 }
 
+// saf3r_layer_host pipelines the layer over groups of heads (heads are independent): the host->device copy of
+// group g+1 runs under the select + attention of group g, and the device->host copy of group g under the compute of group
+// g+1 (separate copy engines), on ctx-owned side streams forked from / joined to the caller's stream with events.
+constexpr int kHostGroups = 8, kHostStreams = 3;
+struct HostGroup { int h0, hn; size_t ws, row_ptr, col_idx; int64_t entries; };
 struct HostLayout {
-  size_t q, k, v, out, ws, row_ptr, col_idx, total;
-  int64_t entries;
+  size_t q, k, v, out, total;
+  int n_groups;
+  HostGroup grp[kHostGroups];
 };
+static SelGeom sub_geom(const SelGeom &g, int hn) {
+  SelGeom s = g;
+  s.H = hn;
+  return s;
+}
 static HostLayout host_layout(const SelGeom &g, const saf3r_head_cfg *cfg) {
   HostLayout l;
   const size_t t = align256((size_t)g.H * g.N * 64 * 2);
@@ -580,10 +598,19 @@ static HostLayout host_layout(const SelGeom &g, const saf3r_head_cfg *cfg) {
   l.k = off; off += t;
   l.v = off; off += t;
   l.out = off; off += t;
-  l.ws = off; off += ws_layout(g).total;
-  l.row_ptr = off; off = align256(off + ((size_t)g.H * g.NB + 1) * 8);
-  l.entries = total_entries(g, cfg);
-  l.col_idx = off; off = align256(off + (size_t)(l.entries > 0 ? l.entries : 1) * 4);
+  l.n_groups = g.H < kHostGroups ? g.H : kHostGroups;
+  int h0 = 0;
+  for (int i = 0; i < l.n_groups; ++i) {
+    HostGroup &gr = l.grp[i];
+    gr.h0 = h0;
+    gr.hn = (g.H - h0 + (l.n_groups - i) - 1) / (l.n_groups - i);
+    h0 += gr.hn;
+    const SelGeom sg = sub_geom(g, gr.hn);
+    gr.ws = off; off += ws_layout(sg).total;
+    gr.row_ptr = off; off = align256(off + ((size_t)gr.hn * g.NB + 1) * 8);
+    gr.entries = total_entries(sg, cfg + gr.h0);
+    gr.col_idx = off; off = align256(off + (size_t)(gr.entries > 0 ? gr.entries : 1) * 4);
+  }
   l.total = off;
   return l;
 }
@@ -611,18 +638,38 @@ saf3r_status saf3r_layer_host(saf3r_ctx *ctx, const void *qh, const void *kh, co
   if (!qh || !kh || !vh || !scratch || !out_host) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
   const HostLayout l = host_layout(g, cfg);
   if (scratch_bytes < l.total) return fail(ctx, SAF3R_ERR_CAPACITY, "scratch too small (see saf3r_layer_host_scratch_bytes)");
+  if (!ctx->side[0]) {
+    for (auto &sd : ctx->side) CU_CHECK(cudaStreamCreateWithFlags(&sd, cudaStreamNonBlocking));
+    CU_CHECK(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
+    for (auto &e : ctx->ev_join) CU_CHECK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  }
   cudaStream_t st = (cudaStream_t)stream_;
   uint8_t *sb = (uint8_t *)scratch;
-  const size_t bytes = (size_t)g.H * g.N * 64 * 2;
-  CU_CHECK(cudaMemcpyAsync(sb + l.q, qh, bytes, cudaMemcpyHostToDevice, st));
-  CU_CHECK(cudaMemcpyAsync(sb + l.k, kh, bytes, cudaMemcpyHostToDevice, st));
-  CU_CHECK(cudaMemcpyAsync(sb + l.v, vh, bytes, cudaMemcpyHostToDevice, st));
-  saf3r_lists lists{(int64_t *)(sb + l.row_ptr), (int32_t *)(sb + l.col_idx), l.entries > 0 ? l.entries : 1};
-  saf3r_status s = saf3r_select(ctx, sb + l.q, sb + l.k, &shape, cfg, sb + l.ws, ws_layout(g).total, &lists, stream_);
-  if (s != SAF3R_OK) return s;
-  s = saf3r_sparse_attn(ctx, sb + l.q, sb + l.k, sb + l.v, &shape, &lists, sb + l.out, 0, nullptr, stream_);
-  if (s != SAF3R_OK) return s;
-  CU_CHECK(cudaMemcpyAsync(out_host, sb + l.out, bytes, cudaMemcpyDeviceToHost, st));
+  const size_t head_bytes = (size_t)g.N * 64 * 2;
+  CU_CHECK(cudaEventRecord(ctx->ev_fork, st));
+  const int n_streams = l.n_groups < kHostStreams ? l.n_groups : kHostStreams;
+  for (int i = 0; i < n_streams; ++i) CU_CHECK(cudaStreamWaitEvent(ctx->side[i], ctx->ev_fork, 0));
+  for (int i = 0; i < l.n_groups; ++i) {
+    const HostGroup &gr = l.grp[i];
+    cudaStream_t ss = ctx->side[i % kHostStreams];
+    const size_t o = (size_t)gr.h0 * head_bytes, nb = (size_t)gr.hn * head_bytes;
+    CU_CHECK(cudaMemcpyAsync(sb + l.q + o, (const uint8_t *)qh + o, nb, cudaMemcpyHostToDevice, ss));
+    CU_CHECK(cudaMemcpyAsync(sb + l.k + o, (const uint8_t *)kh + o, nb, cudaMemcpyHostToDevice, ss));
+    CU_CHECK(cudaMemcpyAsync(sb + l.v + o, (const uint8_t *)vh + o, nb, cudaMemcpyHostToDevice, ss));
+    saf3r_shape sub = shape;
+    sub.num_heads = gr.hn;
+    saf3r_lists lists{(int64_t *)(sb + gr.row_ptr), (int32_t *)(sb + gr.col_idx), gr.entries > 0 ? gr.entries : 1};
+    saf3r_status s = saf3r_select(ctx, sb + l.q + o, sb + l.k + o, &sub, cfg + gr.h0, sb + gr.ws, ws_layout(sub_geom(g, gr.hn)).total,
+                                  &lists, ss);
+    if (s != SAF3R_OK) return s;
+    s = saf3r_sparse_attn(ctx, sb + l.q + o, sb + l.k + o, sb + l.v + o, &sub, &lists, sb + l.out + o, 0, nullptr, ss);
+    if (s != SAF3R_OK) return s;
+    CU_CHECK(cudaMemcpyAsync((uint8_t *)out_host + o, sb + l.out + o, nb, cudaMemcpyDeviceToHost, ss));
+  }
+  for (int i = 0; i < n_streams; ++i) {
+    CU_CHECK(cudaEventRecord(ctx->ev_join[i], ctx->side[i]));
+    CU_CHECK(cudaStreamWaitEvent(st, ctx->ev_join[i], 0));
+  }
   return SAF3R_OK;
 }
 
