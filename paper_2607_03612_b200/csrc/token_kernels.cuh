@@ -108,6 +108,9 @@ __global__ void __launch_bounds__(256) token_probe_kernel(const __nv_bfloat16 *_
 }
 
 // grid (H), 1024 threads.  idx[h][0..K): the K tokens with the largest keys, ascending; ties at the cut by lower index.
+// Every pass keeps eight independent loads in flight per thread (the keys are L2-resident; one CTA per head is latency-bound
+// otherwise).  Histogram passes read strided (order does not matter), the compaction pass reads eight CONSECUTIVE keys per
+// thread so that a block-wide scan of per-thread counts gives ordered output positions.
 __global__ void __launch_bounds__(1024) token_topk_kernel(const uint32_t *__restrict__ keys, int32_t *__restrict__ idx, int64_t N, int K) {
   const int h = blockIdx.x;
   const uint32_t *key = keys + (int64_t)h * N;
@@ -122,9 +125,18 @@ __global__ void __launch_bounds__(1024) token_topk_kernel(const uint32_t *__rest
   for (int shift = 24; shift >= 0; shift -= 8) {
     for (int i = threadIdx.x; i < 32 * 256; i += 1024) (&hist[0][0])[i] = 0;
     __syncthreads();
-    for (int64_t j = threadIdx.x; j < N; j += 1024) {
-      const uint32_t kv = key[j];
-      if ((kv & mask) == prefix) atomicAdd(&hist[warp][(kv >> shift) & 255u], 1u);
+    for (int64_t j0 = 0; j0 < N; j0 += 8 * 1024) {
+      uint32_t kv[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int64_t j = j0 + threadIdx.x + 1024 * i;
+        kv[i] = j < N ? __ldg(key + j) : 0u;
+      }
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int64_t j = j0 + threadIdx.x + 1024 * i;
+        if (j < N && (kv[i] & mask) == prefix) atomicAdd(&hist[warp][(kv[i] >> shift) & 255u], 1u);
+      }
     }
     __syncthreads();
     if (threadIdx.x < 256) {
@@ -152,29 +164,57 @@ __global__ void __launch_bounds__(1024) token_topk_kernel(const uint32_t *__rest
   }
   const uint32_t tau = prefix;  // K-th largest key; take all keys above it and the first `need` (by index) equal to it
   int written = 0, eq_seen = 0;
-  const uint32_t lt = (1u << lane) - 1u;
-  for (int64_t j0 = 0; j0 < N; j0 += 1024) {
-    const int64_t j = j0 + threadIdx.x;
-    const uint32_t kv = j < N ? key[j] : 0u;
-    const bool gt = j < N && kv > tau, eq = j < N && kv == tau;
-    const uint32_t eqb = __ballot_sync(0xffffffffu, eq);
-    if (lane == 0) weq[warp] = __popc(eqb);
+  for (int64_t j0 = 0; j0 < N; j0 += 8 * 1024) {
+    const int64_t jb = j0 + 8 * (int64_t)threadIdx.x;  // this thread's eight consecutive keys
+    uint32_t kv[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) kv[i] = jb + i < N ? __ldg(key + jb + i) : 0u;
+    int n_eq = 0, n_gt = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const bool in = jb + i < N;
+      n_eq += (in && kv[i] == tau) ? 1 : 0;
+      n_gt += (in && kv[i] > tau) ? 1 : 0;
+    }
+    // block-wide exclusive scan of the tie counts (needed to decide which ties are among the first `need`)
+    int eq_inc = n_eq;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, eq_inc, off);
+      if (lane >= off) eq_inc += t;
+    }
+    if (lane == 31) weq[warp] = eq_inc;
     __syncthreads();
-    int eq_before = eq_seen, eq_total = 0;
+    int eq_before = eq_seen + eq_inc - n_eq, eq_total = 0;
     for (int w = 0; w < 32; ++w) {
       if (w < warp) eq_before += weq[w];
       eq_total += weq[w];
     }
-    const bool take = gt || (eq && eq_before + __popc(eqb & lt) < need);
-    const uint32_t tb = __ballot_sync(0xffffffffu, take);
-    if (lane == 0) wtake[warp] = __popc(tb);
+    int n_take = n_gt, eq_room = need - eq_before;  // ties this thread may still take
+    if (eq_room < 0) eq_room = 0;
+    n_take += n_eq < eq_room ? n_eq : eq_room;
+    int tk_inc = n_take;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, tk_inc, off);
+      if (lane >= off) tk_inc += t;
+    }
+    if (lane == 31) wtake[warp] = tk_inc;
     __syncthreads();
-    int before = written, total = 0;
+    int pos = written + tk_inc - n_take, total = 0;
     for (int w = 0; w < 32; ++w) {
-      if (w < warp) before += wtake[w];
+      if (w < warp) pos += wtake[w];
       total += wtake[w];
     }
-    if (take) out[before + __popc(tb & lt)] = (int32_t)j;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const bool in = jb + i < N;
+      bool take = in && kv[i] > tau;
+      if (in && kv[i] == tau) {
+        if (eq_room > 0) { take = true; --eq_room; }
+      }
+      if (take) out[pos++] = (int32_t)(jb + i);
+    }
     written += total;
     eq_seen += eq_total;
     __syncthreads();
