@@ -45,6 +45,8 @@ struct saf3r_ctx {
   // per-head list totals of the lists saf3r_select last wrote into a given row_ptr buffer (scheduling hint only)
   struct LenHint { const int64_t *row_ptr; int32_t H, NB; int64_t len[SAF3R_MAX_HEADS]; };
   std::vector<LenHint> hints;
+  struct SizeMemo { int32_t H, S, T, B; saf3r_head_cfg cfg[SAF3R_MAX_HEADS]; int64_t len[SAF3R_MAX_HEADS]; int64_t total; };
+  std::vector<SizeMemo> sizes;
 };
 
 static saf3r_status fail(saf3r_ctx *ctx, saf3r_status st, const std::string &msg) {
@@ -264,7 +266,24 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
   const WsLayout w = ws_layout(g);
   saf3r_ctx::LenHint hint;
   memset(&hint, 0, sizeof hint);
-  const int64_t need = total_entries(g, cfg, hint.len);
+  // list sizes are a closed form of (shape, cfg); the per-row-length STATIC rules cost O(NB) .. O(NB*S) host work, so the last
+  // few (shape, cfg) -> sizes results are memoised
+  int64_t need = -1;
+  for (auto &e : ctx->sizes)
+    if (e.H == g.H && e.S == g.S && e.T == g.T && e.B == g.B && memcmp(e.cfg, cfg, sizeof(saf3r_head_cfg) * g.H) == 0) {
+      memcpy(hint.len, e.len, sizeof hint.len);
+      need = e.total;
+    }
+  if (need < 0) {
+    need = total_entries(g, cfg, hint.len);
+    saf3r_ctx::SizeMemo m;
+    m.H = g.H; m.S = g.S; m.T = g.T; m.B = g.B; m.total = need;
+    memset(m.cfg, 0, sizeof m.cfg);
+    memcpy(m.cfg, cfg, sizeof(saf3r_head_cfg) * g.H);
+    memcpy(m.len, hint.len, sizeof m.len);
+    if (ctx->sizes.size() >= 64) ctx->sizes.erase(ctx->sizes.begin());
+    ctx->sizes.push_back(m);
+  }
   if (ws_bytes < w.total || lists->capacity < need) {
     char buf[160];
     snprintf(buf, sizeof buf, "capacity: need %lld list entries (have %lld), %zu workspace bytes (have %zu)", (long long)need,

@@ -260,9 +260,51 @@ __device__ __forceinline__ void emit_light_row(const SelGeom &g, const saf3r_hea
       hi = (((t1 - 1) / g.T + 1) * g.T - 1) / g.B;
     }
     for (int64_t J = lo + lane; J <= hi; J += 32) out[J - lo] = (int32_t)J;
-  } else if (lane == 0) {
-    int64_t w = 0;
-    closed_form_row(g, c, I, [&](int64_t J) { out[w++] = (int32_t)J; });
+  } else {
+    // POSITION_BAND, lane-parallel: the row is a sequence of (frame, interval) block ranges [a_i, b_i]; b_i is a closed form and
+    // a_i = max(first block of the interval, b_{i-1} + 1) only needs the previous range's END, so 32 ranges are sized at once
+    // and placed with a warp prefix sum (same set and order as closed_form_row, which the host sizing uses)
+    const int64_t T = g.T, B = g.B;
+    const int64_t t0 = I * B, t1 = i64min(t0 + B, g.N);
+    const int64_t f0 = t0 / T, f1 = (t1 - 1) / T, r = c.band_radius;
+    int64_t lo[2], hi[2];
+    int ni;
+    if (f1 == f0) {
+      lo[0] = i64max(0, t0 - f0 * T - r); hi[0] = i64min(T - 1, (t1 - 1) - f0 * T + r); ni = 1;
+    } else if (f1 - f0 >= 2) {
+      lo[0] = 0; hi[0] = T - 1; ni = 1;
+    } else {
+      const int64_t loA = i64max(0, t0 - f0 * T - r), hiB = i64min(T - 1, (t1 - 1) - f1 * T + r);
+      if (hiB + 1 >= loA) { lo[0] = 0; hi[0] = T - 1; ni = 1; }
+      else { lo[0] = 0; hi[0] = hiB; lo[1] = loA; hi[1] = T - 1; ni = 2; }
+    }
+    const int64_t items = (int64_t)g.S * ni;
+    int64_t base = 0;
+    for (int64_t i0 = 0; i0 < items; i0 += 32) {
+      const int64_t i = i0 + lane;
+      int64_t a = 0, b = -1;
+      if (i < items) {
+        const int64_t fr = i / ni;
+        const int qi = (int)(i % ni);
+        b = (fr * T + hi[qi]) / B;
+        a = (fr * T + lo[qi]) / B;
+        if (i > 0) {
+          const int64_t pf = (i - 1) / ni;
+          const int pq = (int)((i - 1) % ni);
+          a = i64max(a, (pf * T + hi[pq]) / B + 1);  // the previous range's end (ends are non-decreasing)
+        }
+      }
+      const int cnt = (int)i64max(0, b - a + 1);
+      int inc = cnt;
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, off);
+        if (lane >= off) inc += t;
+      }
+      int32_t *dst = out + base + inc - cnt;
+      for (int j = 0; j < cnt; ++j) dst[j] = (int32_t)(a + j);
+      base += __shfl_sync(0xffffffffu, inc, 31);
+    }
   }
 }
 constexpr int kLightRows = 32;  // rows per CTA of the light emitters (8 warps x 4 rows)
