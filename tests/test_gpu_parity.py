@@ -488,3 +488,18 @@ def test_token_variants_at_c2_size_sampled_rows(env):
     oi, p = orc.token_probe_topk(L.q[12], L.k[12], 1024)         # a sink head: the special tokens of every frame
     assert len(np.setxor1d(gi[12], oi)) <= 4
     assert np.isin(np.arange(sh.S) * sh.T, gi[12]).all()
+
+
+def test_select_position_band_many_frames(env):
+    """POSITION_BAND with more than 32 (frame, interval) ranges per row (the lane-parallel emitter runs several warp rounds),
+    blocks that straddle frames (two intervals per row) and radii from 0 to >= T (dense)."""
+    sf, ctx, torch = env
+    radii = [0, 3, 40, 200]
+    sh = sy.Shape(S=40, G=9, H=len(radii), D=64, B=64)            # T = 86, N = 3440, NB = 54
+    cfgs = [sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_POSITION_BAND, band_radius=r) for r in radii]
+    L = sy.make_layer(sh, [sy.GEN_SAME_POSITION] * len(radii), cfgs, seed=61)
+    q, k, _ = upload(L)
+    lists = ctx.select(q, k, c_shape(sf, sh), L.cfgs)
+    torch.cuda.synchronize()
+    stats = compare_lists(L, lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy(), oracle_lists(L, want_scores=False))
+    assert stats["tie_floored"] == 0 and stats["entries"] > 0
