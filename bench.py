@@ -319,6 +319,22 @@ def run_ours(args):
             result["dense_attn_ms"] = dense_ms
             result["dense_tflops"] = dense_flop / (dense_ms * 1e-3) / 1e12
             result["speedup_vs_own_dense"] = dense_ms / ms_per_step
+            # quality of the sparse layer against the library's own dense output (Eq. 1 of the paper; reported,
+            # not a gate): NMSE per head of layer 0, summarised by head generator.  d["out"] holds the dense output now.
+            sp = torch.empty_like(d["out"])
+            ctx.select(d["q"], d["k"], shape, d["cfgs"], workspace=d["ws"], lists=d["lists"])
+            ctx.sparse_attn(d["q"], d["k"], d["v"], shape, d["lists"], out=sp)
+            torch.cuda.synchronize()
+            nm = []
+            for h in range(sh.H):                                 # per head, to bound the fp32 temporaries
+                a, b = d["out"][h].float(), sp[h].float()
+                nm.append(float(((a - b).double().pow(2).sum() / a.double().pow(2).sum()).item()))
+            by = {}
+            for h, gname in enumerate(layers[0].gens):
+                by.setdefault(gname, []).append(nm[h])
+            result["quality_vs_own_dense"] = {"nmse_by_generator": {k2: float(np.mean(v2)) for k2, v2 in by.items()},
+                                              "nmse_max": float(max(nm)), "note": "layer 0; Eq. 1 (PAPER.md:L108) with O_full = dense mode, bf16 outputs"}
+            del sp
 
         # e2e through the C ABI with HOST buffers (pinned), H2D + D2H inside the timed region
         if not args.skip_e2e:
