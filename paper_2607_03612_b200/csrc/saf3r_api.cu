@@ -520,7 +520,7 @@ saf3r_status saf3r_token_stride_attn(saf3r_ctx *ctx, const void *q, const void *
 }
 
 struct TokWs {
-  size_t part, keys, select_total, kc, vc, attn_total;
+  size_t part, keys, hist1, select_total, kc, vc, attn_total;
   int n_chunks;
 };
 static TokWs tok_ws(const SelGeom &g, int K) {
@@ -529,6 +529,7 @@ static TokWs tok_ws(const SelGeom &g, int K) {
   size_t off = 0;
   w.part = off; off = align256(off + (size_t)g.H * w.n_chunks * 64 * sizeof(float));
   w.keys = off; off = align256(off + (size_t)g.H * g.N * sizeof(uint32_t));
+  w.hist1 = off; off = align256(off + (size_t)g.H * kTokBins1 * sizeof(uint32_t));
   w.select_total = off;
   off = 0;
   w.kc = off; off = align256(off + (size_t)g.H * K * 64 * 2);
@@ -562,11 +563,11 @@ saf3r_status saf3r_token_probe_select(saf3r_ctx *ctx, const void *q, const void 
   if (ws_bytes < w.select_total) return fail(ctx, SAF3R_ERR_CAPACITY, "workspace too small (saf3r_token_query_sizes)");
   cudaStream_t st = (cudaStream_t)stream_;
   float *part = (float *)((uint8_t *)ws + w.part);
-  uint32_t *keys = (uint32_t *)((uint8_t *)ws + w.keys);
-  token_qsum_kernel<<<dim3(w.n_chunks, g.H), 256, 0, st>>>((const __nv_bfloat16 *)q, part, g);
-  token_probe_kernel<<<dim3((unsigned)((g.N + kTokTile - 1) / kTokTile), g.H), 256, 0, st>>>((const __nv_bfloat16 *)k, part, keys, g,
-                                                                                           w.n_chunks);
-  token_topk_kernel<<<g.H, 1024, 0, st>>>(keys, idx, g.N, K);
+  uint32_t *keys = (uint32_t *)((uint8_t *)ws + w.keys), *hist1 = (uint32_t *)((uint8_t *)ws + w.hist1);
+  token_qsum_kernel<<<dim3(w.n_chunks, g.H), 256, 0, st>>>((const __nv_bfloat16 *)q, part, hist1, g);
+  token_probe_kernel<<<dim3((unsigned)((g.N + kTokTile - 1) / kTokTile), g.H), 256, 0, st>>>((const __nv_bfloat16 *)k, part, keys, hist1,
+                                                                                           g, w.n_chunks);
+  token_topk_kernel<<<g.H, 1024, 0, st>>>(keys, hist1, idx, g.N, K);
   ctx->launches += 3;
   CU_CHECK(cudaGetLastError());
   return SAF3R_OK;

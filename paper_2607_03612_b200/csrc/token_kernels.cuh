@@ -30,8 +30,13 @@ __device__ __forceinline__ void bf16x8_to_f32(const uint4 &raw, float (&v)[8]) {
 }
 
 // grid (ceil(N / kTokChunk), H), 256 threads: lane group of 8 threads = one token row (16 B each), 32 rows per step.
-__global__ void __launch_bounds__(256) token_qsum_kernel(const __nv_bfloat16 *__restrict__ q, float *__restrict__ part, SelGeom g) {
+constexpr int kTokBins1 = 2048;  // histogram of the top 11 key bits, built by the probe pass for the top-K pass
+
+__global__ void __launch_bounds__(256) token_qsum_kernel(const __nv_bfloat16 *__restrict__ q, float *__restrict__ part,
+                                                         uint32_t *__restrict__ hist1, SelGeom g) {
   const int h = blockIdx.y, chunk = blockIdx.x;
+  if (chunk == 0)  // the probe launch that follows accumulates into it
+    for (int i = threadIdx.x; i < kTokBins1; i += 256) hist1[(int64_t)h * kTokBins1 + i] = 0u;
   const int sub = threadIdx.x & 7, row = threadIdx.x >> 3;
   const int64_t t0 = (int64_t)chunk * kTokChunk;
   const int cnt = (int)i64min(kTokChunk, g.N - t0);
@@ -67,9 +72,12 @@ __global__ void __launch_bounds__(256) token_qsum_kernel(const __nv_bfloat16 *__
 
 // grid (ceil(N / kTokTile), H), 256 threads.  keys[h][j] = order-preserving key of p[j] = qbar . k_j / sqrt(D).
 __global__ void __launch_bounds__(256) token_probe_kernel(const __nv_bfloat16 *__restrict__ k, const float *__restrict__ part,
-                                                          uint32_t *__restrict__ keys, SelGeom g, int n_chunks) {
+                                                          uint32_t *__restrict__ keys, uint32_t *__restrict__ hist1, SelGeom g,
+                                                          int n_chunks) {
   const int h = blockIdx.y;
   __shared__ float qb[64];
+  __shared__ uint32_t sh1[kTokBins1];
+  for (int i = threadIdx.x; i < kTokBins1; i += 256) sh1[i] = 0u;
   if (threadIdx.x < 64) {
     float t = 0.f;
     for (int c = 0; c < n_chunks; ++c) t += part[((int64_t)h * n_chunks + c) * 64 + threadIdx.x];  // fixed order
@@ -102,28 +110,64 @@ __global__ void __launch_bounds__(256) token_probe_kernel(const __nv_bfloat16 *_
       d += __shfl_xor_sync(0xffffffffu, d, 2);
       d += __shfl_xor_sync(0xffffffffu, d, 4);
       const int r = r0 + row + 32 * i;
-      if (sub == 0 && r < cnt) keys[(int64_t)h * g.N + t0 + r] = score_key(d * 0.125f);
+      if (sub == 0 && r < cnt) {
+        const uint32_t key = score_key(d * 0.125f);
+        keys[(int64_t)h * g.N + t0 + r] = key;
+        atomicAdd(&sh1[key >> 21], 1u);
+      }
     }
   }
+  __syncthreads();
+  for (int i = threadIdx.x; i < kTokBins1; i += 256)
+    if (sh1[i]) atomicAdd(&hist1[(int64_t)h * kTokBins1 + i], sh1[i]);
 }
 
 // grid (H), 1024 threads.  idx[h][0..K): the K tokens with the largest keys, ascending; ties at the cut by lower index.
-// Every pass keeps eight independent loads in flight per thread (the keys are L2-resident; one CTA per head is latency-bound
-// otherwise).  Histogram passes read strided (order does not matter), the compaction pass reads eight CONSECUTIVE keys per
-// thread so that a block-wide scan of per-thread counts gives ordered output positions.
-__global__ void __launch_bounds__(1024) token_topk_kernel(const uint32_t *__restrict__ keys, int32_t *__restrict__ idx, int64_t N, int K) {
+// Radix select in three digits (11 + 11 + 10 bits).  The histogram of the first digit over ALL keys comes from the probe pass
+// (hist1), so no pass here issues a shared-memory atomic per key: the two remaining histogram passes only count the keys that
+// match the prefix found so far.  Every pass keeps eight independent loads in flight per thread (the keys are L2-resident; one
+// CTA per head is latency-bound otherwise).  Histogram passes read strided (order does not matter), the compaction pass reads
+// eight CONSECUTIVE keys per thread so that a block-wide scan of per-thread counts gives ordered output positions.
+__global__ void __launch_bounds__(1024) token_topk_kernel(const uint32_t *__restrict__ keys, const uint32_t *__restrict__ hist1,
+                                                          int32_t *__restrict__ idx, int64_t N, int K) {
   const int h = blockIdx.x;
   const uint32_t *key = keys + (int64_t)h * N;
   int32_t *out = idx + (int64_t)h * K;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  __shared__ uint32_t hist[32][256];  // one private histogram per warp
-  __shared__ uint32_t tot[256];
+  __shared__ uint32_t hist[kTokBins1];
+  __shared__ uint32_t wsum[32];
   __shared__ uint32_t s_prefix, s_need;
   __shared__ int wtake[32], weq[32];
   uint32_t prefix = 0, mask = 0;
   int need = K;
-  for (int shift = 24; shift >= 0; shift -= 8) {
-    for (int i = threadIdx.x; i < 32 * 256; i += 1024) (&hist[0][0])[i] = 0;
+  // digit d of `bits` bits at `shift`: hist[] holds the counts of the keys that match (prefix, mask); pick the bin, from the top,
+  // in which the running count reaches `need` (block-wide: each thread owns two adjacent bins, suffix sums by warp scans)
+  auto pick_bin = [&](int shift, int bins) {
+    const int b0 = bins - 1 - 2 * (int)threadIdx.x, b1 = b0 - 1;  // descending bin order
+    const uint32_t c0 = b0 >= 0 ? hist[b0] : 0u, c1 = b1 >= 0 ? hist[b1] : 0u;
+    uint32_t inc = c0 + c1;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, off);
+      if (lane >= off) inc += t;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    uint32_t before = inc - (c0 + c1);  // keys in higher bins
+    for (int w = 0; w < warp; ++w) before += wsum[w];
+    if (before < (uint32_t)need && before + c0 + c1 >= (uint32_t)need) {  // exactly one thread
+      const bool first = before + c0 >= (uint32_t)need;
+      s_prefix = prefix | ((uint32_t)(first ? b0 : b1) << shift);
+      s_need = (uint32_t)need - before - (first ? 0u : c0);
+    }
+    __syncthreads();
+    prefix = s_prefix;
+    need = (int)s_need;
+    mask |= (uint32_t)(bins - 1) << shift;
+    __syncthreads();
+  };
+  auto count_digit = [&](int shift, int bins) {
+    for (int i = threadIdx.x; i < bins; i += 1024) hist[i] = 0u;
     __syncthreads();
     for (int64_t j0 = 0; j0 < N; j0 += 8 * 1024) {
       uint32_t kv[8];
@@ -135,33 +179,18 @@ __global__ void __launch_bounds__(1024) token_topk_kernel(const uint32_t *__rest
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
         const int64_t j = j0 + threadIdx.x + 1024 * i;
-        if (j < N && (kv[i] & mask) == prefix) atomicAdd(&hist[warp][(kv[i] >> shift) & 255u], 1u);
+        if (j < N && (kv[i] & mask) == prefix) atomicAdd(&hist[(kv[i] >> shift) & (uint32_t)(bins - 1)], 1u);
       }
     }
     __syncthreads();
-    if (threadIdx.x < 256) {
-      uint32_t t = 0;
-#pragma unroll
-      for (int w = 0; w < 32; ++w) t += hist[w][threadIdx.x];
-      tot[threadIdx.x] = t;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {  // 256 bins from the top: find the bin in which the running count reaches `need`
-      uint32_t run = 0;
-      int b = 255;
-      for (; b > 0; --b) {
-        if (run + tot[b] >= (uint32_t)need) break;
-        run += tot[b];
-      }
-      s_prefix = prefix | ((uint32_t)b << shift);
-      s_need = (uint32_t)need - run;
-    }
-    __syncthreads();
-    prefix = s_prefix;
-    need = (int)s_need;
-    mask |= 255u << shift;
-    __syncthreads();
-  }
+  };
+  for (int i = threadIdx.x; i < kTokBins1; i += 1024) hist[i] = hist1[(int64_t)h * kTokBins1 + i];
+  __syncthreads();
+  pick_bin(21, 2048);
+  count_digit(10, 2048);
+  pick_bin(10, 2048);
+  count_digit(0, 1024);
+  pick_bin(0, 1024);
   const uint32_t tau = prefix;  // K-th largest key; take all keys above it and the first `need` (by index) equal to it
   int written = 0, eq_seen = 0;
   for (int64_t j0 = 0; j0 < N; j0 += 8 * 1024) {
