@@ -5,8 +5,8 @@
 //       top-K tokens shared by all queries:
 //         token_qsum_kernel    per-chunk token sums of Q (HBM stream)
 //         token_probe_kernel   qbar from the chunk sums (fixed order), p[j] as order-preserving keys (HBM stream of K)
-//         token_topk_kernel    one CTA per head: 4x8-bit radix select of the K-th largest key over N keys (per-warp private
-//                              histograms), then an ordered block compaction -> ascending token indices, ties by lower index
+//         token_topk_kernel    one CTA per head: 11+11+10-bit radix select of the K-th largest key over N keys (first digit's
+//                              histogram from the probe pass), then an ordered block compaction -> ascending indices, ties by lower index
 //         token_gather_kernel  K/V rows of the selected tokens -> compact [H][K][64] tiles for the dense mode of the attention
 #pragma once
 #include <cuda_bf16.h>
