@@ -131,6 +131,12 @@ saf3r_status saf3r_sparse_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_
                                const saf3r_shape *shape, const saf3r_lists *lists, void *out_dev, int out_is_fp32,
                                float *lse_dev_or_null, void *cuda_stream);
 
+/* Validates caller-made lists (the format is open): row_ptr non-decreasing and within capacity, every row ascending, unique and
+ * inside [0, NB).  Writes the number of malformed rows to *bad_rows_host.  Synchronises `cuda_stream` (a debugging aid, not
+ * part of the hot path; saf3r_sparse_attn itself does not validate). */
+saf3r_status saf3r_check_lists(saf3r_ctx *ctx, const saf3r_shape *shape, const saf3r_lists *lists, int64_t *bad_rows_host,
+                               void *cuda_stream);
+
 /* Dense mode of the same kernel (implicit list 0..NB-1, no list reads). */
 saf3r_status saf3r_dense_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const void *v_dev,
                               const saf3r_shape *shape, void *out_dev, int out_is_fp32, float *lse_dev_or_null,

@@ -27,7 +27,7 @@ SCORE_DOT, SCORE_COSINE = range(2)
 EXPORTS = ("saf3r_create", "saf3r_destroy", "saf3r_last_error", "saf3r_query_sizes", "saf3r_select", "saf3r_sparse_attn",
            "saf3r_dense_attn", "saf3r_layer_host_scratch_bytes", "saf3r_layer_host", "saf3r_launch_count",
            "saf3r_set_stage_timing", "saf3r_last_select_stage_ms", "saf3r_select_cached", "saf3r_token_stride_attn",
-           "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn")
+           "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn", "saf3r_check_lists")
 
 
 class Saf3rError(RuntimeError):
@@ -76,6 +76,7 @@ def load_library():
         L.saf3r_token_query_sizes.argtypes = [C.POINTER(ShapeC), C.c_int32, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         L.saf3r_token_probe_select.argtypes = [vp, vp, vp, C.POINTER(ShapeC), C.c_int32, vp, C.c_size_t, vp, vp]
         L.saf3r_token_set_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), vp, C.c_int32, vp, C.c_size_t, vp, i32, vp, vp]
+        L.saf3r_check_lists.argtypes = [vp, C.POINTER(ShapeC), C.POINTER(ListsC), C.POINTER(i64), vp]
         L.saf3r_sparse_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(ListsC), vp, i32, vp, vp]
         L.saf3r_dense_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), vp, i32, vp, vp]
         L.saf3r_layer_host_scratch_bytes.argtypes = [C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(C.c_size_t)]
@@ -193,6 +194,13 @@ class Context:
             self._check(self.lib.saf3r_select(self.h, q.data_ptr(), k.data_ptr(), C.byref(shape), arr, workspace.data_ptr(),
                                               workspace.numel() * workspace.element_size(), C.byref(lc), _stream_ptr(stream)))
         return lists
+
+    # ---- saf3r_check_lists
+    def check_lists(self, shape: ShapeC, lists: Lists, stream=None) -> int:
+        """Number of malformed rows of caller-made lists (synchronises the stream)."""
+        lc, bad = lists.c(), C.c_int64()
+        self._check(self.lib.saf3r_check_lists(self.h, C.byref(shape), C.byref(lc), C.byref(bad), _stream_ptr(stream)))
+        return int(bad.value)
 
     # ---- saf3r_sparse_attn / saf3r_dense_attn
     def sparse_attn(self, q, k, v, shape: ShapeC, lists: Lists, out=None, out_fp32: bool = False, want_lse: bool = False, stream=None):

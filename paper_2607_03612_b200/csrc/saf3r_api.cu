@@ -38,6 +38,7 @@ struct saf3r_ctx {
   int64_t launches = 0;
   cudaStream_t side[3] = {nullptr, nullptr, nullptr};  // saf3r_layer_host: head-group pipeline (created on first use)
   cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
+  unsigned long long *counter_dev = nullptr;  // tiny device scratch (saf3r_check_lists)
   bool stage_timing = false;
   cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};  // select: start, after the pool launch, after the select launch
   bool ev_valid = false;
@@ -194,8 +195,9 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
   e = cudaFuncSetAttribute(saf3r_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->counter_dev, sizeof(unsigned long long));
   if (e != cudaSuccess) {
-    fprintf(stderr, "saf3r_create: cudaFuncSetAttribute failed: %s\n", cudaGetErrorString(e));
+    fprintf(stderr, "saf3r_create: cudaFuncSetAttribute / cudaMalloc failed: %s\n", cudaGetErrorString(e));
     delete ctx;
     return SAF3R_ERR_CUDA;
   }
@@ -207,6 +209,7 @@ void saf3r_destroy(saf3r_ctx *ctx) {
   if (!ctx) return;
   for (auto &e : ctx->ev)
     if (e) cudaEventDestroy(e);
+  if (ctx->counter_dev) cudaFree(ctx->counter_dev);
   for (auto &sd : ctx->side)
     if (sd) cudaStreamDestroy(sd);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -497,6 +500,26 @@ saf3r_status saf3r_sparse_attn(saf3r_ctx *ctx, const void *q, const void *k, con
                                const saf3r_lists *lists, void *out, int out_is_fp32, float *lse, void *stream) {
   if (!lists) return fail(ctx, SAF3R_ERR_INVALID_ARG, "lists is null");
   return attn_common(ctx, q, k, v, shape, lists, out, out_is_fp32, lse, stream);
+}
+
+saf3r_status saf3r_check_lists(saf3r_ctx *ctx, const saf3r_shape *shape, const saf3r_lists *lists, int64_t *bad_rows, void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_shape(shape, false)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  if (!lists || !lists->row_ptr || !lists->col_idx || !bad_rows) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  const SelGeom g = make_geom(shape);
+  cudaStream_t st = (cudaStream_t)stream_;
+  unsigned long long *bad = ctx->counter_dev, host = 0;  // allocated by saf3r_create
+  CU_CHECK(cudaMemsetAsync(bad, 0, sizeof *bad, st));
+  const int64_t rows = (int64_t)g.H * g.NB;
+  check_lists_kernel<<<(unsigned)((rows + 255) / 256 < 4096 ? (rows + 255) / 256 : 4096), 256, 0, st>>>(lists->row_ptr, lists->col_idx,
+                                                                                                       rows, g.NB, lists->capacity, bad);
+  ctx->launches += 1;
+  CU_CHECK(cudaMemcpyAsync(&host, bad, sizeof host, cudaMemcpyDeviceToHost, st));
+  CU_CHECK(cudaStreamSynchronize(st));
+  *bad_rows = (int64_t)host;
+  return SAF3R_OK;
 }
 
 saf3r_status saf3r_dense_attn(saf3r_ctx *ctx, const void *q, const void *k, const void *v, const saf3r_shape *shape, void *out,

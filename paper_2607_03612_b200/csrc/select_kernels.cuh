@@ -698,4 +698,23 @@ __global__ void __launch_bounds__(256, 2) select_kernel(const float *__restrict_
   }
 }
 
+// ------------------------------------------------------------------------------------------------ list validation
+// grid-stride over the H*NB rows: row_ptr non-decreasing, every row ascending, unique and inside [0, NB).  Counts bad rows.
+__global__ void __launch_bounds__(256) check_lists_kernel(const int64_t *__restrict__ row_ptr, const int32_t *__restrict__ col_idx,
+                                                          int64_t rows, int32_t NB, int64_t capacity, unsigned long long *bad) {
+  for (int64_t r = (int64_t)blockIdx.x * 256 + threadIdx.x; r < rows; r += (int64_t)gridDim.x * 256) {
+    const int64_t a = row_ptr[r], b = row_ptr[r + 1];
+    bool ok = a >= 0 && b >= a && b <= capacity && b - a <= NB;
+    if (ok) {
+      int32_t prev = -1;
+      for (int64_t i = a; i < b; ++i) {
+        const int32_t J = col_idx[i];
+        ok = ok && J > prev && J < NB;
+        prev = J;
+      }
+    }
+    if (!ok) atomicAdd(bad, 1ull);
+  }
+}
+
 }  // namespace saf3r

@@ -503,3 +503,23 @@ def test_select_position_band_many_frames(env):
     torch.cuda.synchronize()
     stats = compare_lists(L, lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy(), oracle_lists(L, want_scores=False))
     assert stats["tie_floored"] == 0 and stats["entries"] > 0
+
+
+def test_check_lists_flags_malformed_rows(env):
+    """The list format is open; saf3r_check_lists is the validation aid: lists written by saf3r_select are clean, rows that are
+    not ascending / not unique / out of range are counted."""
+    sf, ctx, torch = env
+    L = sy.config_c1()
+    q, k, _ = upload(L)
+    shape = c_shape(sf, L.shape)
+    lists = ctx.select(q, k, shape, L.cfgs)
+    assert ctx.check_lists(shape, lists) == 0
+    col = lists.col_idx.clone()
+    rp = lists.row_ptr.cpu().numpy()
+    r0 = int(np.nonzero(np.diff(rp) >= 2)[0][0])                 # a row with at least two entries
+    bad = sf.Lists(lists.row_ptr, col)
+    col[rp[r0]], col[rp[r0] + 1] = col[rp[r0] + 1].item(), col[rp[r0]].item()   # descending pair
+    assert ctx.check_lists(shape, bad) == 1
+    r1 = int(np.nonzero(np.diff(rp) >= 1)[0][-1])
+    col[rp[r1 + 1] - 1] = L.shape.NB                             # out of range in another row
+    assert ctx.check_lists(shape, bad) == (2 if r1 != r0 else 1)
