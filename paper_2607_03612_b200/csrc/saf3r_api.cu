@@ -373,8 +373,21 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
   }
   const int sel_ctas = sets.n_probe + sets.n_block * ((g.NB + R - 1) / R) + (sets.n_light + sets.n_cached) * light_chunks;
   if (sel_ctas > 0) {
-    select_kernel<<<sel_ctas, 256, sm, st>>>(qt, kt, probe, lists->row_ptr, qpart, probe, lists->col_idx,
-                                             cache ? cache->row_ptr : nullptr, cache ? cache->col_idx : nullptr, g, ca, sets, R);
+    cudaLaunchConfig_t lc;
+    memset(&lc, 0, sizeof lc);
+    lc.gridDim = dim3(sel_ctas);
+    lc.blockDim = dim3(256);
+    lc.dynamicSmemBytes = sm;
+    lc.stream = st;
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;  // may start while the pool grid drains (see the kernels)
+    attr.val.programmaticStreamSerializationAllowed = 1;
+    lc.attrs = &attr;
+    lc.numAttrs = 1;
+    CU_CHECK(cudaLaunchKernelEx(&lc, select_kernel, (const float *)qt, (const float *)kt, (const int32_t *)probe,
+                                (const int64_t *)lists->row_ptr, (const float *)qpart, probe, lists->col_idx,
+                                (const int64_t *)(cache ? cache->row_ptr : nullptr), (const int32_t *)(cache ? cache->col_idx : nullptr),
+                                g, ca, sets, R));
     ctx->launches += 1;
   }
   if (ctx->stage_timing) {

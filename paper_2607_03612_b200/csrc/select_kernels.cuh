@@ -406,6 +406,9 @@ __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16
                                                           float *__restrict__ qt, float *__restrict__ kt, float *__restrict__ qpart,
                                                           int64_t *__restrict__ row_ptr, int32_t *__restrict__ col_idx, SelGeom g, PoolJobs jobs, RowPtrPlan plan,
                                                           HeadCfgArray cfg, HeadSets sets, int pool_ctas, int pool_tasks) {
+  // programmatic dependent launch: let the select launch that follows become resident as this grid drains; it waits
+  // (griddepcontrol.wait) for this grid's completion before it reads anything written here
+  asm volatile("griddepcontrol.launch_dependents;");
   if ((int)blockIdx.x >= pool_ctas + g.H) {
     // ---------------------------------------------------------------- lists of a constant-length closed-form head
     const int chunks = (g.NB + kLightRows - 1) / kLightRows;
@@ -644,6 +647,7 @@ __global__ void __launch_bounds__(256, 2) select_kernel(const float *__restrict_
   extern __shared__ float sm[];
   __shared__ float part[4][64];
   __shared__ float qb[64];
+  asm volatile("griddepcontrol.wait;" ::: "memory");  // the pool launch has completed and its writes are visible
   const int strips = (g.NB + R - 1) / R;
   const int probe_ctas = sets.n_probe;
   const int heavy_ctas = sets.n_block * strips;
