@@ -523,3 +523,33 @@ def test_check_lists_flags_malformed_rows(env):
     r1 = int(np.nonzero(np.diff(rp) >= 1)[0][-1])
     col[rp[r1 + 1] - 1] = L.shape.NB                             # out of range in another row
     assert ctx.check_lists(shape, bad) == (2 if r1 != r0 else 1)
+
+
+def test_c5_shape_three_heads(env):
+    """BASELINE.json's largest configuration (S = 500 frames, N = 687 000, NB = 5368, tail 24) with three heads instead of 16 so
+    that the oracle finishes in about a minute: block top-k (score strips of few rows, top-n bisection over keys in shared
+    memory, 5 main passes of 1024 columns + left-over), query-probe over 5368 blocks, frame-local; sampled q-blocks of the
+    attention against the oracle on the GPU's own lists."""
+    sf, ctx, torch = env
+    sh = sy.Shape(S=500, G=37, H=3, D=64, B=128)
+    assert sh.NB == 5368
+    gens = [sy.GEN_SAME_POSITION, sy.GEN_SINK, sy.GEN_FRAME_LOCAL]
+    cfgs = [sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=537),
+            sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=500),
+            sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_FRAME_LOCAL)]
+    L = sy.make_layer(sh, gens, cfgs, seed=5005)
+    q, k, v = upload(L)
+    shape = c_shape(sf, sh)
+    lists = ctx.select(q, k, shape, L.cfgs)
+    out = ctx.sparse_attn(q, k, v, shape, lists, out_fp32=True)
+    torch.cuda.synchronize()
+    assert ctx.check_lists(shape, lists) == 0
+    rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
+    stats = compare_lists(L, rp, col, oracle_lists(L))
+    print("C5-shape near-ties:", stats)
+    assert stats["tie_floored"] <= 1e-3 * stats["entries"]
+    for h in range(sh.H):
+        qb = np.array([sh.NB // 3, sh.NB - 1], np.int64)
+        r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
+        ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, r - r[0], col[r[0]:r[-1]], qb, want_lse=False)
+        check_attention(out[h].cpu().numpy(), ref, f"C5-shape head {h} ({gens[h]})")
