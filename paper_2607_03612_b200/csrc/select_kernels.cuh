@@ -115,15 +115,16 @@ __device__ __forceinline__ uint32_t score_key(float s) {
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
 
-constexpr int kKeysPerLaneReg = 36;  // rows with NB <= 32*36 keep their keys in registers during the bisection
+// rows with NB <= 32*36 (or <= 32*72) keep their keys in registers during the bisection; longer rows re-read shared memory
 
 // One warp: keep the n largest of key[0..NB) (order-preserving keys in shared memory) under (key desc, index asc);
 // write their indices ascending to out.  No atomics, no sort: a bitwise bisection finds the n-th largest key tau (one
 // warp-wide count of {key >= candidate} per bit, keys distributed over the lanes; it stops early as soon as a candidate
 // splits the row into exactly n and NB-n keys), then an ordered ballot compaction emits {key > tau} plus the first
 // `need` (by index) of {key == tau}.
-template <bool kRegs>
+template <int kKeysPerLaneReg>  // 0: keys stay in shared memory
 __device__ __forceinline__ void warp_topn_bisect_impl(const uint32_t *key, int NB, int n, int32_t *out) {
+  constexpr bool kRegs = kKeysPerLaneReg > 0;
   const int lane = threadIdx.x & 31;
   uint32_t kk[kRegs ? kKeysPerLaneReg : 1];
   if (kRegs) {
@@ -194,8 +195,9 @@ __device__ __forceinline__ void warp_topn_bisect_impl(const uint32_t *key, int N
   }
 }
 __device__ __forceinline__ void warp_topn_bisect(const uint32_t *key, int NB, int n, int32_t *out) {
-  if (NB <= 32 * kKeysPerLaneReg) warp_topn_bisect_impl<true>(key, NB, n, out);
-  else warp_topn_bisect_impl<false>(key, NB, n, out);
+  if (NB <= 32 * 36) warp_topn_bisect_impl<36>(key, NB, n, out);
+  else if (NB <= 32 * 72) warp_topn_bisect_impl<72>(key, NB, n, out);
+  else warp_topn_bisect_impl<0>(key, NB, n, out);
 }
 
 // One warp: per-frame top-k (PER_FRAME scope): in every frame's candidate range keep the kf best; ascending output.
