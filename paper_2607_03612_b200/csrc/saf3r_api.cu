@@ -339,12 +339,12 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
   // launch 1: pooling (one warp per token block of every tensor a rule reads) + one row_ptr CTA per head + the lists of the
   // constant-length closed-form heads
   const int pool_tasks = jobs.n * ((g.NB + 7) / 8);
-  // persistent pool CTAs, at most 4 per SM, and as many as give every CTA the SAME number of tasks (2.76 tasks per CTA would
-  // run as long as 3: launch tasks/3 CTAs instead)
+  // persistent pool CTAs, at most 4 per SM; with few rounds, as many as give every CTA the SAME number of tasks (2.76 tasks per
+  // CTA would run as long as 3: launch tasks/3 CTAs instead)
   int pool_ctas = pool_tasks;
   if (pool_tasks > 4 * ctx->sm_count) {
     const int per_cta = (pool_tasks + 4 * ctx->sm_count - 1) / (4 * ctx->sm_count);
-    pool_ctas = (pool_tasks + per_cta - 1) / per_cta;
+    pool_ctas = per_cta <= 4 ? (pool_tasks + per_cta - 1) / per_cta : 4 * ctx->sm_count;  // many rounds: keep every slot busy
   }
   const int light_chunks = (g.NB + kLightRows - 1) / kLightRows;
   if (ctx->stage_timing) cudaEventRecord(ctx->ev[0], st);
