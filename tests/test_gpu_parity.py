@@ -553,3 +553,30 @@ def test_c5_shape_three_heads(env):
         r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
         ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, r - r[0], col[r[0]:r[-1]], qb, want_lse=False)
         check_attention(out[h].cpu().numpy(), ref, f"C5-shape head {h} ({gens[h]})")
+
+
+@pytest.mark.parametrize("S,G,B,H", [(32, 3, 64, 1), (64, 3, 128, 2), (1, 3, 64, 1)])
+def test_no_tail_single_head_and_tiny_shapes(env, S, G, B, H):
+    """Degenerate shapes: N an exact multiple of the block (no partial tail: T = 14, N = 448 = 7*64 or 896 = 7*128), a single head
+    (the TMA head stride is irrelevant then), and one frame smaller than one block (N = 14)."""
+    sf, ctx, torch = env
+    gens = [sy.GEN_SAME_POSITION, sy.GEN_SINK][:H]
+    NB = (S * (G * G + 5) + B - 1) // B
+    cfgs = [sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=min(3, NB)),
+            sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=min(2, NB))][:H]
+    L = small_layer(S, G, H, B, gens, cfgs, seed=71)
+    sh = L.shape
+    q, k, v = upload(L)
+    shape = c_shape(sf, sh)
+    lists = ctx.select(q, k, shape, L.cfgs)
+    out = ctx.sparse_attn(q, k, v, shape, lists, out_fp32=True)
+    dense = ctx.dense_attn(q, k, v, shape, out_fp32=True)
+    torch.cuda.synchronize()
+    hls = oracle_lists(L)
+    stats = compare_lists(L, lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy(), hls)
+    assert stats["tie_floored"] == 0
+    for h, hl in enumerate(hls):
+        ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], B, hl.row_ptr, hl.col_idx)
+        check_attention(out[h].cpu().numpy(), ref, f"head {h}")
+        ref, _ = orc.attn_dense(L.q[h], L.k[h], L.v[h])
+        check_attention(dense[h].cpu().numpy(), ref, f"dense head {h}")
