@@ -140,7 +140,7 @@ static WsLayout ws_layout(const SelGeom &g) {
   size_t off = 0;
   w.qt = off; off = align256(off + (size_t)g.H * g.NB * 64 * sizeof(float));
   w.kt = off; off = align256(off + (size_t)g.H * kt_stride(g.NB) * 64 * sizeof(float));
-  w.qpart = off; off = align256(off + (size_t)g.H * ((g.NB + 7) / 8) * 64 * sizeof(float));
+  w.qpart = off; off = align256(off + (size_t)g.H * ((g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask) * 64 * sizeof(float));
   w.probe = off; off = align256(off + (size_t)g.H * g.NB * sizeof(int32_t));
   w.total = off;
   return w;
@@ -338,7 +338,7 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
     }
   // launch 1: pooling (one warp per token block of every tensor a rule reads) + one row_ptr CTA per head + the lists of the
   // constant-length closed-form heads
-  const int pool_tasks = jobs.n * ((g.NB + 7) / 8);
+  const int pool_tasks = jobs.n * ((g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask);
   // persistent pool CTAs, at most 4 per SM; with few rounds, as many as give every CTA the SAME number of tasks (2.76 tasks per
   // CTA would run as long as 3: launch tasks/3 CTAs instead)
   int pool_ctas = pool_tasks;

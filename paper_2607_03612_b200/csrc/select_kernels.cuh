@@ -333,6 +333,7 @@ struct HeadSets {
 //                            rows all have the same length, a block scan of the closed-form lengths otherwise.
 //   remaining CTAs          : the lists of the closed-form heads whose rows all have the same length (DENSE, UNIFORM_STRIDE,
 //                            STATIC/ANCHOR): 32 rows per CTA, written under the pooling's HBM time.
+constexpr int kPoolBlocksPerTask = 2;
 struct PoolJobs {
   int32_t n;                            // number of (tensor, head) jobs
   uint8_t head[2 * SAF3R_MAX_HEADS];
@@ -355,7 +356,7 @@ __device__ __forceinline__ uint4 ld_stream_16(const void *p) {
 // per-CTA token sums of the pool launch, p[J] = qbar . Ktilde_J / sqrt(D), top-n -> probe_list[h][0..n).
 __device__ inline void probe_head(const float *qpart, const float *kt, int32_t *probe_list, int32_t *head_lists, const SelGeom &g,
                                   int h, int n, uint32_t *key /* dynamic smem, NB */, float (*part)[64], float *qb) {
-  const int nparts = (g.NB + 7) / 8;
+  const int nparts = (g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask;
   {
     const int d = threadIdx.x & 63, grp = threadIdx.x >> 6;
     const float *base = qpart + (int64_t)h * nparts * 64 + d;
@@ -452,32 +453,31 @@ __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16
     if (h == g.H - 1 && threadIdx.x == 0) row_ptr[(int64_t)g.H * g.NB] = plan.head_base[g.H];
     return;
   }
-  // ------------------------------------------------------------------ pool: one warp per token block
-  // CTA c of a job covers blocks 8c .. 8c+7 (jobs are padded to a multiple of 8 blocks, so a CTA never straddles jobs)
-  // The pool CTAs are persistent: pool_ctas <= 4 per SM of them stride over the pool_tasks (job, 8 blocks) tasks, so that
-  // all of them end together instead of leaving a partial last wave.
-  __shared__ float qsum[8][64];
+  // ------------------------------------------------------------------ pool: four warps per token block, two blocks per task
+  // Task t of a job covers blocks 2t, 2t+1 (jobs are padded to a multiple of 2 blocks, so a task never straddles jobs); warp w
+  // takes quarter (w & 3) of block (w >> 2): B/4 token rows, one round of at most eight 16-byte loads per lane.  Small tasks
+  // keep the tail of the launch short (a warp that streams a whole 16 KB block alone needs four dependent DRAM round trips).
+  // The pool CTAs are persistent: pool_ctas <= 4 per SM of them stride over the pool_tasks tasks.
+  __shared__ float wsum[8][64];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int ctas_per_job = (g.NB + 7) / 8;
-  for (int task = blockIdx.x; task < pool_tasks; task += pool_ctas) {
-  const int job = task / ctas_per_job, cta_in_job = task % ctas_per_job;
-  const int J = cta_in_job * 8 + warp;
-  const int h = jobs.head[job], which = jobs.which[job];
-  const bool probe = jobs.probe[job] != 0;
-  const bool want_part = probe && which == 0;  // Q of a QUERY_PROBE head: also emit this CTA's token sum (for qbar)
-  const bool valid = J < g.NB;
+  const int tasks_per_job = (g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask;
   const int sub = lane & 7, rg = lane >> 3;
-  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  if (valid) {
+  const int rows_q = g.B / 4;  // token rows per warp
+  for (int task = blockIdx.x; task < pool_tasks; task += pool_ctas) {
+    const int job = task / tasks_per_job, task_in_job = task % tasks_per_job;
+    const int J = task_in_job * kPoolBlocksPerTask + (warp >> 2);
+    const int h = jobs.head[job], which = jobs.which[job];
+    const bool want_part = jobs.probe[job] != 0 && which == 0;  // Q of a QUERY_PROBE head: also emit the task's token sum (qbar)
     const bool cosine = jobs.cosine[job] != 0;
-    const int64_t t0 = (int64_t)J * g.B;
-    const int cnt = (int)i64min(g.B, g.N - t0);
-    const __nv_bfloat16 *src = (which ? k : q) + (int64_t)h * g.stride_head + t0 * g.stride_token + sub * 8;
-    for (int r0 = 0; r0 < g.B; r0 += 32) {  // 8 loads of 16 B in flight per lane (rows r0 + rg + 4i)
+    float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (J < g.NB) {
+      const int64_t t0 = (int64_t)J * g.B + (warp & 3) * rows_q;
+      const int cnt = (int)i64max(0, i64min(rows_q, g.N - t0));
+      const __nv_bfloat16 *src = (which ? k : q) + (int64_t)h * g.stride_head + t0 * g.stride_token + sub * 8;
       uint4 raw[8];
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
-        const int r = r0 + rg + 4 * i;
+        const int r = rg + 4 * i;
         raw[i] = make_uint4(0, 0, 0, 0);
         if (r < cnt) raw[i] = ld_stream_16(src + (int64_t)r * g.stride_token);
       }
@@ -504,41 +504,34 @@ __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16
 #pragma unroll
         for (int c = 0; c < 8; ++c) acc[c] = fmaf(v[c], inv, acc[c]);
       }
-    }
 #pragma unroll
-    for (int c = 0; c < 8; ++c) {
-      acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 8);
-      acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 16);
-    }
-    const float invc = 1.f / (float)cnt;
-    if (rg == 0) {
-      if (which == 0) {  // Qtilde row-major [H][NB][64]
-        float4 *dst = reinterpret_cast<float4 *>(qt + ((int64_t)h * g.NB + J) * 64 + sub * 8);
-        dst[0] = make_float4(acc[0] * invc, acc[1] * invc, acc[2] * invc, acc[3] * invc);
-        dst[1] = make_float4(acc[4] * invc, acc[5] * invc, acc[6] * invc, acc[7] * invc);
-      } else {  // Ktilde transposed [H][64][NBp]
-        const int64_t ld = kt_stride(g.NB);
-#pragma unroll
-        for (int c = 0; c < 8; ++c) kt[((int64_t)h * 64 + sub * 8 + c) * ld + J] = acc[c] * invc;
+      for (int c = 0; c < 8; ++c) {
+        acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 8);
+        acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 16);
       }
     }
-  }
-  if (!want_part) continue;  // CTA-uniform
-  if (rg == 0) {
+    if (rg == 0) {
 #pragma unroll
-    for (int c = 0; c < 8; ++c) qsum[warp][sub * 8 + c] = acc[c];  // zero for warps past the last block
-  }
-  __syncthreads();
-  if (warp == 0) {
-#pragma unroll
-    for (int d = lane; d < 64; d += 32) {
+      for (int c = 0; c < 8; ++c) wsum[warp][sub * 8 + c] = acc[c];  // zero for warps past the last block / token
+    }
+    __syncthreads();
+    if (threadIdx.x < 64 * kPoolBlocksPerTask) {  // block sums in a fixed order (quarters 0..3), mean, store
+      const int bb = threadIdx.x >> 6, d = threadIdx.x & 63;
+      const int Jb = task_in_job * kPoolBlocksPerTask + bb;
+      if (Jb < g.NB) {
+        const float sum = (wsum[4 * bb][d] + wsum[4 * bb + 1][d]) + (wsum[4 * bb + 2][d] + wsum[4 * bb + 3][d]);
+        const float mean = sum / (float)i64min(g.B, g.N - (int64_t)Jb * g.B);
+        if (which == 0) qt[((int64_t)h * g.NB + Jb) * 64 + d] = mean;                    // Qtilde row-major [H][NB][64]
+        else kt[((int64_t)h * 64 + d) * kt_stride(g.NB) + Jb] = mean;                   // Ktilde transposed [H][64][NBp]
+      }
+    } else if (want_part && threadIdx.x >= 192) {  // the task's token sum, for qbar
+      const int d = threadIdx.x - 192;
       float t = 0.f;
 #pragma unroll
-      for (int w = 0; w < 8; ++w) t += qsum[w][d];
-      qpart[((int64_t)h * ctas_per_job + cta_in_job) * 64 + d] = t;
+      for (int w = 0; w < 8; ++w) t += wsum[w][d];
+      qpart[((int64_t)h * tasks_per_job + task_in_job) * 64 + d] = t;
     }
-  }
-  __syncthreads();  // qsum is reused by this CTA's next task
+    __syncthreads();  // wsum is reused by this CTA's next task
   }
 }
 
