@@ -294,6 +294,8 @@ def run_ours(args):
         pool_ms, ssel_ms = [], []
         for i in range(2 * n_res):
             d = dl[i % n_res]
+            torch.cuda._sleep(1_000_000)   # ~0.5 ms of GPU spin first, so that the host has queued the whole call before
+                                           # its first kernel can start (otherwise the stage times include host submission)
             ctx.select(d["q"], d["k"], shape, d["cfgs"], workspace=d["ws"], lists=d["lists"])
             a, b = ctx.last_select_stage_ms()
             if i >= n_res:
