@@ -358,10 +358,11 @@ def run_ours(args):
                              "steps": e_steps, "api": "saf3r_layer_host (pinned host q/k/v -> device, select + sparse_attn, out -> host; pipelined over 8 head groups)"}
 
         if world == 1 and not args.skip_cpu:
-            ms, sel, cores = cpu_oracle_layer_ms(layers[0], 1)
+            nq_cpu = 4 if args.config in ("c2", "c3") else 1
+            ms, sel, cores = cpu_oracle_layer_ms(layers[0], nq_cpu)
             result["cpu_baseline"] = {"value": ms, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                      "sample": f"layer 0: full select of all {sh.H} heads ({sel:.0f} ms) + attention on 1 sampled "
-                                                f"q-block/head scaled by NB={sh.NB} (extrapolated)"}
+                                      "sample": f"layer 0: full select of all {sh.H} heads ({sel:.0f} ms) + attention on {nq_cpu} sampled "
+                                                f"q-block(s)/head scaled by NB={sh.NB}/{nq_cpu} (extrapolated)"}
         print(json.dumps(result))
     if world > 1:
         dist.destroy_process_group()
