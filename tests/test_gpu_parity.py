@@ -580,3 +580,26 @@ def test_no_tail_single_head_and_tiny_shapes(env, S, G, B, H):
         check_attention(out[h].cpu().numpy(), ref, f"head {h}")
         ref, _ = orc.attn_dense(L.q[h], L.k[h], L.v[h])
         check_attention(dense[h].cpu().numpy(), ref, f"dense head {h}")
+
+
+def test_select_sixteen_block_heads(env):
+    """Sixteen BLOCK_TOPK heads at the C2 shape: enough score strips for 16-row score CTAs (dot and cosine, global and
+    per-frame).  Lists against the oracle under the near-tie rule; the count is printed."""
+    sf, ctx, torch = env
+    sh = sy.shape_c2()
+    gens = [sy.GEN_SAME_POSITION] * 8 + [sy.GEN_UNIFORM] * 4 + [sy.GEN_SINK] * 4
+    cfgs = []
+    for h in range(16):
+        if h % 4 == 3:
+            cfgs.append(sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=1 + h % 3, score_mode=h % 2))
+        else:
+            cfgs.append(sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=10 + 7 * h, score_mode=(h // 2) % 2))
+    L = sy.make_layer(sh, gens, cfgs, seed=81)
+    q, k, _ = upload(L)
+    shape = c_shape(sf, sh)
+    lists = ctx.select(q, k, shape, L.cfgs)
+    torch.cuda.synchronize()
+    assert ctx.check_lists(shape, lists) == 0
+    stats = compare_lists(L, lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy(), oracle_lists(L))
+    print("16 block heads near-ties:", stats)
+    assert stats["tie_floored"] <= 1e-3 * stats["entries"]
