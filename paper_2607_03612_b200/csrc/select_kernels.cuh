@@ -559,7 +559,7 @@ __device__ __forceinline__ uint64_t sel_fma2(uint64_t a, uint64_t b, uint64_t c)
 // Score rows I0 .. I0+rows-1 (rows <= RT) of head h against every k-block: keys[r][J] = key(Qtilde_{I0+r} . Ktilde_J * cs).
 // Groups of 1024 columns: each thread owns four consecutive columns (one 16-byte load of Ktilde^T per d, coalesced across
 // the warp) and RT rows, 4*RT accumulators as packed row pairs.  The columns left over (< 1024) are spread over all threads
-// as (row, four columns) tasks.  Every sum runs in the order d = 0..63 with fp32 FMAs, so both paths give the same bits.
+// as (four rows, four columns) tasks.  Every sum runs in the order d = 0..63 with fp32 FMAs, so both paths give the same bits.
 template <int RT>
 __device__ __forceinline__ void score_rows(const float *__restrict__ qt, const float *__restrict__ kt, uint32_t *keys, float *qT,
                                            const SelGeom &g, int h, int I0, int rows, float cs) {
@@ -611,24 +611,40 @@ __device__ __forceinline__ void score_rows(const float *__restrict__ qt, const f
             make_uint4(score_key(hi[0] * cs), score_key(hi[1] * cs), score_key(hi[2] * cs), score_key(hi[3] * cs));
     }
   }
-  // left-over columns: (row, column quad) tasks; the padded columns NB..NBp-1 of Ktilde^T are never written, so their
+  // left-over columns: (four rows, column quad) tasks; the padded columns NB..NBp-1 of Ktilde^T are never written, so their
   // scores are computed from garbage and stored into the row's padding, which nothing reads
   const int quads = (int)((ld - Jb) / 4);
-  for (int idx = threadIdx.x; idx < quads * rows; idx += blockDim.x) {
-    const int r = idx / quads, J = Jb + 4 * (idx % quads);
+  constexpr int RG = RT / 4;  // row groups of four
+  for (int idx = threadIdx.x; idx < quads * RG; idx += blockDim.x) {
+    const int rgp = idx / quads, J = Jb + 4 * (idx % quads);
     const float *kp = kh + J;
-    float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+    uint64_t a[4][2];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) a[c][0] = a[c][1] = 0ull;
 #pragma unroll 8
     for (int d = 0; d < 64; ++d) {
       const float4 kv = __ldg(reinterpret_cast<const float4 *>(kp + (int64_t)d * ld));
-      const float qv = qT[d * RT + r];
-      a0 = fmaf(qv, kv.x, a0);
-      a1 = fmaf(qv, kv.y, a1);
-      a2 = fmaf(qv, kv.z, a2);
-      a3 = fmaf(qv, kv.w, a3);
+      const float4 t = *reinterpret_cast<const float4 *>(qT + d * RT + 4 * rgp);
+      const uint64_t qa = sel_pack2(t.x, t.y), qb = sel_pack2(t.z, t.w);
+      const uint64_t k0 = sel_pack2(kv.x, kv.x), k1 = sel_pack2(kv.y, kv.y), k2 = sel_pack2(kv.z, kv.z), k3 = sel_pack2(kv.w, kv.w);
+      a[0][0] = sel_fma2(qa, k0, a[0][0]); a[0][1] = sel_fma2(qb, k0, a[0][1]);
+      a[1][0] = sel_fma2(qa, k1, a[1][0]); a[1][1] = sel_fma2(qb, k1, a[1][1]);
+      a[2][0] = sel_fma2(qa, k2, a[2][0]); a[2][1] = sel_fma2(qb, k2, a[2][1]);
+      a[3][0] = sel_fma2(qa, k3, a[3][0]); a[3][1] = sel_fma2(qb, k3, a[3][1]);
     }
-    *reinterpret_cast<uint4 *>(keys + (size_t)r * ld + J) =
-        make_uint4(score_key(a0 * cs), score_key(a1 * cs), score_key(a2 * cs), score_key(a3 * cs));
+#pragma unroll
+    for (int r2 = 0; r2 < 2; ++r2) {
+      float lo[4], hi[4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) asm("mov.b64 {%0, %1}, %2;" : "=f"(lo[c]), "=f"(hi[c]) : "l"(a[c][r2]));
+      const int r = 4 * rgp + 2 * r2;
+      if (r < rows)
+        *reinterpret_cast<uint4 *>(keys + (size_t)r * ld + J) =
+            make_uint4(score_key(lo[0] * cs), score_key(lo[1] * cs), score_key(lo[2] * cs), score_key(lo[3] * cs));
+      if (r + 1 < rows)
+        *reinterpret_cast<uint4 *>(keys + (size_t)(r + 1) * ld + J) =
+            make_uint4(score_key(hi[0] * cs), score_key(hi[1] * cs), score_key(hi[2] * cs), score_key(hi[3] * cs));
+    }
   }
 }
 
