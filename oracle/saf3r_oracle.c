@@ -16,8 +16,8 @@
  *
  * Citations are PAPER.md line numbers and DESIGN.md readings.
  *
- * Parity pins: every function below is pinned by tests/test_oracle_pins.py (P1..P13 of
- * DESIGN.md).  Unpinned *choices* (not arithmetic): POSITION_BAND radius and the
+ * Parity pins: every function below is pinned by tests/test_oracle_pins.py (P1..P16 of
+ * DESIGN.md; P14-P16 pin the token-granular functions orc_attn_tokens / orc_token_probe).  Unpinned *choices* (not arithmetic): POSITION_BAND radius and the
  * DOT-vs-COSINE default for correspondence heads -- "parity unpinned" for those choices.
  */
 #include <math.h>
