@@ -579,23 +579,30 @@ __device__ __forceinline__ void score_rows(const float *__restrict__ qt, const f
 #pragma unroll
       for (int r = 0; r < RT / 2; ++r) a[c][r] = 0ull;
     const float *kp = kh + J;
-#pragma unroll 4
-    for (int d = 0; d < 64; ++d) {
-      const float4 kv = __ldg(reinterpret_cast<const float4 *>(kp + (int64_t)d * ld));
-      const uint64_t k0 = sel_pack2(kv.x, kv.x), k1 = sel_pack2(kv.y, kv.y), k2 = sel_pack2(kv.z, kv.z), k3 = sel_pack2(kv.w, kv.w);
-      const float4 *qr = reinterpret_cast<const float4 *>(qT + d * RT);
+    constexpr int KB = RT <= 4 ? 16 : (RT <= 8 ? 8 : 4);  // 16-byte loads in flight per thread (short strips have the registers)
+#pragma unroll 1
+    for (int d0 = 0; d0 < 64; d0 += KB) {
+      float4 kvb[KB];
 #pragma unroll
-      for (int r4 = 0; r4 < RT / 4; ++r4) {
-        const float4 t = qr[r4];
-        const uint64_t qa = sel_pack2(t.x, t.y), qb = sel_pack2(t.z, t.w);
-        a[0][2 * r4] = sel_fma2(qa, k0, a[0][2 * r4]);
-        a[0][2 * r4 + 1] = sel_fma2(qb, k0, a[0][2 * r4 + 1]);
-        a[1][2 * r4] = sel_fma2(qa, k1, a[1][2 * r4]);
-        a[1][2 * r4 + 1] = sel_fma2(qb, k1, a[1][2 * r4 + 1]);
-        a[2][2 * r4] = sel_fma2(qa, k2, a[2][2 * r4]);
-        a[2][2 * r4 + 1] = sel_fma2(qb, k2, a[2][2 * r4 + 1]);
-        a[3][2 * r4] = sel_fma2(qa, k3, a[3][2 * r4]);
-        a[3][2 * r4 + 1] = sel_fma2(qb, k3, a[3][2 * r4 + 1]);
+      for (int i = 0; i < KB; ++i) kvb[i] = __ldg(reinterpret_cast<const float4 *>(kp + (int64_t)(d0 + i) * ld));
+#pragma unroll
+      for (int i = 0; i < KB; ++i) {
+        const float4 kv = kvb[i];
+        const uint64_t k0 = sel_pack2(kv.x, kv.x), k1 = sel_pack2(kv.y, kv.y), k2 = sel_pack2(kv.z, kv.z), k3 = sel_pack2(kv.w, kv.w);
+        const float4 *qr = reinterpret_cast<const float4 *>(qT + (d0 + i) * RT);
+#pragma unroll
+        for (int r4 = 0; r4 < RT / 4; ++r4) {
+          const float4 t = qr[r4];
+          const uint64_t qa = sel_pack2(t.x, t.y), qb = sel_pack2(t.z, t.w);
+          a[0][2 * r4] = sel_fma2(qa, k0, a[0][2 * r4]);
+          a[0][2 * r4 + 1] = sel_fma2(qb, k0, a[0][2 * r4 + 1]);
+          a[1][2 * r4] = sel_fma2(qa, k1, a[1][2 * r4]);
+          a[1][2 * r4 + 1] = sel_fma2(qb, k1, a[1][2 * r4 + 1]);
+          a[2][2 * r4] = sel_fma2(qa, k2, a[2][2 * r4]);
+          a[2][2 * r4 + 1] = sel_fma2(qb, k2, a[2][2 * r4 + 1]);
+          a[3][2 * r4] = sel_fma2(qa, k3, a[3][2 * r4]);
+          a[3][2 * r4 + 1] = sel_fma2(qb, k3, a[3][2 * r4 + 1]);
+        }
       }
     }
 #pragma unroll
