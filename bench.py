@@ -324,9 +324,13 @@ def run_ours(args):
             # quality of the sparse layer against the library's own dense output (Eq. 1 of the paper; reported,
             # not a gate): NMSE per head of layer 0, summarised by head generator.  d["out"] holds the dense output now.
             sp = torch.empty_like(d["out"])
+            _, lse_d = ctx.dense_attn(d["q"], d["k"], d["v"], shape, out=d["out"], want_lse=True)
             ctx.select(d["q"], d["k"], shape, d["cfgs"], workspace=d["ws"], lists=d["lists"])
-            ctx.sparse_attn(d["q"], d["k"], d["v"], shape, d["lists"], out=sp)
+            _, lse_s = ctx.sparse_attn(d["q"], d["k"], d["v"], shape, d["lists"], out=sp, want_lse=True)
             torch.cuda.synchronize()
+            # attention-mass recall ("coverage of the full attention distribution"): the dense softmax
+            # mass that falls on the kept keys = exp(lse_sparse - lse_dense), averaged over the queries of a head
+            recall = torch.exp(lse_s - lse_d).mean(dim=1).cpu().tolist()
             nm = []
             for h in range(sh.H):                                 # per head, to bound the fp32 temporaries
                 a, b = d["out"][h].float(), sp[h].float()
@@ -334,7 +338,11 @@ def run_ours(args):
             by = {}
             for h, gname in enumerate(layers[0].gens):
                 by.setdefault(gname, []).append(nm[h])
+            rec = {}
+            for h, gname in enumerate(layers[0].gens):
+                rec.setdefault(gname, []).append(recall[h])
             result["quality_vs_own_dense"] = {"nmse_by_generator": {k2: float(np.mean(v2)) for k2, v2 in by.items()},
+                                              "mass_recall_by_generator": {k2: float(np.mean(v2)) for k2, v2 in rec.items()},
                                               "nmse_max": float(max(nm)), "note": "layer 0; Eq. 1 (PAPER.md:L108) with O_full = dense mode, bf16 outputs"}
             del sp
 
