@@ -19,6 +19,8 @@
  *   - Asynchrony: select / *_attn enqueue work on `cuda_stream` (a cudaStream_t passed as void*) and return.
  *     Argument errors are returned synchronously before anything is enqueued.
  *   - Errors: every call returns a saf3r_status; text via saf3r_last_error(ctx).  SAF3R_ERR_CUDA is sticky.
+ *   - A context is not thread-safe: use one context per host thread (or serialise calls).  Calls on one context may target
+ *     different streams one after another; saf3r_layer_host additionally uses context-owned side streams.
  *   - There is no CPU fallback: on a machine without an sm_100 device saf3r_create fails with SAF3R_ERR_UNSUPPORTED.
  */
 #ifndef SAF3R_H_
