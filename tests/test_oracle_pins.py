@@ -280,6 +280,36 @@ def test_p8_static_closed_forms():
         assert list(hl.col_idx[hl.row_ptr[i]:hl.row_ptr[i + 1]]) == exp
 
 
+@pytest.mark.parametrize("S,T,B", [(4, 23, 8), (5, 261, 64), (3, 1374, 128), (6, 10, 16), (4, 24, 8), (5, 12, 8)])
+def test_p8_position_band_and_anchor_per_token_at_block_granularity(S, T, B):
+    """P8 at B > 1, derived per TOKEN ("fixed across all image blocks", L96; readings A5/A6/A12): q-blocks straddle
+    frames here, so a row can hold two position intervals, each clipped to [0, T-1] in its own frame.  The expected block set of
+    q-block I is built token by token -- every token t of I reaches the positions p(t)-r .. p(t)+r (clipped) of EVERY frame g --
+    and only then lifted to blocks; nothing of the oracle's interval arithmetic is restated.  (B=16 > T=10: whole frames inside
+    one q-block; T=24, B=8: frame
+    boundaries coincide with block boundaries, where clipping at T instead of T-1 would leak into the next frame's first block.)"""
+    rng = np.random.default_rng(19)
+    N, D = S * T, 8
+    NB = (N + B - 1) // B
+    q = k = rand_bits(rng, (N, D))
+    for r in (0, 3, T // 2):
+        hl = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_POSITION_BAND, band_radius=r)))
+        for I in range(NB):
+            expect = set()
+            for t in range(I * B, min(N, (I + 1) * B)):
+                p = t % T
+                for pp in range(max(0, p - r), min(T - 1, p + r) + 1):
+                    expect.update((g * T + pp) // B for g in range(S))
+            row = hl.col_idx[hl.row_ptr[I]:hl.row_ptr[I + 1]]
+            assert np.all(np.diff(row) > 0)
+            assert set(row.tolist()) == expect, f"POSITION_BAND S={S} T={T} B={B} r={r} row {I}"
+    for a in range(S):                                            # ANCHOR: the blocks that hold a token of frame a, from the token list
+        hl = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_ANCHOR, anchor_frame=a)))
+        expect = sorted({t // B for t in range(N) if t // T == a})
+        for I in range(NB):
+            assert hl.col_idx[hl.row_ptr[I]:hl.row_ptr[I + 1]].tolist() == expect, f"ANCHOR a={a} row {I}"
+
+
 # ---------------------------------------------------------------- P9
 def test_p9_softmax_special_cases():
     rng = np.random.default_rng(10)
