@@ -118,31 +118,63 @@ class ClockSampler:
                 "samples": len(sm), "power_w_max": max(pw) if pw else None, "source": "nvml" if self.nvml is not None else "nvidia-smi"}
 
 
-def cpu_oracle_layer_ms(L: sy.Layer, qblocks_per_head: int, one_per_type: bool = False):
-    """The oracle as it stands on the host cores: selection of every head + attention on a bounded sample of q-blocks per
-    head, extrapolated to the layer (attention time scaled by NB / sampled).  one_per_type: time one head of each head
-    type and scale by the number of heads of that type (keeps a reference step to a few seconds)."""
+def cpu_sample_qblocks() -> int:
+    """q-blocks sampled per head by the CPU-oracle legs: the oracle parallelises its attention over q-blocks (OpenMP, one
+    q-block per thread at a time), so at least 2 per host core are needed to keep every core busy (>= 32)."""
+    return max(32, 2 * (os.cpu_count() or 1))
+
+
+def cpu_oracle_layer_ms(L: sy.Layer, nq: int | None = None):
+    """The oracle as it stands on ALL host cores, on a bounded sample of the layer, extrapolated to the whole layer.  The one
+    sampler both arms use (the GPU arm's cpu_baseline leg and --impl reference), so that their numbers agree:
+      - one head of each head generator is run (the first of its kind): its full selection (timed, scaled by the number of heads
+        of that kind) and its attention on `nq` sampled q-blocks (all cores busy: nq >= 2 x cores);
+      - the attention time is scaled by listed (q-block, k-block) pairs: (pairs of ALL heads of that kind) / (pairs of the sampled
+        q-blocks), since the oracle's attention time is proportional to the number of listed pairs.
+    Returns (layer ms, select ms, cores, threads_busy, sample description)."""
     import oracle as orc
     sh = L.shape
+    nq = min(sh.NB, nq or cpu_sample_qblocks())
     rng = np.random.default_rng(0)
-    heads, weight = list(range(sh.H)), [1.0] * sh.H
-    if one_per_type:
-        first = {}
-        for h, g in enumerate(L.gens):
-            first.setdefault(g, h)
-        heads = sorted(first.values())
-        weight = [float(sum(1 for g in L.gens if g == L.gens[h])) for h in heads]
+    first = {}
+    for h, g in enumerate(L.gens):
+        first.setdefault(g, h)
     t_sel = t_att = 0.0
-    for h, w in zip(heads, weight):
+    for g, h in sorted(first.items(), key=lambda kv: kv[1]):
+        same = [i for i, gg in enumerate(L.gens) if gg == g]
         t0 = time.perf_counter()
         hl = orc.select_head(L.q[h], L.k[h], sh.S, sh.T, sh.B, orc.make_cfg(**L.cfgs[h]))
         t1 = time.perf_counter()
-        qb = np.sort(rng.choice(sh.NB, qblocks_per_head, replace=False)).astype(np.int64)
+        qb = np.sort(rng.choice(sh.NB, nq, replace=False)).astype(np.int64)
         orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, hl.row_ptr, hl.col_idx, qb, want_lse=False)
         t2 = time.perf_counter()
-        t_sel += w * (t1 - t0)
-        t_att += w * (t2 - t1) * sh.NB / qblocks_per_head
-    return (t_sel + t_att) * 1e3, t_sel * 1e3, orc.num_threads()
+        pairs_sampled = int(np.sum(hl.row_ptr[qb + 1] - hl.row_ptr[qb]))
+        pairs_kind = 0
+        for i in same:                                           # list lengths are closed forms of (shape, cfg): no data needed
+            c = L.cfgs[i]
+            if c == L.cfgs[h]:
+                pairs_kind += int(hl.row_ptr[-1])
+            else:
+                pairs_kind += closed_form_pairs(sh, c, hl, L.cfgs[h])
+        t_sel += len(same) * (t1 - t0)
+        t_att += (t2 - t1) * pairs_kind / max(1, pairs_sampled)
+    cores = orc.num_threads()
+    sample = (f"one head per head generator ({len(first)} of {sh.H} heads): full select (scaled by heads of that kind) + attention on "
+              f"{nq} sampled q-blocks of that head, scaled by listed block pairs of all heads of that kind / pairs sampled "
+              f"(extrapolated to the layer)")
+    return (t_sel + t_att) * 1e3, t_sel * 1e3, cores, min(cores, nq), sample
+
+
+def closed_form_pairs(sh: sy.Shape, c: dict, hl_ref, c_ref: dict) -> int:
+    """Listed pairs of a head with configuration c, given the oracle lists hl_ref of a head of the same kind with c_ref: list
+    lengths depend only on (shape, cfg).  Top-n / stride-n heads: NB x n; per-row closed forms (frame-local): same as the reference."""
+    if c["type"] in (sy.HEAD_QUERY_PROBE_TOPK, sy.HEAD_BLOCK_TOPK) and c.get("topk_scope", 0) == sy.SCOPE_GLOBAL:
+        return sh.NB * min(sh.NB, c["keep_blocks"])
+    if c["type"] == sy.HEAD_UNIFORM_STRIDE:
+        n = c["keep_blocks"] if c["stride"] == 0 else -(-(sh.NB - c["offset"]) // c["stride"])
+        return sh.NB * n
+    assert c == c_ref, "per-row closed forms: heads of one kind share one configuration in the bench recipes"
+    return int(hl_ref.row_ptr[-1])
 
 
 def run_reference(args):
@@ -150,22 +182,19 @@ def run_reference(args):
     if rank != 0:
         return
     sh = shape_for(args.config)
-    nq = 1 if args.config != "c2" else 2
     layers = make_layers(args.config, 1)
     times = []
     for i in range(args.warmup + args.steps):
-        ms, _, cores = cpu_oracle_layer_ms(layers[0], nq, one_per_type=True)
+        ms, _, cores, busy, sample = cpu_oracle_layer_ms(layers[0])
         if i >= args.warmup:
             times.append(ms)
     v = float(np.mean(times))
-    sample = (f"per step: select + attention on {nq} sampled q-block(s) for one head of each head type, scaled by heads per type and "
-              f"by NB/{nq} (extrapolated to the layer)")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(args.config, sh), "note": "CPU oracle (oracle/), not tuned"},
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "threads_busy": busy, "kind": "oracle", "sample": "per step: " + sample},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
@@ -274,13 +303,20 @@ def run_ours(args):
     if rank == 0:
         result["clocks"] = clk.summary()
         # roofline of the dominant kernel (block-sparse attention): executed FLOP per launch / mean launch duration
-        traffic = None
+        traffic, traffic_note = None, "no ncu capture recorded (profiles/traffic.json)"
         tp = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tp):
-            traffic = json.load(open(tp)).get("saf3r_attn_kernel_bytes_per_launch")
+            tj = json.load(open(tp))
+            import hashlib
+            sha = hashlib.sha256(open(os.path.join(ROOT, "paper_2607_03612_b200", "csrc", "attn_kernel.cuh"), "rb").read()).hexdigest()[:16]
+            if tj.get("attn_kernel_sha16") == sha:               # the capture belongs to the kernel source that is running
+                traffic = tj.get("saf3r_attn_kernel_bytes_per_launch")
+                traffic_note = "ncu dram bytes read + written of the layer-0 launch (profiles/traffic.json, same attn_kernel.cuh); achieved is the mean over the resident layers"
+            else:
+                traffic_note = f"profiles/traffic.json was captured for another build of attn_kernel.cuh ({tj.get('attn_kernel_sha16')} != {sha}): dropped"
         result["roofline"] = {"bound": "tensor", "achieved": exec_tflops, "peak": peaks["tflops_sustained"], "unit": "TFLOP/s",
                               "frac": exec_tflops / peaks["tflops_sustained"], "traffic": traffic,
-                              "traffic_note": "ncu dram bytes of the layer-0 launch (profiles/traffic.json); achieved is the mean over the resident layers",
+                              "traffic_note": traffic_note,
                               "kernel": "saf3r_attn_kernel", "peak_source": f"{peaks['source']} sustained bf16 (kernel timed inside a long step)",
                               "frac_of_burst": exec_tflops / peaks["tflops_burst"]}
         # selection pass against HBM: algorithmic bytes = Q and/or K of the heads whose rule reads them
@@ -366,11 +402,10 @@ def run_ours(args):
                              "steps": e_steps, "api": "saf3r_layer_host (pinned host q/k/v -> device, select + sparse_attn, out -> host; pipelined over 8 head groups)"}
 
         if world == 1 and not args.skip_cpu:
-            nq_cpu = 4 if args.config in ("c2", "c3") else 1
-            ms, sel, cores = cpu_oracle_layer_ms(layers[0], nq_cpu)
-            result["cpu_baseline"] = {"value": ms, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                      "sample": f"layer 0: full select of all {sh.H} heads ({sel:.0f} ms) + attention on {nq_cpu} sampled "
-                                                f"q-block(s)/head scaled by NB={sh.NB}/{nq_cpu} (extrapolated)"}
+            ms, sel, cores, busy, sample = cpu_oracle_layer_ms(layers[0])
+            result["cpu_baseline"] = {"value": ms, "unit": UNIT, "cores": cores, "threads_busy": busy, "kind": "oracle",
+                                      "sample": "layer 0: " + sample, "select_ms": sel}
+            result["vs_cpu_oracle"] = {"ratio": ms / ms_per_step, "note": "extrapolated, untuned CPU oracle / this run; reported, not a target"}
         print(json.dumps(result))
     if world > 1:
         dist.destroy_process_group()

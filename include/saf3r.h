@@ -155,6 +155,13 @@ saf3r_status saf3r_layer_host(saf3r_ctx *ctx, const void *q_host, const void *k_
                               const saf3r_shape *shape, const saf3r_head_cfg *cfg_host, void *scratch_dev,
                               size_t scratch_bytes, void *out_host, void *cuda_stream);
 
+/* Launch plan of saf3r_select for (shape, cfg) on this context's device (host only; a testing aid): *strip_rows = q-block rows
+ * scored per CTA of the score + select kernel (0 when no head is BLOCK_TOPK), *smem_bytes = its dynamic shared memory.  A closed
+ * form of (shape, cfg, SM count); SAF3R_ERR_UNSUPPORTED when NB is too large for the kernel (the same answer saf3r_select gives,
+ * before it enqueues anything).  Either output pointer may be NULL. */
+saf3r_status saf3r_select_plan(const saf3r_ctx *ctx, const saf3r_shape *shape, const saf3r_head_cfg *cfg_host, int32_t *strip_rows,
+                               size_t *smem_bytes);
+
 /* Number of kernels the library has launched on this context since creation (for bench.py's gpu_launches). */
 int64_t saf3r_launch_count(const saf3r_ctx *ctx);
 
@@ -166,7 +173,7 @@ int64_t saf3r_launch_count(const saf3r_ctx *ctx);
  *   V are read through a strided TMA view.  stride >= 1, 0 <= offset < min(stride, N).  One launch.
  * saf3r_token_probe_select: Query-Probe Top-K at token level: qbar = (1/N) sum_i q_i,
  *   p[j] = qbar . k_j / sqrt(D) for every key token j, the K tokens with the largest p (score desc, index asc) written
- *   ascending to idx_dev[h][0..K) (int32, [H][K]).  1 <= K <= N, the same K for every head of the call.  Four launches.
+ *   ascending to idx_dev[h][0..K) (int32, [H][K]).  1 <= K <= N, the same K for every head of the call.  Three launches.
  * saf3r_token_set_attn: every query of head h attends the key tokens idx_dev[h][0..K) (ascending, unique, < N; the output of
  *   saf3r_token_probe_select or any caller-made set): gathers those K/V rows into the workspace and runs the dense mode over
  *   them.  Two launches.
@@ -186,8 +193,9 @@ saf3r_status saf3r_token_set_attn(saf3r_ctx *ctx, const void *q_dev, const void 
 /* Measurement aid ("select ms split into pool and score+select stages").  When enabled, saf3r_select records
  * CUDA events on its stream before the pool launch, between the two launches and after the select launch (three
  * cudaEventRecord calls, no synchronisation).  saf3r_last_select_stage_ms blocks until the last timed saf3r_select has
- * finished and returns the two stage durations in milliseconds: pool_ms = pooling (+ row_ptr, + the probe of QUERY_PROBE
- * heads, which runs inside the pool launch), select_ms = score + select + list emission. */
+ * finished and returns the two stage durations in milliseconds: pool_ms = the first launch (pooling, row_ptr, the lists of the
+ * constant-length closed-form heads), select_ms = the second launch (the probe of QUERY_PROBE heads, block scores, top-n, every
+ * other list). */
 saf3r_status saf3r_set_stage_timing(saf3r_ctx *ctx, int enable);
 saf3r_status saf3r_last_select_stage_ms(saf3r_ctx *ctx, float *pool_ms, float *select_ms);
 

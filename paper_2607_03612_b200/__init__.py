@@ -13,7 +13,7 @@ import os
 from dataclasses import dataclass
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("SAF3R_LIB", os.path.join(HERE, "libsaf3r.so"))  # env override: kernel-variant experiments only
+LIB_PATH = os.path.join(HERE, "libsaf3r.so")
 
 MAX_HEADS = 64
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CAPACITY, ERR_CUDA = range(5)
@@ -27,7 +27,7 @@ SCORE_DOT, SCORE_COSINE = range(2)
 EXPORTS = ("saf3r_create", "saf3r_destroy", "saf3r_last_error", "saf3r_query_sizes", "saf3r_select", "saf3r_sparse_attn",
            "saf3r_dense_attn", "saf3r_layer_host_scratch_bytes", "saf3r_layer_host", "saf3r_launch_count",
            "saf3r_set_stage_timing", "saf3r_last_select_stage_ms", "saf3r_select_cached", "saf3r_token_stride_attn",
-           "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn", "saf3r_check_lists")
+           "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn", "saf3r_check_lists", "saf3r_select_plan")
 
 
 class Saf3rError(RuntimeError):
@@ -81,6 +81,7 @@ def load_library():
         L.saf3r_dense_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), vp, i32, vp, vp]
         L.saf3r_layer_host_scratch_bytes.argtypes = [C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(C.c_size_t)]
         L.saf3r_layer_host.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), vp, C.c_size_t, vp, vp]
+        L.saf3r_select_plan.argtypes = [vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(C.c_int32), C.POINTER(C.c_size_t)]
         L.saf3r_launch_count.argtypes = [vp]
         L.saf3r_launch_count.restype = i64
         L.saf3r_set_stage_timing.argtypes = [vp, i32]
@@ -120,6 +121,15 @@ def _stream_ptr(stream=None):
     import torch
     s = torch.cuda.current_stream() if stream is None else stream
     return C.c_void_p(s.cuda_stream)
+
+
+def _on_stream(stream, *tensors):
+    """Tensors this binding allocated itself and that kernels enqueued on `stream` touch: tell the caching allocator, so that a
+    block dropped by the caller is not handed to another stream's allocation while those kernels still run."""
+    if stream is not None:
+        for t in tensors:
+            if t is not None:
+                t.record_stream(stream)
 
 
 class Context:
@@ -164,9 +174,16 @@ class Context:
         self._check(self.lib.saf3r_last_select_stage_ms(self.h, C.byref(a), C.byref(b)))
         return float(a.value), float(b.value)
 
-    # ---- saf3r_query_sizes
+    # ---- saf3r_query_sizes / saf3r_select_plan
     def query_sizes(self, shape: ShapeC, cfgs) -> tuple[int, int]:
         return query_sizes(shape, cfgs)
+
+    def select_plan(self, shape: ShapeC, cfgs) -> tuple[int, int]:
+        """(rows per score strip, dynamic shared-memory bytes) of the score + select launch for (shape, cfgs)."""
+        arr = make_cfgs(cfgs)
+        r, b = C.c_int32(), C.c_size_t()
+        self._check(self.lib.saf3r_select_plan(self.h, C.byref(shape), arr, C.byref(r), C.byref(b)))
+        return int(r.value), int(b.value)
 
     # ---- saf3r_select / saf3r_select_cached
     def select(self, q, k, shape: ShapeC, cfgs, workspace=None, lists: Lists | None = None, stream=None,
@@ -179,11 +196,13 @@ class Context:
         dev = q.device
         if workspace is None:
             workspace = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+            _on_stream(stream, workspace)
         if lists is None:
             N = shape.num_frames * shape.tokens_per_frame
             NB = (N + shape.block - 1) // shape.block
             lists = Lists(torch.empty(shape.num_heads * NB + 1, dtype=torch.int64, device=dev),
                           torch.empty(max(entries, 1), dtype=torch.int32, device=dev))
+            _on_stream(stream, lists.row_ptr, lists.col_idx)
         lc = lists.c()
         if cache is not None:
             cc = cache.c()
@@ -211,10 +230,7 @@ class Context:
 
     def _attn(self, q, k, v, shape, lists, out, out_fp32, want_lse, stream):
         import torch
-        if out is None:
-            out = torch.empty(q.shape, dtype=torch.float32 if out_fp32 else torch.bfloat16, device=q.device)
-        N = shape.num_frames * shape.tokens_per_frame
-        lse = torch.empty((shape.num_heads, N), dtype=torch.float32, device=q.device) if want_lse else None
+        out, lse = self._out_lse(q, shape, out, out_fp32, want_lse, stream)
         lp = lse.data_ptr() if lse is not None else None
         if lists is not None:
             lc = lists.c()
@@ -227,17 +243,19 @@ class Context:
         return (out, lse) if want_lse else out
 
     # ---- token-granular variants: saf3r_token_stride_attn / saf3r_token_probe_select / saf3r_token_set_attn
-    def _out_lse(self, q, shape, out, out_fp32, want_lse):
+    def _out_lse(self, q, shape, out, out_fp32, want_lse, stream=None):
         import torch
         if out is None:
             out = torch.empty(q.shape, dtype=torch.float32 if out_fp32 else torch.bfloat16, device=q.device)
+            _on_stream(stream, out)
         N = shape.num_frames * shape.tokens_per_frame
         lse = torch.empty((shape.num_heads, N), dtype=torch.float32, device=q.device) if want_lse else None
+        _on_stream(stream, lse)
         return out, lse
 
     def token_stride_attn(self, q, k, v, shape: ShapeC, stride: int, offset: int = 0, out=None, out_fp32=False, want_lse=False,
                           stream=None):
-        out, lse = self._out_lse(q, shape, out, out_fp32, want_lse)
+        out, lse = self._out_lse(q, shape, out, out_fp32, want_lse, stream)
         self._check(self.lib.saf3r_token_stride_attn(self.h, q.data_ptr(), k.data_ptr(), v.data_ptr(), C.byref(shape), int(stride),
                                                      int(offset), out.data_ptr(), int(out_fp32),
                                                      lse.data_ptr() if lse is not None else None, _stream_ptr(stream)))
@@ -249,8 +267,10 @@ class Context:
         sel_ws, _ = token_query_sizes(shape, K)
         if workspace is None:
             workspace = torch.empty(sel_ws, dtype=torch.uint8, device=q.device)
+            _on_stream(stream, workspace)
         if idx is None:
             idx = torch.empty((shape.num_heads, K), dtype=torch.int32, device=q.device)
+            _on_stream(stream, idx)
         self._check(self.lib.saf3r_token_probe_select(self.h, q.data_ptr(), k.data_ptr(), C.byref(shape), int(K), workspace.data_ptr(),
                                                       workspace.numel(), idx.data_ptr(), _stream_ptr(stream)))
         return idx
@@ -261,7 +281,8 @@ class Context:
         _, att_ws = token_query_sizes(shape, K)
         if workspace is None:
             workspace = torch.empty(att_ws, dtype=torch.uint8, device=q.device)
-        out, lse = self._out_lse(q, shape, out, out_fp32, want_lse)
+            _on_stream(stream, workspace)
+        out, lse = self._out_lse(q, shape, out, out_fp32, want_lse, stream)
         self._check(self.lib.saf3r_token_set_attn(self.h, q.data_ptr(), k.data_ptr(), v.data_ptr(), C.byref(shape), idx.data_ptr(), K,
                                                   workspace.data_ptr(), workspace.numel(), out.data_ptr(), int(out_fp32),
                                                   lse.data_ptr() if lse is not None else None, _stream_ptr(stream)))

@@ -6,7 +6,7 @@
 //   warps 0-3   "MUFU" softmax: thread r owns q-row r (TMEM lane r), columns [0, kSplit): p = ex2.approx(s*c - m*c)
 //   warps 4-7   "FMA"  softmax: same rows, columns [kSplit, B): 2^x by Cody-Waite + degree-3 polynomial on the FMA/ALU
 //               pipes (no MUFU).  The two halves of a row exchange their partial row max through shared memory.
-//   warp  8     TMA producer: Q tile once, then K_J into a 2-stage ring and V_J into a 3-stage ring
+//   warp  8     TMA producer: Q tile once, then K_J into a 3-stage ring and V_J into a 2-stage ring
 //   warp  9     TMEM allocator + MMA issuer (one thread): S = Q K_J^T (tcgen05 SS), O += P V_J (tcgen05 TS: P from TMEM)
 //   warps 10-11 idle (they only complete the third warpgroup so that setmaxnreg can hand its registers over)
 // Running max is lazy (moves only when a row max grows by more than 2^8), so O in TMEM is rescaled rarely.
@@ -14,14 +14,6 @@
 #pragma once
 #include "ptx.cuh"
 #include "saf3r.h"
-
-#ifndef SAF3R_SPLIT_128
-#define SAF3R_SPLIT_128 80  // columns of a 128-wide tile whose exponentials use the MUFU (rest: FMA-pipe polynomial)
-#endif
-
-#ifndef SAF3R_MUFU_WARP0
-#define SAF3R_MUFU_WARP0 0  // first warp of the MUFU softmax group (the FMA group takes the other of warps 0-3 / 4-7)
-#endif
 
 namespace saf3r {
 
@@ -49,7 +41,7 @@ constexpr int kRegsMufu = 112, kRegsFma = 88, kRegsIdle = 40;  // 128*(112+88+40
 
 template <int B>
 struct AttnSmem {
-  static constexpr int kSplit = (B == 128) ? SAF3R_SPLIT_128 : 32;
+  static constexpr int kSplit = (B == 128) ? 80 : 32;  // columns whose exponentials use the MUFU (rest: FMA-pipe polynomial)
   static constexpr int kQ = 0;                          // 128 x 64 bf16 (only the first B rows are loaded)
   static constexpr int kK = kQ + 128 * 128;             // kKStages x (B x 64 bf16)
   static constexpr int kV = kK + kKStages * B * 128;    // kVStages x (B x 64 bf16)
@@ -336,7 +328,7 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
         }
       }
     }
-  } else if (warp >= SAF3R_MUFU_WARP0 && warp < SAF3R_MUFU_WARP0 + 4) {
+  } else if (warp < 4) {
     setmaxnreg_inc<kRegsMufu>();
     softmax_half<B, 0, L::kSplit, false>(p, smem, tmem, n_ent, e0, h, I, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
   } else {

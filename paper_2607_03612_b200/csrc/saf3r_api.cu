@@ -29,6 +29,8 @@ struct MapKey {
   }
 };
 
+constexpr size_t kMapCacheEntries = 512;
+
 struct saf3r_ctx {
   int device = 0;
   int sm_count = 0;
@@ -42,7 +44,7 @@ struct saf3r_ctx {
   bool stage_timing = false;
   cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};  // select: start, after the pool launch, after the select launch
   bool ev_valid = false;
-  std::vector<std::pair<MapKey, CUtensorMap>> maps;  // small LRU-less cache
+  std::vector<std::pair<MapKey, CUtensorMap>> maps;  // LRU cache, most recently used last (a 24-layer stack holds 72 q/k/v keys)
   // per-head list totals of the lists saf3r_select last wrote into a given row_ptr buffer (scheduling hint only)
   struct LenHint { const int64_t *row_ptr; int32_t H, NB; int64_t len[SAF3R_MAX_HEADS]; };
   std::vector<LenHint> hints;
@@ -253,6 +255,30 @@ saf3r_status saf3r_query_sizes(const saf3r_shape *shape, const saf3r_head_cfg *c
 
 }  // extern "C"
 
+
+// Launch plan of the score + select kernel: rows per score strip R (16; fewer when R*NB keys do not fit the shared-memory budget of
+// two CTAs per SM - then of one - or when the BLOCK_TOPK heads are few, so that the strips cover every SM twice) and the dynamic
+// shared memory.  A closed form of (shape, cfg, SM count), computed BEFORE anything is enqueued.
+struct SelPlan { int R; size_t smem; const char *unsupported; };
+static SelPlan select_plan(const SelGeom &g, int n_block, int n_probe, int sm_count) {
+  SelPlan p{kSelRows, 0, nullptr};
+  const size_t row = (size_t)kt_stride(g.NB) * 4;
+  if (n_block > 0) {
+    const size_t qbytes = 64 * kSelRows * 4;
+    size_t budget = 108 * 1024 - qbytes;
+    if (row > budget) budget = 220 * 1024 - qbytes;
+    if (row > budget) { p.unsupported = "NB too large for the select kernel"; return p; }
+    while ((size_t)p.R * row > budget) --p.R;
+    while (p.R > 8 && (int64_t)n_block * ((g.NB + p.R - 1) / p.R) < 2 * (int64_t)sm_count) p.R = (p.R + 1) / 2;
+    p.smem = (size_t)p.R * row + qbytes;
+  }
+  if (n_probe > 0) {
+    if (row > 200 * 1024) { p.unsupported = "NB too large for the probe stage"; return p; }
+    if (p.smem < row) p.smem = row;
+  }
+  return p;
+}
+
 static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, const saf3r_shape *shape, const saf3r_head_cfg *cfg,
                                 const saf3r_lists *cache, int cache_heads, void *ws, size_t ws_bytes, saf3r_lists *lists,
                                 void *stream_) {
@@ -306,12 +332,9 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
   memset(&plan, 0, sizeof plan);
   HeadSets sets;
   memset(&sets, 0, sizeof sets);
-  bool any_block = false, any_probe = false;
   int64_t base = 0;
   for (int h = 0; h < g.H; ++h) {
     ca.c[h] = cfg[h];
-    any_block |= cfg[h].type == SAF3R_HEAD_BLOCK_TOPK;
-    any_probe |= cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK;
     const bool per_row = cfg[h].type == SAF3R_HEAD_STATIC && cfg[h].static_mode != SAF3R_STATIC_ANCHOR;
     if (cfg[h].type == SAF3R_HEAD_CACHED) sets.cached[sets.n_cached++] = (uint8_t)h;
     else if (cfg[h].type == SAF3R_HEAD_BLOCK_TOPK) sets.block[sets.n_block++] = (uint8_t)h;
@@ -323,7 +346,7 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
     base += hint.len[h];
   }
   plan.head_base[g.H] = base;
-  // pool jobs: QUERY_PROBE heads first (their probe runs in the last pool CTA of the head, under the other heads' pooling)
+  // pool jobs: QUERY_PROBE heads first (their probe CTAs come first in launch 2 and overlap with its score CTAs)
   for (int pass = 0; pass < 2; ++pass)
     for (int h = 0; h < g.H; ++h) {
       const bool probe = cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK, block = cfg[h].type == SAF3R_HEAD_BLOCK_TOPK;
@@ -336,6 +359,11 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
         ++jobs.n;
       }
     }
+  // launch 2's plan first: an UNSUPPORTED shape must be reported before anything is enqueued (saf3r.h "Asynchrony")
+  const SelPlan sp = select_plan(g, sets.n_block, sets.n_probe, ctx->sm_count);
+  if (sp.unsupported) return fail(ctx, SAF3R_ERR_UNSUPPORTED, sp.unsupported);
+  const int R = sp.R;
+  const size_t sm = sp.smem;
   // launch 1: pooling (one warp per token block of every tensor a rule reads) + one row_ptr CTA per head + the lists of the
   // constant-length closed-form heads
   const int pool_tasks = jobs.n * ((g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask);
@@ -352,25 +380,9 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
       (const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart, lists->row_ptr, lists->col_idx, g, jobs, plan, ca, sets,
       pool_ctas, pool_tasks);
   ctx->launches += 1;
+  CU_CHECK(cudaGetLastError());
   if (ctx->stage_timing) cudaEventRecord(ctx->ev[1], st);
-  // launch 2: probe CTAs, score + select CTAs (R rows each: 16, fewer when NB is large - two CTAs per SM if possible - or
-  // when the BLOCK_TOPK heads are few), light CTAs of the per-row-length STATIC heads
-  int R = kSelRows;
-  size_t sm = 0;
-  const size_t row = (size_t)kt_stride(g.NB) * 4;
-  if (any_block) {
-    const size_t qbytes = 64 * kSelRows * 4;
-    size_t budget = 108 * 1024 - qbytes;
-    if (row > budget) budget = 220 * 1024 - qbytes;
-    if (row > budget) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the select kernel");
-    while ((size_t)R * row > budget) --R;
-    while (R > 8 && (int64_t)sets.n_block * ((g.NB + R - 1) / R) < 2 * (int64_t)ctx->sm_count) R = (R + 1) / 2;
-    sm = (size_t)R * row + qbytes;
-  }
-  if (any_probe) {
-    if (row > 200 * 1024) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "NB too large for the probe stage");
-    if (sm < row) sm = row;
-  }
+  // launch 2: probe CTAs, score + select CTAs (R rows each), light CTAs of the per-row-length STATIC heads and of CACHED heads
   const int sel_ctas = sets.n_probe + sets.n_block * ((g.NB + R - 1) / R) + (sets.n_light + sets.n_cached) * light_chunks;
   if (sel_ctas > 0) {
     cudaLaunchConfig_t lc;
@@ -423,8 +435,16 @@ saf3r_status saf3r_select_cached(saf3r_ctx *ctx, const void *q, const void *k, c
 
 static saf3r_status get_map(saf3r_ctx *ctx, const void *ptr, const SelGeom &g, CUtensorMap *out) {
   MapKey key{ptr, g.N, g.stride_head, g.stride_token, g.H, g.B};
-  for (auto &kv : ctx->maps)
-    if (kv.first == key) { *out = kv.second; return SAF3R_OK; }
+  for (size_t i = ctx->maps.size(); i-- > 0;)  // most recently used at the back
+    if (ctx->maps[i].first == key) {
+      *out = ctx->maps[i].second;
+      if (i + 1 != ctx->maps.size()) {  // LRU: move the hit to the back
+        auto hit = ctx->maps[i];
+        ctx->maps.erase(ctx->maps.begin() + (long)i);
+        ctx->maps.push_back(hit);
+      }
+      return SAF3R_OK;
+    }
   CUtensorMap m;
   const cuuint64_t dims[3] = {64, (cuuint64_t)g.N, (cuuint64_t)g.H};
   const cuuint64_t strides[2] = {(cuuint64_t)g.stride_token * 2, (cuuint64_t)g.stride_head * 2};
@@ -441,7 +461,7 @@ static saf3r_status get_map(saf3r_ctx *ctx, const void *ptr, const SelGeom &g, C
     snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
     return fail(ctx, SAF3R_ERR_INVALID_ARG, buf);
   }
-  if (ctx->maps.size() >= 64) ctx->maps.erase(ctx->maps.begin());
+  if (ctx->maps.size() >= kMapCacheEntries) ctx->maps.erase(ctx->maps.begin());  // evict the least recently used
   ctx->maps.emplace_back(key, m);
   *out = m;
   return SAF3R_OK;
@@ -519,6 +539,24 @@ saf3r_status saf3r_sparse_attn(saf3r_ctx *ctx, const void *q, const void *k, con
                                const saf3r_lists *lists, void *out, int out_is_fp32, float *lse, void *stream) {
   if (!lists) return fail(ctx, SAF3R_ERR_INVALID_ARG, "lists is null");
   return attn_common(ctx, q, k, v, shape, lists, out, out_is_fp32, lse, stream);
+}
+
+saf3r_status saf3r_select_plan(const saf3r_ctx *ctx, const saf3r_shape *shape, const saf3r_head_cfg *cfg, int32_t *strip_rows,
+                               size_t *smem_bytes) {
+  if (!ctx || validate_shape(shape, false) || !cfg) return SAF3R_ERR_INVALID_ARG;
+  if (unsupported_shape(shape)) return SAF3R_ERR_UNSUPPORTED;
+  const SelGeom g = make_geom(shape);
+  if (validate_cfg(g, cfg, SAF3R_MAX_HEADS)) return SAF3R_ERR_INVALID_ARG;
+  int nb = 0, np = 0;
+  for (int h = 0; h < g.H; ++h) {
+    nb += cfg[h].type == SAF3R_HEAD_BLOCK_TOPK;
+    np += cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK;
+  }
+  const SelPlan sp = select_plan(g, nb, np, ctx->sm_count);
+  if (sp.unsupported) return SAF3R_ERR_UNSUPPORTED;
+  if (strip_rows) *strip_rows = nb > 0 ? sp.R : 0;
+  if (smem_bytes) *smem_bytes = sp.smem;
+  return SAF3R_OK;
 }
 
 saf3r_status saf3r_check_lists(saf3r_ctx *ctx, const saf3r_shape *shape, const saf3r_lists *lists, int64_t *bad_rows, void *stream_) {

@@ -1,9 +1,10 @@
 // Online pattern adaptation at block granularity (steps a-1..a-3 of DESIGN.md):
-//   pool_rowptr_kernel  Q,K bf16 -> Qtilde,Ktilde fp32 block means (HBM-bound stream, one warp per block); in extra CTAs
-//                       of the same launch, row_ptr from the closed-form row lengths; and, in the last pool CTA of each
-//                       QUERY_PROBE head, the probe: qbar = (1/N) sum_t q_t, p[J] = qbar . Ktilde_J / sqrt(D),
-//                       top-n -> one shared list per head
-//   select_kernel       per (head, q-block): closed-form emit, probe-list copy, or score row + top-n / per-frame top-k
+//   pool_rowptr_kernel  Q,K bf16 -> Qtilde,Ktilde fp32 block means and per-task token sums of Q (HBM-bound stream); in extra
+//                       CTAs of the same launch, row_ptr from the closed-form row lengths and the lists of the constant-length
+//                       closed-form heads
+//   select_kernel       one probe CTA per QUERY_PROBE head: qbar = (1/N) sum_t q_t, p[J] = qbar . Ktilde_J /
+//                       sqrt(D), top-n -> the head's lists; score CTAs per (BLOCK_TOPK head, strip of q-blocks): score rows +
+//                       top-n / per-frame top-k; light CTAs: per-row closed forms and copies from the index cache
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>

@@ -124,8 +124,8 @@ __global__ void __launch_bounds__(256) token_probe_kernel(const __nv_bfloat16 *_
 
 // grid (H), 1024 threads.  idx[h][0..K): the K tokens with the largest keys, ascending; ties at the cut by lower index.
 // Radix select in three digits (11 + 11 + 10 bits).  The histogram of the first digit over ALL keys comes from the probe pass
-// (hist1), so no pass here issues a shared-memory atomic per key: the two remaining histogram passes only count the keys that
-// match the prefix found so far.  Every pass keeps eight independent loads in flight per thread (the keys are L2-resident; one
+// (hist1: the probe kernel counts every key once with a shared-memory atomic), so the two histogram passes here only issue a
+// shared-memory atomic for the keys that match the prefix found so far (a small fraction of N).  Every pass keeps eight independent loads in flight per thread (the keys are L2-resident; one
 // CTA per head is latency-bound otherwise).  Histogram passes read strided (order does not matter), the compaction pass reads
 // eight CONSECUTIVE keys per thread so that a block-wide scan of per-thread counts gives ordered output positions.
 __global__ void __launch_bounds__(1024) token_topk_kernel(const uint32_t *__restrict__ keys, const uint32_t *__restrict__ hist1,

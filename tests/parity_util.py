@@ -43,7 +43,10 @@ def concat_lists(hls):
     return np.concatenate(row_ptr), np.concatenate(cols) if cols else np.zeros(0, np.int32)
 
 
-def compare_lists(L: sy.Layer, gpu_row_ptr: np.ndarray, gpu_col: np.ndarray, hls) -> dict:
+LIST_REPORT: dict = {}  # tag -> near-tie statistics of compare_lists (written next to REPORT)
+
+
+def compare_lists(L: sy.Layer, gpu_row_ptr: np.ndarray, gpu_col: np.ndarray, hls, tag: str | None = None) -> dict:
     """Bit-exact comparison except at near-ties of the selection cut.  Returns counts; raises on a real mismatch."""
     sh = L.shape
     NB, S, T, B = sh.NB, sh.S, sh.T, sh.B
@@ -80,15 +83,25 @@ def compare_lists(L: sy.Layer, gpu_row_ptr: np.ndarray, gpu_col: np.ndarray, hls
                     f"head {h} row {I}: block {J} differs and is not a near-tie (|s-tau|={d:.3e}, tau={tau:.3e})"
                 stats["tie_floored"] += 1
                 stats["tie_strict"] += int(d <= TIE_REL * abs(tau))
+    if tag:
+        LIST_REPORT[tag] = dict(stats)
     return stats
 
 
-def check_attention(out: np.ndarray, ref: np.ndarray, what: str = "") -> tuple[float, float]:
+REPORT: dict = {}      # tag -> [worst max-abs, worst mean-abs, checks]; written to gpurun_out/ at session end (conftest.py)
+
+
+def check_attention(out: np.ndarray, ref: np.ndarray, what: str = "", tag: str | None = None) -> tuple[float, float]:
+    """Asserts the north_star tolerances, prints (max-abs, mean-abs) (visible under -s) and keeps the worst per tag (default:
+    the first word of `what`, e.g. "C3") for the parity report."""
     mask = ~np.isnan(ref)
     assert mask.any()
     assert not np.isnan(out[mask]).any(), f"{what}: NaN in GPU output"
     d = np.abs(out[mask].astype(np.float64) - ref[mask])
     mx, mean = float(d.max()), float(d.mean())
+    print(f"parity {what}: max-abs {mx:.3e} (budget {MAX_ABS_TOL:g}), mean-abs {mean:.3e} (budget {MEAN_ABS_TOL:g})")
+    r = REPORT.setdefault(tag or (what.split()[0] if what else "?"), [0.0, 0.0, 0])
+    r[0], r[1], r[2] = max(r[0], mx), max(r[1], mean), r[2] + 1
     assert mx <= MAX_ABS_TOL, f"{what}: max-abs {mx:.3e} > {MAX_ABS_TOL}"
     assert mean <= MEAN_ABS_TOL, f"{what}: mean-abs {mean:.3e} > {MEAN_ABS_TOL}"
     return mx, mean

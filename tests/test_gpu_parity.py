@@ -148,7 +148,7 @@ def test_c1_end_to_end(env):
     torch.cuda.synchronize()
     hls = oracle_lists(L)
     rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
-    stats = compare_lists(L, rp, col, hls)
+    stats = compare_lists(L, rp, col, hls, tag="C1 (4 heads, full)")
     assert stats["tie_floored"] == 0
     for h in range(sh.H):
         # protocol (iii): oracle attention evaluated on the GPU's own lists
@@ -202,7 +202,7 @@ def test_c2_full_size_lists_and_sampled_attention(env):
     torch.cuda.synchronize()
     hls = oracle_lists(L)
     rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
-    stats = compare_lists(L, rp, col, hls)
+    stats = compare_lists(L, rp, col, hls, tag="C2 (16 heads, full size)")
     print("C2 near-ties:", stats)
     assert stats["tie_floored"] <= 1e-3 * stats["entries"]
     rng = np.random.default_rng(2)
@@ -245,7 +245,7 @@ def test_c3_full_size_lists_and_sampled_attention(env):
     torch.cuda.synchronize()
     hls = oracle_lists(L)
     rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
-    stats = compare_lists(L, rp, col, hls)
+    stats = compare_lists(L, rp, col, hls, tag="C3 layer 0 (16 heads, full size)")
     print("C3 near-ties:", stats)
     assert stats["tie_floored"] <= 1e-3 * stats["entries"]
     rng = np.random.default_rng(3)
@@ -286,8 +286,9 @@ def test_select_planted_exact_ties(env):
 
 
 def test_select_large_nb_paths(env):
-    """NB = 1160 > 1152: the top-n bisection reads its keys from shared memory (no register cache) and the score stage
-    runs its 1024-column main pass plus a left-over pass; n = NB keeps everything (degenerate cut)."""
+    """NB = 1160 > 1152: the top-n keeps 72 keys per lane in registers (the 36-key variant ends at NB = 1152; only NB > 2304, the
+    C5 shape, reads its keys from shared memory) and the score stage runs its 1024-column main pass plus a left-over pass;
+    n = NB keeps everything (degenerate cut)."""
     sf, ctx, torch = env
     gens = [sy.GEN_SAME_POSITION, sy.GEN_SINK, sy.GEN_SAME_POSITION, sy.GEN_UNIFORM]
     sh = sy.Shape(S=54, G=37, H=4, D=64, B=64)                   # N = 74196, NB = 1160, tail 20
@@ -303,7 +304,7 @@ def test_select_large_nb_paths(env):
     out = ctx.sparse_attn(q, k, v, shape, lists, out_fp32=True)
     torch.cuda.synchronize()
     rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
-    stats = compare_lists(L, rp, col, oracle_lists(L))
+    stats = compare_lists(L, rp, col, oracle_lists(L), tag="NB=1160 (4 heads)")
     print("NB=1160 near-ties:", stats)
     assert stats["tie_floored"] <= 1e-3 * stats["entries"]
     for h in (0, 1):
@@ -545,7 +546,7 @@ def test_c5_shape_three_heads(env):
     torch.cuda.synchronize()
     assert ctx.check_lists(shape, lists) == 0
     rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
-    stats = compare_lists(L, rp, col, oracle_lists(L))
+    stats = compare_lists(L, rp, col, oracle_lists(L), tag="C5 shape (3 heads)")
     print("C5-shape near-ties:", stats)
     assert stats["tie_floored"] <= 1e-3 * stats["entries"]
     for h in range(sh.H):
@@ -553,6 +554,73 @@ def test_c5_shape_three_heads(env):
         r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
         ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, r - r[0], col[r[0]:r[-1]], qb, want_lse=False)
         check_attention(out[h].cpu().numpy(), ref, f"C5-shape head {h} ({gens[h]})")
+
+
+def test_c4_shape_three_heads(env):
+    """BASELINE.json's sparsity-sweep configuration (S = 200 frames, N = 274 800, NB = 2147, tail 112) with three heads so that
+    the oracle finishes in about a minute.  At NB = 2147 a key row is 8592 bytes, so the score strips are R = 12 rows high (108 KB
+    budget): the 16-row score routine runs with rows = 12 < 16 on EVERY strip, a path no other test reaches (asserted through
+    saf3r_select_plan).  Lists against the oracle under reading A11, attention on 2 sampled q-blocks per head on the GPU's own
+    lists (protocol iii), saf3r_check_lists == 0."""
+    sf, ctx, torch = env
+    sh = sy.Shape(S=200, G=37, H=3, D=64, B=128)
+    assert sh.NB == 2147 and sh.N - (sh.NB - 1) * sh.B == 112
+    gens = [sy.GEN_SAME_POSITION, sy.GEN_SAME_POSITION, sy.GEN_SINK]
+    cfgs = [sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=215),
+            sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=1, score_mode=sy.SCORE_COSINE),
+            sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=200)]
+    L = sy.make_layer(sh, gens, cfgs, seed=4004)
+    q, k, v = upload(L)
+    shape = c_shape(sf, sh)
+    strip_rows, smem = ctx.select_plan(shape, L.cfgs)
+    print("C4-shape select plan: strip rows", strip_rows, "smem", smem)
+    assert 8 < strip_rows < 16, "this shape is meant to exercise score strips whose height is not 4, 8 or 16"
+    lists = ctx.select(q, k, shape, L.cfgs)
+    out = ctx.sparse_attn(q, k, v, shape, lists, out_fp32=True)
+    torch.cuda.synchronize()
+    assert ctx.check_lists(shape, lists) == 0
+    rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
+    stats = compare_lists(L, rp, col, oracle_lists(L), tag="C4 shape (3 heads)")
+    print("C4-shape near-ties:", stats)
+    assert stats["tie_floored"] <= 1e-3 * stats["entries"]
+    for h in range(sh.H):
+        qb = np.array([sh.NB // 3, sh.NB - 1], np.int64)
+        r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
+        ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, r - r[0], col[r[0]:r[-1]], qb, want_lse=False)
+        check_attention(out[h].cpu().numpy(), ref, f"C4-shape head {h} ({gens[h]})")
+
+
+def test_layer_host_sixteen_mixed_heads_back_to_back(env):
+    """saf3r_layer_host in the geometry bench.py's e2e key times: H = 16 mixed heads = 8 groups of 2 heads wrapping over the 3
+    side streams (groups i and i+3 share a stream), per-group sub-geometry / list bases / cfg offsets; and a SECOND call issued
+    before the first has finished (no sync in between, different scratch and output buffers).  Every head of both calls against
+    the oracle on the oracle's lists (bf16 output)."""
+    sf, ctx, torch = env
+    sh = sy.Shape(S=6, G=16, H=16, D=64, B=64)                    # T = 261, N = 1566, NB = 25
+    gens = [sy.GEN_UNIFORM, sy.GEN_FRAME_LOCAL, sy.GEN_SAME_POSITION, sy.GEN_SINK] * 4
+    cfgs = []
+    for h in range(16):
+        cfgs.append([sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=0, keep_blocks=3 + h),
+                     sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_FRAME_LOCAL) if h % 8 == 1 else
+                     sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_POSITION_BAND, band_radius=4 + h),
+                     sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=2 + h // 2) if h % 8 == 2 else
+                     sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=1 + h % 3, score_mode=sy.SCORE_COSINE),
+                     sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=4 + h // 4)][h % 4])
+    layers = [sy.make_layer(sh, gens, cfgs, seed=91 + i, layer=i) for i in range(2)]
+    shape = c_shape(sf, sh)
+    pin = lambda x: torch.from_numpy(x.view(np.int16)).view(torch.bfloat16).pin_memory()
+    host = [(pin(L.q), pin(L.k), pin(L.v)) for L in layers]
+    outs = [torch.zeros_like(h3[0]).pin_memory() for h3 in host]
+    nbytes = ctx.layer_host_scratch_bytes(shape, cfgs)
+    scratch = [torch.empty(nbytes, dtype=torch.uint8, device="cuda") for _ in layers]
+    for (qh, kh, vh), o, sc in zip(host, outs, scratch):           # two calls back to back, no synchronisation in between
+        ctx.layer_host(qh, kh, vh, shape, cfgs, sc, o)
+    torch.cuda.synchronize()
+    for L, o in zip(layers, outs):
+        for h, hl in enumerate(oracle_lists(L, want_scores=False)):
+            ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, hl.row_ptr, hl.col_idx)
+            d = np.abs(o[h].float().numpy() - ref)
+            assert d.max() <= 3e-2 and d.mean() <= 2e-3, f"layer_host head {h} ({gens[h]}): max {d.max():.3e} mean {d.mean():.3e}"
 
 
 @pytest.mark.parametrize("S,G,B,H", [(32, 3, 64, 1), (64, 3, 128, 2), (1, 3, 64, 1)])
@@ -600,6 +668,6 @@ def test_select_sixteen_block_heads(env):
     lists = ctx.select(q, k, shape, L.cfgs)
     torch.cuda.synchronize()
     assert ctx.check_lists(shape, lists) == 0
-    stats = compare_lists(L, lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy(), oracle_lists(L))
+    stats = compare_lists(L, lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy(), oracle_lists(L), tag="C2 shape, 16 BLOCK_TOPK heads")
     print("16 block heads near-ties:", stats)
     assert stats["tie_floored"] <= 1e-3 * stats["entries"]
