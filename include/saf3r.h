@@ -139,6 +139,15 @@ saf3r_status saf3r_sparse_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_
 saf3r_status saf3r_check_lists(saf3r_ctx *ctx, const saf3r_shape *shape, const saf3r_lists *lists, int64_t *bad_rows_host,
                                void *cuda_stream);
 
+/* Union of two sets of block lists, row by row ("combining Top-K with uniform striding to
+ * reduce missing regions"): out(h, I) = a(h, I) U b(h, I), ascending and unique - e.g. the lists of one saf3r_select call with
+ * BLOCK_TOPK rules and of another with UNIFORM_STRIDE rules.  a, b: lists over the same (H, NB); out: caller-owned, must not
+ * alias an input; out->capacity >= entries(a) + entries(b) always suffices.  Entries that would not fit out->capacity are not
+ * written; out->row_ptr[H*NB] always holds the true total, so a caller in doubt compares it with the capacity
+ * (saf3r_check_lists reports such lists as malformed).  Three launches (count, scan, write); enqueues and returns. */
+saf3r_status saf3r_union_lists(saf3r_ctx *ctx, const saf3r_shape *shape, const saf3r_lists *a, const saf3r_lists *b,
+                               saf3r_lists *out, void *cuda_stream);
+
 /* Dense mode of the same kernel (implicit list 0..NB-1, no list reads). */
 saf3r_status saf3r_dense_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const void *v_dev,
                               const saf3r_shape *shape, void *out_dev, int out_is_fp32, float *lse_dev_or_null,

@@ -56,6 +56,8 @@ def lib():
         L.orc_attn_dense.argtypes = [vp, vp, vp, i64, i32, i64, i64, vp, vp]
         L.orc_attn_tokens.argtypes = [vp, vp, vp, i64, i32, vp, i64, i64, i64, vp, vp]
         L.orc_token_probe.argtypes = [vp, vp, i64, i32, vp]
+        L.orc_union_lists.argtypes = [vp, vp, vp, vp, i64, i64, vp, vp, i64]
+        L.orc_union_lists.restype = i64
         L.orc_nmse.argtypes = [vp, vp, i64]
         L.orc_nmse.restype = dbl
         L.orc_num_threads.restype = i32
@@ -199,6 +201,21 @@ def token_probe_topk(q_bits, k_bits, K: int):
     p = token_probe(q_bits, k_bits)
     keep = topn(p, K, use_sort=True)
     return keep.astype(np.int64), p
+
+
+def union_lists(row_ptr_a, col_a, row_ptr_b, col_b, NB: int):
+    """Row-wise set union of two CSR block lists over the same rows; returns (row_ptr, col_idx), rows ascending."""
+    ra, rb = np.ascontiguousarray(row_ptr_a, np.int64), np.ascontiguousarray(row_ptr_b, np.int64)
+    ca, cb = np.ascontiguousarray(col_a, np.int32), np.ascontiguousarray(col_b, np.int32)
+    assert ra.shape == rb.shape
+    rows = ra.shape[0] - 1
+    cap = int(ca.size + cb.size) + 1
+    ro, co = np.empty((rows + 1,), np.int64), np.empty((cap,), np.int32)
+    pa = ca if ca.size else np.zeros((1,), np.int32)
+    pb = cb if cb.size else np.zeros((1,), np.int32)
+    n = lib().orc_union_lists(_p(ra), _p(pa), _p(rb), _p(pb), rows, NB, _p(ro), _p(co), cap)
+    assert n >= 0
+    return ro, co[:n].copy()
 
 
 def nmse(o_full: np.ndarray, o_sparse: np.ndarray) -> float:

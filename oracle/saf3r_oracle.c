@@ -408,6 +408,29 @@ void orc_token_probe(const uint16_t *q, const uint16_t *k, int64_t N, int32_t D,
   free(qbar);
 }
 
+/* ---- union of block lists ("combining Top-K with uniform striding") ----------------------
+ * out(I) = a(I) U b(I) for every row I, by the definition of a set union: J is kept iff it is in a's row or in b's row.
+ * Rows are emitted ascending.  Returns the number of entries, or -(needed) if capacity is too small. */
+int64_t orc_union_lists(const int64_t *rp_a, const int32_t *col_a, const int64_t *rp_b, const int32_t *col_b, int64_t rows,
+                        int64_t NB, int64_t *rp_o, int32_t *col_o, int64_t capacity) {
+  uint8_t *keep = (uint8_t *)malloc((size_t)(NB > 0 ? NB : 1));
+  int64_t cnt = 0;
+  rp_o[0] = 0;
+  for (int64_t I = 0; I < rows; ++I) {
+    memset(keep, 0, (size_t)NB);
+    for (int64_t e = rp_a[I]; e < rp_a[I + 1]; ++e) keep[col_a[e]] = 1;
+    for (int64_t e = rp_b[I]; e < rp_b[I + 1]; ++e) keep[col_b[e]] = 1;
+    for (int64_t J = 0; J < NB; ++J)
+      if (keep[J]) {
+        if (cnt < capacity) col_o[cnt] = (int32_t)J;
+        ++cnt;
+      }
+    rp_o[I + 1] = cnt;
+  }
+  free(keep);
+  return cnt <= capacity ? cnt : -cnt;
+}
+
 /* O5  NMSE, Eq. 1 (one sample): ||O_full - O_sparse||_2^2 / ||O_full||_2^2. */
 double orc_nmse(const float *o_full, const float *o_sparse, int64_t count) {
   double num = 0.0, den = 0.0;

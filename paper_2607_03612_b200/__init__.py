@@ -27,7 +27,7 @@ SCORE_DOT, SCORE_COSINE = range(2)
 EXPORTS = ("saf3r_create", "saf3r_destroy", "saf3r_last_error", "saf3r_query_sizes", "saf3r_select", "saf3r_sparse_attn",
            "saf3r_dense_attn", "saf3r_layer_host_scratch_bytes", "saf3r_layer_host", "saf3r_launch_count",
            "saf3r_set_stage_timing", "saf3r_last_select_stage_ms", "saf3r_select_cached", "saf3r_token_stride_attn",
-           "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn", "saf3r_check_lists", "saf3r_select_plan")
+           "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn", "saf3r_check_lists", "saf3r_select_plan", "saf3r_union_lists")
 
 
 class Saf3rError(RuntimeError):
@@ -82,6 +82,7 @@ def load_library():
         L.saf3r_layer_host_scratch_bytes.argtypes = [C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(C.c_size_t)]
         L.saf3r_layer_host.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), vp, C.c_size_t, vp, vp]
         L.saf3r_select_plan.argtypes = [vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(C.c_int32), C.POINTER(C.c_size_t)]
+        L.saf3r_union_lists.argtypes = [vp, C.POINTER(ShapeC), C.POINTER(ListsC), C.POINTER(ListsC), C.POINTER(ListsC), vp]
         L.saf3r_launch_count.argtypes = [vp]
         L.saf3r_launch_count.restype = i64
         L.saf3r_set_stage_timing.argtypes = [vp, i32]
@@ -220,6 +221,18 @@ class Context:
         lc, bad = lists.c(), C.c_int64()
         self._check(self.lib.saf3r_check_lists(self.h, C.byref(shape), C.byref(lc), C.byref(bad), _stream_ptr(stream)))
         return int(bad.value)
+
+    # ---- saf3r_union_lists
+    def union_lists(self, shape: ShapeC, a: Lists, b: Lists, out: Lists | None = None, stream=None) -> Lists:
+        """Row-wise union of two sets of block lists (ascending, unique); out defaults to a buffer of entries(a) + entries(b)."""
+        import torch
+        if out is None:
+            out = Lists(torch.empty_like(a.row_ptr), torch.empty(a.col_idx.numel() + b.col_idx.numel(), dtype=torch.int32,
+                                                                 device=a.col_idx.device))
+            _on_stream(stream, out.row_ptr, out.col_idx)
+        ca, cb, co = a.c(), b.c(), out.c()
+        self._check(self.lib.saf3r_union_lists(self.h, C.byref(shape), C.byref(ca), C.byref(cb), C.byref(co), _stream_ptr(stream)))
+        return out
 
     # ---- saf3r_sparse_attn / saf3r_dense_attn
     def sparse_attn(self, q, k, v, shape: ShapeC, lists: Lists, out=None, out_fp32: bool = False, want_lse: bool = False, stream=None):

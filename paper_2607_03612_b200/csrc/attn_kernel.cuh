@@ -9,7 +9,12 @@
 //   warp  8     TMA producer: Q tile once, then K_J into a 3-stage ring and V_J into a 2-stage ring
 //   warp  9     TMEM allocator + MMA issuer (one thread): S = Q K_J^T (tcgen05 SS), O += P V_J (tcgen05 TS: P from TMEM)
 //   warps 10-11 idle (they only complete the third warpgroup so that setmaxnreg can hand its registers over)
-// Running max is lazy (moves only when a row max grows by more than 2^8), so O in TMEM is rescaled rarely.
+// Running max is lazy (moves only when a row max grows by more than 2^8), so O in TMEM is rescaled rarely.  And it is
+// FROZEN as soon as it provably cannot matter: by Cauchy-Schwarz every logit of row i is at most |q_i| * max_j |k_j| / sqrt(D)
+// (kmax[h] = max_j |k_j| comes from knorm_kernel, one streaming pass over K before the launch).  Once that bound is within
+// 2^kFreezeLog2 of the row's reference max for all 32 rows of a warp, no later tile can overflow (p <= 2^64, far inside the
+// bf16 / fp32 exponent range) and none can underflow relative to the true max, so the remaining tiles skip the row-max pass,
+// the exchange between the two halves and the named barrier altogether - about an eighth of the softmax instructions.
 // TMEM columns: S [0,B) fp32, O [128,192) fp32, P [192,192+B/2) packed bf16.
 #pragma once
 #include "ptx.cuh"
@@ -27,6 +32,7 @@ struct AttnParams {
   int32_t N_kv, NB_kv;  // key/value tokens / k-blocks (== N, NB except in the token-granular variants)
   int32_t out_fp32;
   float scale_log2;  // (1/sqrt(D)) * log2(e)
+  const float *kmax;  // [H] max_j |k_j|_2 over the head's key tokens (knorm_kernel), or nullptr: never freeze the max
   uint8_t head_order[SAF3R_MAX_HEADS];  // blockIdx.y -> head, longest lists first
 };
 
@@ -37,11 +43,14 @@ constexpr int kTmemCols = 256;
 constexpr int kTmemO = 128;  // first O column
 constexpr int kTmemP = 192;  // first P column
 constexpr float kLazyLog2 = 8.f;
+constexpr int kSleepTma = 128, kSleepMma = 48;  // ns between two mbarrier polls of the producer / issuer warps
+constexpr float kFreezeLog2 = 64.f;  // freeze the reference max when no logit can exceed it by more than 2^64
+constexpr int kSplit128 = 80;  // columns of a 128-wide tile whose exponentials use the MUFU (rest: FMA-pipe polynomial); any multiple of 8
 constexpr int kRegsMufu = 112, kRegsFma = 88, kRegsIdle = 40;  // 128*(112+88+40) = 30720 = 384 threads * 80 registers
 
 template <int B>
 struct AttnSmem {
-  static constexpr int kSplit = (B == 128) ? 80 : 32;  // columns whose exponentials use the MUFU (rest: FMA-pipe polynomial)
+  static constexpr int kSplit = (B == 128) ? kSplit128 : 32;  // columns whose exponentials use the MUFU (rest: FMA-pipe polynomial)
   static constexpr int kQ = 0;                          // 128 x 64 bf16 (only the first B rows are loaded)
   static constexpr int kK = kQ + 128 * 128;             // kKStages x (B x 64 bf16)
   static constexpr int kV = kK + kKStages * B * 128;    // kVStages x (B x 64 bf16)
@@ -54,11 +63,11 @@ struct AttnSmem {
 // one softmax half: rows = TMEM lanes of this warp, columns [C0, C1) of the B-wide tile
 template <int B, int C0, int C1, bool kFma>
 __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem, uint32_t tmem, int n_ent, int64_t e0, int h,
-                                             int I, uint32_t bar_s_full, uint32_t bar_s_free, uint32_t bar_p_full,
-                                             uint32_t bar_o_done) {
+                                             int I, uint32_t bar_q, uint32_t bar_s_full, uint32_t bar_s_free,
+                                             uint32_t bar_p_full, uint32_t bar_o_done) {
   using L = AttnSmem<B>;
   constexpr int NC = C1 - C0;
-  static_assert(NC % 16 == 0 && C0 % 16 == 0, "column split must be a multiple of 16");
+  static_assert(NC % 8 == 0 && C0 % 8 == 0, "column split must be a multiple of 8");
   constexpr int kHalf = kFma ? 1 : 0;
   const int r = threadIdx.x & 127;
   const int pair_bar = 1 + (r >> 5);  // named barrier shared by the two warps that own these 32 rows
@@ -76,13 +85,37 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
   float m = -INFINITY, l = 0.f;
   const int J_last = (n_ent > 0) ? (p.row_ptr ? p.col_idx[e0 + n_ent - 1] : p.NB_kv - 1) : -1;
   const bool last_is_tail = (J_last == p.NB_kv - 1) && (tail < B);
+  // Cauchy-Schwarz bound of this row's logits (in the units of m: raw scores), from the Q tile in shared memory.  Both halves
+  // of a row read the same eight 16-byte chunks in the same (physical) order, so they get the same bits and take the same
+  // freeze decision without talking to each other.
+  float bound = INFINITY;
+  bool frozen = false;
+  if (p.kmax != nullptr && n_ent > 1) {
+    mbar_wait(bar_q, 0);
+    const uint4 *qrow = reinterpret_cast<const uint4 *>(smem + L::kQ + r * 128);
+    float ss = 0.f;
+#pragma unroll
+    for (int ch = 0; ch < 8; ++ch) {
+      const uint4 w = qrow[ch];
+      const uint32_t u[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const float lo = __uint_as_float(u[i] << 16), hi = __uint_as_float(u[i] & 0xffff0000u);
+        ss = fmaf(lo, lo, ss);
+        ss = fmaf(hi, hi, ss);
+      }
+    }
+    bound = sqrtf(ss) * p.kmax[h] * 1.001f;  // rounding of the two norms and of the tensor-core sums: far below 1e-3
+  }
+  const float freeze_raw = kFreezeLog2 / c;
 
   for (int e = 0; e < n_ent; ++e) {
     uint32_t v[NC];
     mbar_wait(bar_s_full, e & 1);
     tc_fence_after();
 #pragma unroll
-    for (int cb = 0; cb < NC; cb += 16) tmem_ld16(tS + cb, *reinterpret_cast<uint32_t(*)[16]>(&v[cb]));
+    for (int cb = 0; cb + 16 <= NC; cb += 16) tmem_ld16(tS + cb, *reinterpret_cast<uint32_t(*)[16]>(&v[cb]));
+    if (NC % 16) tmem_ld8(tS + NC - 8, *reinterpret_cast<uint32_t(*)[8]>(&v[NC - 8]));
     tmem_ld_wait();
     tc_fence_before();
     mbar_arrive(bar_s_free);
@@ -91,29 +124,34 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
       for (int i = 0; i < NC; ++i)
         if (C0 + i >= tail) v[i] = 0xff800000u;  // -inf
     }
-    // partial row max over this half's columns, then exchange with the other half
-    float mx0 = __uint_as_float(v[0]), mx1 = __uint_as_float(v[1]), mx2 = __uint_as_float(v[2]), mx3 = __uint_as_float(v[3]);
-#pragma unroll
-    for (int i = 4; i < NC; i += 8) {
-      mx0 = max3(mx0, __uint_as_float(v[i]), __uint_as_float(v[i + 1]));
-      mx1 = max3(mx1, __uint_as_float(v[i + 2]), __uint_as_float(v[i + 3]));
-      if (i + 4 < NC) {
-        mx2 = max3(mx2, __uint_as_float(v[i + 4]), __uint_as_float(v[i + 5]));
-        mx3 = max3(mx3, __uint_as_float(v[i + 6]), __uint_as_float(v[i + 7]));
-      }
-    }
-    float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-    float *slot = smax + (e & 1) * 256;
-    slot[kHalf * 128 + r] = mx;
-    named_bar_sync(pair_bar, 64);
-    mx = fmaxf(mx, slot[(1 - kHalf) * 128 + r]);
-    // lazy running max (identical decision in both halves: same rows, same combined max)
     float alpha = 1.f;
-    const bool moved = __any_sync(0xffffffffu, mx > m + lazy_raw);
-    if (moved) {
-      const float m_new = fmaxf(m, mx);
-      alpha = ex2_approx((m - m_new) * c);
-      m = m_new;
+    bool moved = false;
+    if (!frozen) {
+      // partial row max over this half's columns, then exchange with the other half
+      float mx0 = __uint_as_float(v[0]), mx1 = __uint_as_float(v[1]), mx2 = __uint_as_float(v[2]), mx3 = __uint_as_float(v[3]);
+#pragma unroll
+      for (int i = 4; i < NC; i += 8) {
+        mx0 = max3(mx0, __uint_as_float(v[i]), __uint_as_float(v[i + 1]));
+        mx1 = max3(mx1, __uint_as_float(v[i + 2]), __uint_as_float(v[i + 3]));
+        if (i + 4 < NC) {
+          mx2 = max3(mx2, __uint_as_float(v[i + 4]), __uint_as_float(v[i + 5]));
+          mx3 = max3(mx3, __uint_as_float(v[i + 6]), __uint_as_float(v[i + 7]));
+        }
+      }
+      float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+      float *slot = smax + (e & 1) * 256;
+      slot[kHalf * 128 + r] = mx;
+      named_bar_sync(pair_bar, 64);
+      mx = fmaxf(mx, slot[(1 - kHalf) * 128 + r]);
+      // lazy running max (identical decision in both halves: same rows, same combined max)
+      moved = __any_sync(0xffffffffu, mx > m + lazy_raw);
+      if (moved) {
+        const float m_new = fmaxf(m, mx);
+        alpha = ex2_approx((m - m_new) * c);
+        m = m_new;
+      }
+      // no later logit of these 32 rows can exceed m by more than 2^kFreezeLog2: m stays where it is from now on
+      frozen = __all_sync(0xffffffffu, bound <= m + freeze_raw);
     }
     const float nmc = -m * c;
     uint32_t pk[NC / 2];
@@ -152,7 +190,8 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
       }
     }
 #pragma unroll
-    for (int cb = 0; cb < NC / 2; cb += 8) tmem_st8(tP + cb, *reinterpret_cast<uint32_t(*)[8]>(&pk[cb]));
+    for (int cb = 0; cb + 8 <= NC / 2; cb += 8) tmem_st8(tP + cb, *reinterpret_cast<uint32_t(*)[8]>(&pk[cb]));
+    if ((NC / 2) % 8) tmem_st4(tP + NC / 2 - 4, *reinterpret_cast<uint32_t(*)[4]>(&pk[NC / 2 - 4]));
     tmem_st_wait();
     tc_fence_before();
     mbar_arrive(bar_p_full);
@@ -267,13 +306,13 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
         for (int e = 0; e < n_ent; ++e) {
           const int J = Jn;
           if (e + 1 < n_ent) Jn = p.row_ptr ? p.col_idx[e0 + e + 1] : e + 1;
-          mbar_wait(bar_k_empty + 8 * sk, phk ^ 1);
+          mbar_wait_relaxed<kSleepTma>(bar_k_empty + 8 * sk, phk ^ 1);
           if (elect_one_sync()) {
             mbar_arrive_expect_tx(bar_k_full + 8 * sk, B * 128);
             tma_load_3d(sbase + L::kK + sk * B * 128, &map_k, bar_k_full + 8 * sk, 0, J * B, h);
           }
           __syncwarp();
-          mbar_wait(bar_v_empty + 8 * sv, phv ^ 1);
+          mbar_wait_relaxed<kSleepTma>(bar_v_empty + 8 * sv, phv ^ 1);
           if (elect_one_sync()) {
             mbar_arrive_expect_tx(bar_v_full + 8 * sv, B * 128);
             tma_load_3d(sbase + L::kV + sv * B * 128, &map_v, bar_v_full + 8 * sv, 0, J * B, h);
@@ -292,7 +331,7 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
         const uint32_t tS = tmem, tO = tmem + kTmemO, tP = tmem + kTmemP;
         int sk = 0, phk = 0;
         auto issue_qk = [&]() {
-          mbar_wait(bar_k_full + 8 * sk, phk);
+          mbar_wait_relaxed<kSleepMma>(bar_k_full + 8 * sk, phk);
           tc_fence_after();
           if (elect_one_sync()) {
             const uint64_t kdesc = umma_desc_sw128(sbase + L::kK + sk * B * 128);
@@ -304,16 +343,16 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
           __syncwarp();
           if (++sk == kKStages) { sk = 0; phk ^= 1; }
         };
-        mbar_wait(bar_q, 0);
+        mbar_wait_relaxed<kSleepMma>(bar_q, 0);
         issue_qk();
         int sv = 0, phv = 0;
         for (int e = 0; e < n_ent; ++e) {
           if (e + 1 < n_ent) {
-            mbar_wait(bar_s_free, e & 1);  // S(e) is in registers -> overwrite it with S(e+1) while softmax(e) runs
+            mbar_wait_relaxed<kSleepMma>(bar_s_free, e & 1);  // S(e) is in registers -> overwrite it with S(e+1) while softmax(e) runs
             issue_qk();
           }
-          mbar_wait(bar_v_full + 8 * sv, phv);
-          mbar_wait(bar_p_full, e & 1);
+          mbar_wait_relaxed<kSleepMma>(bar_v_full + 8 * sv, phv);
+          mbar_wait_relaxed<kSleepMma>(bar_p_full, e & 1);
           tc_fence_after();
           if (elect_one_sync()) {
             const uint64_t vdesc = umma_desc_sw128(sbase + L::kV + sv * B * 128);
@@ -330,10 +369,10 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
     }
   } else if (warp < 4) {
     setmaxnreg_inc<kRegsMufu>();
-    softmax_half<B, 0, L::kSplit, false>(p, smem, tmem, n_ent, e0, h, I, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
+    softmax_half<B, 0, L::kSplit, false>(p, smem, tmem, n_ent, e0, h, I, bar_q, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
   } else {
     setmaxnreg_inc<kRegsFma>();
-    softmax_half<B, L::kSplit, B, true>(p, smem, tmem, n_ent, e0, h, I, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
+    softmax_half<B, L::kSplit, B, true>(p, smem, tmem, n_ent, e0, h, I, bar_q, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
   }
 
   tc_fence_before();
@@ -341,6 +380,56 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
   if (warp == 9) {
     __syncwarp();
     tmem_dealloc(tmem, kTmemCols);
+  }
+}
+
+// kmax[h] = max over the head's key tokens of |k_j|_2 (the Cauchy-Schwarz factor of the freeze test above).  One streaming pass
+// over K: grid (chunks, H), 256 threads, 8 lanes per 128-byte token row with eight 16-byte loads in flight per lane; the norms
+// are non-negative, so the maximum of their bit patterns as unsigned integers is the maximum of the floats (atomicMax into a
+// zeroed slot).
+constexpr int kKnormRows = 1024;  // token rows per CTA
+__global__ void __launch_bounds__(256) knorm_kernel(const __nv_bfloat16 *__restrict__ k, int64_t n_kv, int64_t stride_head,
+                                                    int64_t stride_token, float *__restrict__ kmax) {
+  const int h = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int sub = lane & 7, rg = lane >> 3;
+  const int64_t t0 = (int64_t)blockIdx.x * kKnormRows + warp * (kKnormRows / 8);
+  const __nv_bfloat16 *src = k + (int64_t)h * stride_head + sub * 8;
+  float best = 0.f;
+#pragma unroll 1
+  for (int r0 = 0; r0 < kKnormRows / 8; r0 += 32) {
+    uint4 raw[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int64_t t = t0 + r0 + rg + 4 * i;
+      raw[i] = make_uint4(0, 0, 0, 0);
+      if (t < n_kv) asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(raw[i].x), "=r"(raw[i].y), "=r"(raw[i].z), "=r"(raw[i].w) : "l"(src + t * stride_token));
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const uint32_t u[4] = {raw[i].x, raw[i].y, raw[i].z, raw[i].w};
+      float ss = 0.f;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const float lo = __uint_as_float(u[c] << 16), hi = __uint_as_float(u[c] & 0xffff0000u);
+        ss = fmaf(lo, lo, ss);
+        ss = fmaf(hi, hi, ss);
+      }
+      ss += __shfl_xor_sync(0xffffffffu, ss, 1);
+      ss += __shfl_xor_sync(0xffffffffu, ss, 2);
+      ss += __shfl_xor_sync(0xffffffffu, ss, 4);
+      best = fmaxf(best, ss);
+    }
+  }
+#pragma unroll
+  for (int off = 8; off < 32; off <<= 1) best = fmaxf(best, __shfl_xor_sync(0xffffffffu, best, off));
+  __shared__ float wmax[8];
+  if (lane == 0) wmax[warp] = best;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    float b = wmax[0];
+#pragma unroll
+    for (int w = 1; w < 8; ++w) b = fmaxf(b, wmax[w]);
+    atomicMax(reinterpret_cast<unsigned int *>(kmax + h), __float_as_uint(sqrtf(b) * 1.0001f));
   }
 }
 

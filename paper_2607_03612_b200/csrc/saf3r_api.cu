@@ -30,6 +30,7 @@ struct MapKey {
 };
 
 constexpr size_t kMapCacheEntries = 512;
+constexpr uint32_t kKmaxSlots = 256;
 
 struct saf3r_ctx {
   int device = 0;
@@ -41,6 +42,10 @@ struct saf3r_ctx {
   cudaStream_t side[3] = {nullptr, nullptr, nullptr};  // saf3r_layer_host: head-group pipeline (created on first use)
   cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
   unsigned long long *counter_dev = nullptr;  // tiny device scratch (saf3r_check_lists)
+  // per-head max key norm of the attention calls (knorm_kernel -> saf3r_attn_kernel): a ring of slots, one per call, so that
+  // calls in flight on different streams never share one (a slot is reused kKmaxSlots calls later)
+  float *kmax_ring = nullptr;
+  uint32_t kmax_next = 0;
   bool stage_timing = false;
   cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};  // select: start, after the pool launch, after the select launch
   bool ev_valid = false;
@@ -198,6 +203,7 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
   if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->counter_dev, sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->kmax_ring, sizeof(float) * kKmaxSlots * SAF3R_MAX_HEADS);
   if (e != cudaSuccess) {
     fprintf(stderr, "saf3r_create: cudaFuncSetAttribute / cudaMalloc failed: %s\n", cudaGetErrorString(e));
     delete ctx;
@@ -212,6 +218,7 @@ void saf3r_destroy(saf3r_ctx *ctx) {
   for (auto &e : ctx->ev)
     if (e) cudaEventDestroy(e);
   if (ctx->counter_dev) cudaFree(ctx->counter_dev);
+  if (ctx->kmax_ring) cudaFree(ctx->kmax_ring);
   for (auto &sd : ctx->side)
     if (sd) cudaStreamDestroy(sd);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -523,6 +530,17 @@ static saf3r_status attn_common(saf3r_ctx *ctx, const void *q, const void *k, co
       }
   }
   cudaStream_t st = (cudaStream_t)stream_;
+  // max key norm per head (one streaming pass over K) for the kernel's frozen-max fast path; worth it from a few k-tiles per
+  // q-block on (the pass reads K once, the attention reads it NB times through L2)
+  p.kmax = nullptr;
+  if (gk.NB >= 4) {
+    float *slot = ctx->kmax_ring + (size_t)(ctx->kmax_next++ % kKmaxSlots) * SAF3R_MAX_HEADS;
+    CU_CHECK(cudaMemsetAsync(slot, 0, sizeof(float) * g.H, st));
+    knorm_kernel<<<dim3((unsigned)((gk.N + kKnormRows - 1) / kKnormRows), g.H), 256, 0, st>>>((const __nv_bfloat16 *)k, gk.N, gk.stride_head,
+                                                                                             gk.stride_token, slot);
+    ctx->launches += 1;
+    p.kmax = slot;
+  }
   dim3 grid(g.NB, g.H);
   if (g.B == 128)
     saf3r_attn_kernel<128><<<grid, kAttnThreads, AttnSmem<128>::kTotal, st>>>(mq, mk, mv, p);
@@ -576,6 +594,28 @@ saf3r_status saf3r_check_lists(saf3r_ctx *ctx, const saf3r_shape *shape, const s
   CU_CHECK(cudaMemcpyAsync(&host, bad, sizeof host, cudaMemcpyDeviceToHost, st));
   CU_CHECK(cudaStreamSynchronize(st));
   *bad_rows = (int64_t)host;
+  return SAF3R_OK;
+}
+
+saf3r_status saf3r_union_lists(saf3r_ctx *ctx, const saf3r_shape *shape, const saf3r_lists *a, const saf3r_lists *b, saf3r_lists *out,
+                               void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_shape(shape, false)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  if (!a || !b || !out || !a->row_ptr || !a->col_idx || !b->row_ptr || !b->col_idx || !out->row_ptr || !out->col_idx)
+    return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  if (out->row_ptr == a->row_ptr || out->row_ptr == b->row_ptr || out->col_idx == a->col_idx || out->col_idx == b->col_idx)
+    return fail(ctx, SAF3R_ERR_INVALID_ARG, "the union is not computed in place: out must not alias an input");
+  const SelGeom g = make_geom(shape);
+  const int64_t rows = (int64_t)g.H * g.NB;
+  cudaStream_t st = (cudaStream_t)stream_;
+  const unsigned ctas = (unsigned)((rows + 127) / 128);
+  union_rows_kernel<false><<<ctas, 128, 0, st>>>(a->row_ptr, a->col_idx, b->row_ptr, b->col_idx, out->row_ptr, out->col_idx, rows, out->capacity);
+  scan_row_ptr_kernel<<<1, 1024, 0, st>>>(out->row_ptr, rows);
+  union_rows_kernel<true><<<ctas, 128, 0, st>>>(a->row_ptr, a->col_idx, b->row_ptr, b->col_idx, out->row_ptr, out->col_idx, rows, out->capacity);
+  ctx->launches += 3;
+  CU_CHECK(cudaGetLastError());
   return SAF3R_OK;
 }
 

@@ -740,4 +740,53 @@ __global__ void __launch_bounds__(256) check_lists_kernel(const int64_t *__restr
   }
 }
 
+// ------------------------------------------------------------------------------------------------ list union (NEXT-4)
+// out(h, I) = list_a(h, I) U list_b(h, I), ascending and unique ("combining Top-K with uniform striding").  Both
+// inputs are ascending and unique, so one thread walks a row of each with two cursors.  Three launches: count (row lengths into
+// out_row_ptr[r + 1]), an in-place inclusive scan by one CTA, write.  Entries past `capacity` are not written; the total in
+// out_row_ptr[rows] tells the caller.
+template <bool kWrite>
+__global__ void __launch_bounds__(128) union_rows_kernel(const int64_t *__restrict__ rp_a, const int32_t *__restrict__ col_a,
+                                                         const int64_t *__restrict__ rp_b, const int32_t *__restrict__ col_b,
+                                                         int64_t *__restrict__ rp_o, int32_t *__restrict__ col_o, int64_t rows,
+                                                         int64_t capacity) {
+  const int64_t r = (int64_t)blockIdx.x * 128 + threadIdx.x;
+  if (r >= rows) return;
+  int64_t a = rp_a[r], b = rp_b[r];
+  const int64_t a1 = rp_a[r + 1], b1 = rp_b[r + 1];
+  int64_t o = kWrite ? rp_o[r] : 0;
+  int32_t ja = a < a1 ? col_a[a] : INT32_MAX, jb = b < b1 ? col_b[b] : INT32_MAX;
+  while (a < a1 || b < b1) {
+    const int32_t j = ja < jb ? ja : jb;
+    if (kWrite && o < capacity) col_o[o] = j;
+    ++o;
+    if (ja == j) { ++a; ja = a < a1 ? col_a[a] : INT32_MAX; }
+    if (jb == j) { ++b; jb = b < b1 ? col_b[b] : INT32_MAX; }
+  }
+  if (!kWrite) rp_o[r + 1] = o;
+}
+
+// rp[0] = 0 and rp[1..rows] hold row lengths: turn them into offsets (inclusive scan in place), one CTA of 1024 threads.
+__global__ void __launch_bounds__(1024) scan_row_ptr_kernel(int64_t *__restrict__ rp, int64_t rows) {
+  __shared__ int64_t part[1024];
+  const int64_t per = (rows + 1023) / 1024;
+  const int64_t a = threadIdx.x * per < rows ? threadIdx.x * per : rows, b = a + per < rows ? a + per : rows;
+  int64_t s = 0;
+  for (int64_t i = a; i < b; ++i) s += rp[i + 1];
+  part[threadIdx.x] = s;
+  __syncthreads();
+  for (int off = 1; off < 1024; off <<= 1) {
+    const int64_t v = (int)threadIdx.x >= off ? part[threadIdx.x - off] : 0;
+    __syncthreads();
+    part[threadIdx.x] += v;
+    __syncthreads();
+  }
+  int64_t run = threadIdx.x ? part[threadIdx.x - 1] : 0;
+  if (threadIdx.x == 0) rp[0] = 0;
+  for (int64_t i = a; i < b; ++i) {
+    run += rp[i + 1];
+    rp[i + 1] = run;
+  }
+}
+
 }  // namespace saf3r

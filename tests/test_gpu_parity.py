@@ -671,3 +671,42 @@ def test_select_sixteen_block_heads(env):
     stats = compare_lists(L, lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy(), oracle_lists(L), tag="C2 shape, 16 BLOCK_TOPK heads")
     print("16 block heads near-ties:", stats)
     assert stats["tie_floored"] <= 1e-3 * stats["entries"]
+
+
+def test_union_lists_topk_with_stride(env):
+    """SURVEY 8(f) NEXT-4, PAPER.md:L263 "combining Top-K with uniform striding": two saf3r_select calls (correspondence rules;
+    uniform-stride rules), saf3r_union_lists, attention over the union.  The union against the oracle's set union of the ORACLE's
+    lists (bit-exact, rows ascending and unique, saf3r_check_lists clean), the attention against the oracle on those lists; a too
+    small output buffer is reported through the total in row_ptr[H*NB] and nothing is written past it."""
+    sf, ctx, torch = env
+    sh = sy.Shape(S=6, G=16, H=4, D=64, B=64)                    # T = 261, N = 1566, NB = 25
+    gens = [sy.GEN_SAME_POSITION, sy.GEN_SAME_POSITION, sy.GEN_SINK, sy.GEN_UNIFORM]
+    topk = [sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=4),
+            sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_PER_FRAME, topk_per_frame=1, score_mode=sy.SCORE_COSINE),
+            sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=6),
+            sy.cfg(type=sy.HEAD_STATIC, static_mode=sy.STATIC_FRAME_LOCAL)]
+    strd = [sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=4, offset=h % 4) for h in range(3)] + [sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=0, keep_blocks=7)]
+    L = sy.make_layer(sh, gens, topk, seed=101)
+    q, k, v = upload(L)
+    shape = c_shape(sf, sh)
+    la = ctx.select(q, k, shape, topk)
+    lb = ctx.select(q, k, shape, strd)
+    lu = ctx.union_lists(shape, la, lb)
+    out = ctx.sparse_attn(q, k, v, shape, lu, out_fp32=True)
+    torch.cuda.synchronize()
+    assert ctx.check_lists(shape, lu) == 0
+    rp, col = lu.row_ptr.cpu().numpy(), lu.col_idx.cpu().numpy()
+    for h in range(sh.H):
+        a = orc.select_head(L.q[h], L.k[h], sh.S, sh.T, sh.B, orc.make_cfg(**topk[h]))
+        b = orc.select_head(L.q[h], L.k[h], sh.S, sh.T, sh.B, orc.make_cfg(**strd[h]))
+        ru, cu = orc.union_lists(a.row_ptr, a.col_idx, b.row_ptr, b.col_idx, sh.NB)
+        r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
+        assert np.array_equal(r - r[0], ru) and np.array_equal(col[r[0]:r[-1]], cu), f"head {h}: union differs from the oracle"
+        ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, ru, cu)
+        check_attention(out[h].cpu().numpy(), ref, f"union head {h} ({gens[h]})")
+    total = int(rp[-1])
+    small = sf.Lists(torch.empty_like(lu.row_ptr), torch.full((total // 2 + 8,), -7, dtype=torch.int32, device="cuda"))
+    guard = small.col_idx[total // 2:]                            # capacity passed to the library stops before these 8 entries
+    ctx.union_lists(shape, la, lb, out=sf.Lists(small.row_ptr, small.col_idx[:total // 2]))
+    torch.cuda.synchronize()
+    assert int(small.row_ptr[-1].item()) == total > total // 2 and bool((guard == -7).all())

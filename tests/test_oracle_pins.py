@@ -507,3 +507,47 @@ def test_p16_token_probe_is_column_mean_of_scores_and_topk_order():
     rank7 = int(np.nonzero(order == 7)[0][0])
     idx2, _ = orc.token_probe_topk(q, k, rank7 + 2)
     assert 7 in idx2 and 40 in idx2 and 41 not in idx2 and 99 not in idx2
+
+
+# ---------------------------------------------------------------- P17 (NEXT-4: Top-K U stride)
+def test_p17_union_lists_is_the_set_union():
+    """orc_union_lists against numpy's union1d (a library routine) row by row on random ascending lists, with empty rows; the
+    algebra of a union (idempotent, commutative, identity = empty lists, |A U B| = |A| + |B| - |A n B|); and the case the paper
+    names ("combining Top-K with uniform striding"): block top-k lists U stride lists of the same head contain both,
+    and the attention over the union equals the brute-force masked attention with mask_topk OR mask_stride."""
+    rng = np.random.default_rng(17)
+    NB, rows = 37, 23
+
+    def rand_lists():
+        rp, cols = [0], []
+        for _ in range(rows):
+            n = int(rng.integers(0, NB + 1)) if rng.random() > 0.2 else 0
+            cols.append(np.sort(rng.choice(NB, n, replace=False)).astype(np.int32))
+            rp.append(rp[-1] + n)
+        return np.array(rp, np.int64), (np.concatenate(cols) if cols else np.zeros(0, np.int32))
+
+    (ra, ca), (rb, cb) = rand_lists(), rand_lists()
+    ro, co = orc.union_lists(ra, ca, rb, cb, NB)
+    inter = 0
+    for I in range(rows):
+        a, b = ca[ra[I]:ra[I + 1]], cb[rb[I]:rb[I + 1]]
+        assert np.array_equal(co[ro[I]:ro[I + 1]], np.union1d(a, b))
+        inter += len(np.intersect1d(a, b))
+    assert len(co) == len(ca) + len(cb) - inter
+    r2, c2 = orc.union_lists(rb, cb, ra, ca, NB)
+    assert np.array_equal(r2, ro) and np.array_equal(c2, co)                       # commutative
+    r3, c3 = orc.union_lists(ra, ca, ra, ca, NB)
+    assert np.array_equal(r3, ra) and np.array_equal(c3, ca)                       # idempotent
+    r4, c4 = orc.union_lists(ra, ca, np.zeros(rows + 1, np.int64), np.zeros(0, np.int32), NB)
+    assert np.array_equal(r4, ra) and np.array_equal(c4, ca)                       # empty lists are the identity
+    # Top-K U stride on a tiny head, attention against the explicit OR of the two masks
+    S, T, B, D = 4, 23, 8, 8
+    N = S * T
+    q, k, v = rand_bits(rng, (N, D), 1.5), rand_bits(rng, (N, D), 1.5), rand_bits(rng, (N, D))
+    top = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=2)))
+    strd = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=4, offset=1)))
+    ru, cu = orc.union_lists(top.row_ptr, top.col_idx, strd.row_ptr, strd.col_idx, (N + B - 1) // B)
+    out, lse = orc.attn_lists(q, k, v, B, ru, cu)
+    mask = lists_to_mask(top.row_ptr, top.col_idx, N, B) | lists_to_mask(strd.row_ptr, strd.col_idx, N, B)
+    ref, ref_lse = brute_masked_attention(q, k, v, mask)
+    assert np.abs(out - ref).max() <= 2e-6 and np.abs(lse - ref_lse).max() <= 2e-6
