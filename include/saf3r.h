@@ -199,6 +199,21 @@ saf3r_status saf3r_token_set_attn(saf3r_ctx *ctx, const void *q_dev, const void 
                                   size_t workspace_bytes, void *out_dev, int out_is_fp32, float *lse_dev_or_null,
                                   void *cuda_stream);
 
+/* ---- Static kernel, "broadcast the first frame's local attention map" -----------------
+ * Reading (A18): the attention of a position head is content-independent and "fixed across all image blocks", so
+ * every T x T image block (f, g) of the N x N map is frame 0's local map P0 = softmax(Q0 K0^T / sqrt(D)) (rows normalised over
+ * the whole row: P0 / S).  Hence, for every frame f and in-frame position p,
+ *     o[f*T + p] = sum_p' P0[p][p'] * vbar[p'],   vbar[p'] = (1/S) sum_g v[g*T + p'],
+ * and lse[f*T + p] = ln sum_p' exp(q[p] . k[p'] / sqrt(D)) + ln S.  Cost O(T^2 D + N D) per head instead of O(N^2 D): logits are
+ * computed for frame 0 only and re-used for every frame pair.  Applies to ALL heads of the call (fold the position heads of a
+ * layer into one call through the strides).  q, k, v, out, lse as in saf3r_dense_attn; workspace_dev: device scratch of
+ * saf3r_static_broadcast_workspace_bytes(shape) bytes, 16-byte aligned (K0 copy, vbar in bf16, frame 0's lse).  Three launches
+ * (+ the key-norm pass of the attention kernel); enqueues and returns. */
+saf3r_status saf3r_static_broadcast_workspace_bytes(const saf3r_shape *shape, size_t *bytes);
+saf3r_status saf3r_static_broadcast_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const void *v_dev,
+                                         const saf3r_shape *shape, void *workspace_dev, size_t workspace_bytes, void *out_dev,
+                                         int out_is_fp32, float *lse_dev_or_null, void *cuda_stream);
+
 /* Measurement aid ("select ms split into pool and score+select stages").  When enabled, saf3r_select records
  * CUDA events on its stream before the pool launch, between the two launches and after the select launch (three
  * cudaEventRecord calls, no synchronisation).  saf3r_last_select_stage_ms blocks until the last timed saf3r_select has

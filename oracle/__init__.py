@@ -56,6 +56,7 @@ def lib():
         L.orc_attn_dense.argtypes = [vp, vp, vp, i64, i32, i64, i64, vp, vp]
         L.orc_attn_tokens.argtypes = [vp, vp, vp, i64, i32, vp, i64, i64, i64, vp, vp]
         L.orc_token_probe.argtypes = [vp, vp, i64, i32, vp]
+        L.orc_attn_broadcast_frame0.argtypes = [vp, vp, vp, i64, i64, i32, vp, vp]
         L.orc_union_lists.argtypes = [vp, vp, vp, vp, i64, i64, vp, vp, i64]
         L.orc_union_lists.restype = i64
         L.orc_nmse.argtypes = [vp, vp, i64]
@@ -201,6 +202,18 @@ def token_probe_topk(q_bits, k_bits, K: int):
     p = token_probe(q_bits, k_bits)
     keep = topn(p, K, use_sort=True)
     return keep.astype(np.int64), p
+
+
+def attn_broadcast_frame0(q_bits, k_bits, v_bits, S: int, T: int):
+    """Static kernel broadcasting frame 0's local attention map to every frame pair (reading A18):
+    returns (out [N][D] fp32, lse [N] fp32)."""
+    q, k, v = _u16(q_bits), _u16(k_bits), _u16(v_bits)
+    N, D = q.shape
+    assert N == S * T
+    out = np.empty((N, D), np.float32)
+    lse = np.empty((N,), np.float32)
+    lib().orc_attn_broadcast_frame0(_p(q), _p(k), _p(v), S, T, D, _p(out), _p(lse))
+    return out, lse
 
 
 def union_lists(row_ptr_a, col_a, row_ptr_b, col_b, NB: int):

@@ -408,6 +408,40 @@ void orc_token_probe(const uint16_t *q, const uint16_t *k, int64_t N, int32_t D,
   free(qbar);
 }
 
+/* ---- Static kernel, "broadcasting the first frame's local attention map to other frames" ----
+ * DESIGN.md reading A18: position heads are content-independent with a pattern "fixed across all image blocks", so
+ * every T x T image block (f, g) of the N x N attention map carries frame 0's local logits z0[p][p'] = q_{0,p} . k_{0,p'} / sqrt(D).
+ * Softmax over the whole row (all S*T keys) of that map gives the weight P0[p][p'] / S on key (g, p'), P0 = softmax_p'(z0), hence
+ *     o_{f,p} = sum_g sum_p' (P0[p][p'] / S) v_{g,p'}          for every frame f,
+ *     lse_{f,p} = ln( S * sum_p' exp(z0[p][p']) ).
+ * Written as the double sum over (g, p') exactly as it reads (no pre-averaging of V).  out [N][D] fp32, lse [N] fp32 or NULL. */
+void orc_attn_broadcast_frame0(const uint16_t *q, const uint16_t *k, const uint16_t *v, int64_t S, int64_t T, int32_t D, float *out,
+                               float *lse) {
+  const double inv_sqrt_d = 1.0 / sqrt((double)D);
+#pragma omp parallel for schedule(dynamic, 8)
+  for (int64_t p = 0; p < T; ++p) {
+    double *w = (double *)malloc(sizeof(double) * (size_t)T);
+    double zmax = -INFINITY;
+    for (int64_t pp = 0; pp < T; ++pp) {
+      double dot = 0.0;
+      for (int d = 0; d < D; ++d) dot += (double)bf16_to_f32(q[p * D + d]) * (double)bf16_to_f32(k[pp * D + d]);
+      w[pp] = dot * inv_sqrt_d;
+      if (w[pp] > zmax) zmax = w[pp];
+    }
+    double denom = 0.0;
+    for (int64_t pp = 0; pp < T; ++pp) { w[pp] = exp(w[pp] - zmax); denom += w[pp]; }
+    for (int d = 0; d < D; ++d) {
+      double o = 0.0;
+      for (int64_t g = 0; g < S; ++g)
+        for (int64_t pp = 0; pp < T; ++pp) o += (w[pp] / (denom * (double)S)) * (double)bf16_to_f32(v[(g * T + pp) * D + d]);
+      for (int64_t f = 0; f < S; ++f) out[(f * T + p) * D + d] = (float)o;
+    }
+    if (lse)
+      for (int64_t f = 0; f < S; ++f) lse[f * T + p] = (float)(zmax + log(denom * (double)S));
+    free(w);
+  }
+}
+
 /* ---- union of block lists ("combining Top-K with uniform striding") ----------------------
  * out(I) = a(I) U b(I) for every row I, by the definition of a set union: J is kept iff it is in a's row or in b's row.
  * Rows are emitted ascending.  Returns the number of entries, or -(needed) if capacity is too small. */

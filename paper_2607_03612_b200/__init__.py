@@ -27,7 +27,8 @@ SCORE_DOT, SCORE_COSINE = range(2)
 EXPORTS = ("saf3r_create", "saf3r_destroy", "saf3r_last_error", "saf3r_query_sizes", "saf3r_select", "saf3r_sparse_attn",
            "saf3r_dense_attn", "saf3r_layer_host_scratch_bytes", "saf3r_layer_host", "saf3r_launch_count",
            "saf3r_set_stage_timing", "saf3r_last_select_stage_ms", "saf3r_select_cached", "saf3r_token_stride_attn",
-           "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn", "saf3r_check_lists", "saf3r_select_plan", "saf3r_union_lists")
+           "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn", "saf3r_check_lists", "saf3r_select_plan", "saf3r_union_lists",
+           "saf3r_static_broadcast_workspace_bytes", "saf3r_static_broadcast_attn")
 
 
 class Saf3rError(RuntimeError):
@@ -83,6 +84,8 @@ def load_library():
         L.saf3r_layer_host.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), vp, C.c_size_t, vp, vp]
         L.saf3r_select_plan.argtypes = [vp, C.POINTER(ShapeC), C.POINTER(HeadCfg), C.POINTER(C.c_int32), C.POINTER(C.c_size_t)]
         L.saf3r_union_lists.argtypes = [vp, C.POINTER(ShapeC), C.POINTER(ListsC), C.POINTER(ListsC), C.POINTER(ListsC), vp]
+        L.saf3r_static_broadcast_workspace_bytes.argtypes = [C.POINTER(ShapeC), C.POINTER(C.c_size_t)]
+        L.saf3r_static_broadcast_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), vp, C.c_size_t, vp, i32, vp, vp]
         L.saf3r_launch_count.argtypes = [vp]
         L.saf3r_launch_count.restype = i64
         L.saf3r_set_stage_timing.argtypes = [vp, i32]
@@ -299,6 +302,23 @@ class Context:
         self._check(self.lib.saf3r_token_set_attn(self.h, q.data_ptr(), k.data_ptr(), v.data_ptr(), C.byref(shape), idx.data_ptr(), K,
                                                   workspace.data_ptr(), workspace.numel(), out.data_ptr(), int(out_fp32),
                                                   lse.data_ptr() if lse is not None else None, _stream_ptr(stream)))
+        return (out, lse) if want_lse else out
+
+    # ---- saf3r_static_broadcast_attn
+    def static_broadcast_attn(self, q, k, v, shape: ShapeC, workspace=None, out=None, out_fp32=False, want_lse=False, stream=None):
+        """Static kernel that broadcasts frame 0's local attention map to every frame pair."""
+        import torch
+        b = C.c_size_t()
+        st = self.lib.saf3r_static_broadcast_workspace_bytes(C.byref(shape), C.byref(b))
+        if st != OK:
+            raise Saf3rError(st, "saf3r_static_broadcast_workspace_bytes rejected the shape")
+        if workspace is None:
+            workspace = torch.empty(int(b.value), dtype=torch.uint8, device=q.device)
+            _on_stream(stream, workspace)
+        out, lse = self._out_lse(q, shape, out, out_fp32, want_lse, stream)
+        self._check(self.lib.saf3r_static_broadcast_attn(self.h, q.data_ptr(), k.data_ptr(), v.data_ptr(), C.byref(shape),
+                                                         workspace.data_ptr(), workspace.numel(), out.data_ptr(), int(out_fp32),
+                                                         lse.data_ptr() if lse is not None else None, _stream_ptr(stream)))
         return (out, lse) if want_lse else out
 
     # ---- saf3r_layer_host

@@ -715,6 +715,59 @@ saf3r_status saf3r_token_set_attn(saf3r_ctx *ctx, const void *q, const void *k, 
   return attn_common(ctx, q, kc, vc, shape, nullptr, out, out_is_fp32, lse, stream_, &kv);
 }
 
+// ------------------------------------------------------------------------------------------------ static broadcast (NEXT-4)
+struct BcastWs { size_t kc, vc, lse0, total; };
+static BcastWs bcast_ws(const SelGeom &g) {
+  BcastWs w;
+  size_t off = 0;
+  w.kc = off; off = align256(off + (size_t)g.H * g.T * 64 * 2);
+  w.vc = off; off = align256(off + (size_t)g.H * g.T * 64 * 2);
+  w.lse0 = off; off = align256(off + (size_t)g.H * g.T * sizeof(float));
+  w.total = off;
+  return w;
+}
+
+saf3r_status saf3r_static_broadcast_workspace_bytes(const saf3r_shape *shape, size_t *bytes) {
+  if (validate_shape(shape, false) || !bytes) return SAF3R_ERR_INVALID_ARG;
+  if (unsupported_shape(shape)) return SAF3R_ERR_UNSUPPORTED;
+  *bytes = bcast_ws(make_geom(shape)).total;
+  return SAF3R_OK;
+}
+
+saf3r_status saf3r_static_broadcast_attn(saf3r_ctx *ctx, const void *q, const void *k, const void *v, const saf3r_shape *shape, void *ws,
+                                         size_t ws_bytes, void *out, int out_is_fp32, float *lse, void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_shape(shape, true)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  if (!q || !k || !v || !ws || !out) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  if (((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out | (uintptr_t)ws) & 15)
+    return fail(ctx, SAF3R_ERR_INVALID_ARG, "q/k/v/out/workspace must be 16-byte aligned");
+  const SelGeom g = make_geom(shape);
+  const BcastWs w = bcast_ws(g);
+  if (ws_bytes < w.total) return fail(ctx, SAF3R_ERR_CAPACITY, "workspace too small (saf3r_static_broadcast_workspace_bytes)");
+  cudaStream_t st = (cudaStream_t)stream_;
+  __nv_bfloat16 *kc = (__nv_bfloat16 *)((uint8_t *)ws + w.kc), *vc = (__nv_bfloat16 *)((uint8_t *)ws + w.vc);
+  float *lse0 = (float *)((uint8_t *)ws + w.lse0);
+  frame_mean_kernel<<<dim3((g.T + 31) / 32, g.H, 2), 256, 0, st>>>((const __nv_bfloat16 *)k, (const __nv_bfloat16 *)v, kc, vc, g);
+  ctx->launches += 1;
+  CU_CHECK(cudaGetLastError());
+  // frame 0's rows of `out` = dense attention of (Q0, K0, vbar); the query geometry is the caller's with a single frame
+  saf3r_shape one = *shape;
+  one.num_frames = 1;
+  const KvGeom kv{g.T, (int64_t)g.T * 64, 64};
+  saf3r_status s = attn_common(ctx, q, kc, vc, &one, nullptr, out, out_is_fp32, lse ? lse0 : nullptr, stream_, &kv);
+  if (s != SAF3R_OK) return s;
+  if (g.S > 1 || lse) {
+    const int elem = out_is_fp32 ? 4 : 2, rows = 256 / (4 * elem);
+    frame_broadcast_kernel<<<dim3((g.T + rows - 1) / rows, g.S, g.H), 256, 0, st>>>((uint8_t *)out, lse, lse0, g, shape->stride_head,
+                                                                                   shape->stride_token, elem);
+    ctx->launches += 1;
+    CU_CHECK(cudaGetLastError());
+  }
+  return SAF3R_OK;
+}
+
 // saf3r_layer_host pipelines the layer over groups of heads (heads are independent): the host->device copy of
 // group g+1 runs under the select + attention of group g, and the device->host copy of group g under the compute of group
 // g+1 (separate copy engines), on ctx-owned side streams forked from / joined to the caller's stream with events.

@@ -13,6 +13,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "ptx.cuh"
 #include "select_kernels.cuh"
 
 namespace saf3r {
@@ -262,6 +263,67 @@ __global__ void __launch_bounds__(256) token_gather_kernel(const __nv_bfloat16 *
   const __nv_bfloat16 *src = (blockIdx.z ? v : k) + (int64_t)h * g.stride_head + t * g.stride_token + sub * 8;
   __nv_bfloat16 *dst = (blockIdx.z ? vc : kc) + ((int64_t)h * K + i) * 64 + sub * 8;
   *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
+}
+
+// ------------------------------------------------------------------------------------------------ static broadcast (NEXT-4)
+// Static kernel, second pattern of PAPER.md:L96 ("broadcasting the first frame's local attention map to other frames for
+// cross-view interaction"; DESIGN reading A18): every T x T image block of the N x N attention map equals frame 0's local map
+// P0 = softmax(Q0 K0^T / sqrt(D)), so a query at (frame f, position p) gets o = sum_p' P0[p][p'] * vbar[p'] with
+// vbar[p'] = (1/S) sum_g v[g][p'] - the same row for every frame.  O(T^2 D + N D) instead of O(N^2 D).
+//   frame_mean_kernel       vbar (bf16, RNE) and a compact copy of K0: grid (ceil(T/32), H, 2), 8 lanes per token row
+//   (dense mode of saf3r_attn_kernel over (Q0, K0, vbar) writes frame 0's rows of out)
+//   frame_broadcast_kernel  frame 0's rows of out (and lse) -> frames 1..S-1
+__global__ void __launch_bounds__(256) frame_mean_kernel(const __nv_bfloat16 *__restrict__ k, const __nv_bfloat16 *__restrict__ v,
+                                                         __nv_bfloat16 *__restrict__ kc, __nv_bfloat16 *__restrict__ vc, SelGeom g) {
+  const int h = blockIdx.y, sub = threadIdx.x & 7, row = threadIdx.x >> 3;
+  const int p = blockIdx.x * 32 + row;
+  if (p >= g.T) return;
+  __nv_bfloat16 *dst = (blockIdx.z ? vc : kc) + ((int64_t)h * g.T + p) * 64 + sub * 8;
+  if (blockIdx.z == 0) {
+    *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(k + (int64_t)h * g.stride_head + (int64_t)p * g.stride_token + sub * 8);
+    return;
+  }
+  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  const __nv_bfloat16 *src = v + (int64_t)h * g.stride_head + (int64_t)p * g.stride_token + sub * 8;
+  for (int f0 = 0; f0 < g.S; f0 += 8) {  // frames in order, eight loads in flight
+    uint4 raw[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      raw[i] = make_uint4(0, 0, 0, 0);
+      if (f0 + i < g.S) raw[i] = ld_stream_16(src + (int64_t)(f0 + i) * g.T * g.stride_token);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      float x[8];
+      bf16x8_to_f32(raw[i], x);
+#pragma unroll
+      for (int c = 0; c < 8; ++c) acc[c] += x[c];
+    }
+  }
+  const float inv = 1.f / (float)g.S;
+  uint4 o;
+  o.x = pack_bf16x2(acc[0] * inv, acc[1] * inv);
+  o.y = pack_bf16x2(acc[2] * inv, acc[3] * inv);
+  o.z = pack_bf16x2(acc[4] * inv, acc[5] * inv);
+  o.w = pack_bf16x2(acc[6] * inv, acc[7] * inv);
+  *reinterpret_cast<uint4 *>(dst) = o;
+}
+
+// grid (ceil(T / rows), S, H), rows = 256 / (16-byte chunks per output row: 8 for bf16, 16 for fp32).  Frames f >= 1 copy frame
+// 0's output row; every frame's lse = lse0 + ln S (the partition function of the full row is S times frame 0's).
+__global__ void __launch_bounds__(256) frame_broadcast_kernel(uint8_t *__restrict__ out, float *__restrict__ lse, const float *__restrict__ lse0,
+                                                              SelGeom g, int64_t out_stride_head, int64_t out_stride_token, int elem_bytes) {
+  const int h = blockIdx.z, f = blockIdx.y;
+  const int chunks = 4 * elem_bytes;
+  const int rows_per_cta = 256 / chunks;
+  const int p = blockIdx.x * rows_per_cta + threadIdx.x / chunks, c = threadIdx.x % chunks;
+  if (p >= g.T) return;
+  if (f >= 1) {
+    const uint8_t *src = out + ((int64_t)h * out_stride_head + (int64_t)p * out_stride_token) * elem_bytes + c * 16;
+    uint8_t *dst = out + ((int64_t)h * out_stride_head + ((int64_t)f * g.T + p) * out_stride_token) * elem_bytes + c * 16;
+    *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
+  }
+  if (lse != nullptr && c == 0) lse[(int64_t)h * g.N + (int64_t)f * g.T + p] = lse0[(int64_t)h * g.T + p] + logf((float)g.S);
 }
 
 }  // namespace saf3r

@@ -710,3 +710,23 @@ def test_union_lists_topk_with_stride(env):
     ctx.union_lists(shape, la, lb, out=sf.Lists(small.row_ptr, small.col_idx[:total // 2]))
     torch.cuda.synchronize()
     assert int(small.row_ptr[-1].item()) == total > total // 2 and bool((guard == -7).all())
+
+
+@pytest.mark.parametrize("S,G,B,H", [(4, 16, 64, 3), (7, 17, 128, 2), (1, 17, 128, 1), (20, 37, 128, 2)])
+def test_static_broadcast_attn_matches_oracle(env, S, G, B, H):
+    """the static kernel that broadcasts frame 0's local attention map to every frame pair,
+    against orc_attn_broadcast_frame0 (fp32 output + lse; bf16 output loosely); S = 1 degenerates to dense attention of frame 0."""
+    sf, ctx, torch = env
+    gens = [sy.GEN_SAME_POSITION, sy.GEN_FRAME_LOCAL, sy.GEN_UNIFORM][:H]
+    L = small_layer(S, G, H, B, gens, [sy.cfg(type=sy.HEAD_DENSE)] * H, seed=111)
+    sh = L.shape
+    q, k, v = upload(L)
+    shape = c_shape(sf, sh)
+    out, lse = ctx.static_broadcast_attn(q, k, v, shape, out_fp32=True, want_lse=True)
+    out_bf = ctx.static_broadcast_attn(q, k, v, shape)
+    torch.cuda.synchronize()
+    for h in range(H):
+        ref, ref_lse = orc.attn_broadcast_frame0(L.q[h], L.k[h], L.v[h], sh.S, sh.T)
+        check_attention(out[h].cpu().numpy(), ref, f"broadcast head {h} ({gens[h]}) S={S}")
+        assert np.abs(lse[h].cpu().numpy() - ref_lse).max() <= 1e-2
+        assert np.abs(out_bf[h].float().cpu().numpy() - ref).max() <= 2e-2

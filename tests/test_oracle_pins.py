@@ -551,3 +551,36 @@ def test_p17_union_lists_is_the_set_union():
     mask = lists_to_mask(top.row_ptr, top.col_idx, N, B) | lists_to_mask(strd.row_ptr, strd.col_idx, N, B)
     ref, ref_lse = brute_masked_attention(q, k, v, mask)
     assert np.abs(out - ref).max() <= 2e-6 and np.abs(lse - ref_lse).max() <= 2e-6
+
+
+# ---------------------------------------------------------------- P18 (NEXT-4: static broadcast of frame 0's local map)
+def test_p18_broadcast_of_frame0_local_map():
+    """orc_attn_broadcast_frame0 (reading A18) against: (a) the explicit N x N matrix whose every T x T image block
+    is frame 0's unnormalised map, row-normalised, times V (numpy float64 brute force); (b) S = 1: the separately written dense
+    function on frame 0; (c) V identical in every frame: frame 0's dense local attention, for every frame; (d) rows sum to one
+    (V = 1 gives 1) and the output does not depend on the queries or keys of frames >= 1."""
+    rng = np.random.default_rng(18)
+    S, T, D = 4, 23, 8
+    N = S * T
+    q, k, v = rand_bits(rng, (N, D), 1.5), rand_bits(rng, (N, D), 1.5), rand_bits(rng, (N, D))
+    out, lse = orc.attn_broadcast_frame0(q, k, v, S, T)
+    qf, kf, vf = (sy.bf16_bits_to_f32(x).astype(np.float64) for x in (q, k, v))
+    z0 = qf[:T] @ kf[:T].T / np.sqrt(D)
+    A = np.tile(np.exp(z0 - z0.max(axis=1, keepdims=True)), (S, S))                # every image block = frame 0's block
+    A /= A.sum(axis=1, keepdims=True)
+    assert np.abs(out - A @ vf).max() <= 2e-6
+    ref_lse = np.tile(np.log(np.exp(z0).sum(axis=1) * S), S)
+    assert np.abs(lse - ref_lse).max() <= 2e-6
+    o1, l1 = orc.attn_broadcast_frame0(q[:T], k[:T], v[:T], 1, T)                    # (b)
+    o2, l2 = orc.attn_dense(q[:T], k[:T], v[:T])
+    assert np.abs(o1 - o2).max() <= 1e-6 and np.abs(l1 - l2).max() <= 1e-5
+    vrep = np.tile(v[:T], (S, 1))                                                    # (c)
+    o3, _ = orc.attn_broadcast_frame0(q, k, vrep, S, T)
+    assert np.abs(o3 - np.tile(o2, (S, 1))).max() <= 1e-6
+    ones = sy.f32_to_bf16_bits(np.ones((N, D), np.float32))                          # (d)
+    o4, _ = orc.attn_broadcast_frame0(q, k, ones, S, T)
+    assert np.abs(o4 - 1.0).max() <= 1e-6
+    q2, k2 = q.copy(), k.copy()
+    q2[T:], k2[T:] = rand_bits(rng, (N - T, D)), rand_bits(rng, (N - T, D))
+    o5, _ = orc.attn_broadcast_frame0(q2, k2, v, S, T)
+    assert np.array_equal(o5, out)
