@@ -56,6 +56,9 @@ def lib():
         L.orc_attn_dense.argtypes = [vp, vp, vp, i64, i32, i64, i64, vp, vp]
         L.orc_attn_tokens.argtypes = [vp, vp, vp, i64, i32, vp, i64, i64, i64, vp, vp]
         L.orc_token_probe.argtypes = [vp, vp, i64, i32, vp]
+        L.orc_token_topk_per_frame.argtypes = [vp, i64, i64, i32, i64, i64, i64, vp]
+        L.orc_token_cosine_row.argtypes = [vp, i64, i32, i64, vp]
+        L.orc_attn_token_lists.argtypes = [vp, vp, vp, i64, i32, vp, i64, i64, i64, vp, vp]
         L.orc_attn_broadcast_frame0.argtypes = [vp, vp, vp, i64, i64, i32, vp, vp]
         L.orc_union_lists.argtypes = [vp, vp, vp, vp, i64, i64, vp, vp, i64]
         L.orc_union_lists.restype = i64
@@ -202,6 +205,39 @@ def token_probe_topk(q_bits, k_bits, K: int):
     p = token_probe(q_bits, k_bits)
     keep = topn(p, K, use_sort=True)
     return keep.astype(np.int64), p
+
+
+def token_topk_per_frame(feat_bits, S: int, T: int, K: int, i0: int = 0, i1: int | None = None) -> np.ndarray:
+    """Token-wise DINO Top-K (PAPER.md:L100, L126): for the queries [i0, i1) the K most cosine-similar tokens of EVERY frame;
+    returns int32 [(i1 - i0)][S][K] global token indices, ascending."""
+    f = _u16(feat_bits)
+    N, D = f.shape
+    assert N == S * T and 1 <= K <= T
+    i1 = N if i1 is None else i1
+    out = np.empty((i1 - i0, S, K), np.int32)
+    lib().orc_token_topk_per_frame(_p(f), S, T, D, K, i0, i1, _p(out))
+    return out
+
+
+def token_cosine_row(feat_bits, i: int) -> np.ndarray:
+    f = _u16(feat_bits)
+    N, D = f.shape
+    out = np.empty((N,), np.float32)
+    lib().orc_token_cosine_row(_p(f), N, D, i, _p(out))
+    return out
+
+
+def attn_token_lists(q_bits, k_bits, v_bits, idx: np.ndarray, i0: int = 0, i1: int | None = None):
+    """Attention with per-query key lists: idx int32 [(i1 - i0)][L] (negative = padding).  Returns (out [N][D], lse [N]); rows
+    outside [i0, i1) are NaN."""
+    q, k, v = _u16(q_bits), _u16(k_bits), _u16(v_bits)
+    N, D = q.shape
+    i1 = N if i1 is None else i1
+    idx = np.ascontiguousarray(idx, np.int32).reshape(i1 - i0, -1)
+    out = np.full((N, D), np.nan, np.float32)
+    lse = np.full((N,), np.nan, np.float32)
+    lib().orc_attn_token_lists(_p(q), _p(k), _p(v), N, D, _p(idx), idx.shape[1], i0, i1, _p(out), _p(lse))
+    return out, lse
 
 
 def attn_broadcast_frame0(q_bits, k_bits, v_bits, S: int, T: int):

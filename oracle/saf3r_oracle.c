@@ -16,8 +16,9 @@
  *
  * Citations are PAPER.md line numbers and DESIGN.md readings.
  *
- * Parity pins: every function below is pinned by tests/test_oracle_pins.py (P1..P16 of
- * DESIGN.md; P14-P16 pin the token-granular functions orc_attn_tokens / orc_token_probe).  Unpinned *choices* (not arithmetic): POSITION_BAND radius and the
+ * Parity pins: every function below is pinned by tests/test_oracle_pins.py (P1..P19 of
+ * DESIGN.md; P14-P16 pin orc_attn_tokens / orc_token_probe, P17 orc_union_lists, P18 orc_attn_broadcast_frame0,
+ * P19 orc_token_topk_per_frame / orc_token_cosine_row / orc_attn_token_lists).  Unpinned *choices* (not arithmetic): POSITION_BAND radius and the
  * DOT-vs-COSINE default for correspondence heads -- "parity unpinned" for those choices.
  */
 #include <math.h>
@@ -406,6 +407,109 @@ void orc_token_probe(const uint16_t *q, const uint16_t *k, int64_t N, int32_t D,
     p[j] = (float)(dot * inv_sqrt_d);
   }
   free(qbar);
+}
+
+/* ---- DINO Top-K kernel, TOKEN-WISE (Tab. 6/7 L241-249) ------------------
+ * "we pre-compute the cosine similarity between each patch token and all other patch tokens using the DINO features, and select
+ * the Top-K most similar tokens from each frame as the keys and values for attention" (L100); "compute the global cosine similarity
+ * between all patches, storing the indices of the per-frame Top-K matched patches ... token-wise ... exact token-level
+ * similarities" (L126).  feat: per-sequence features [N][D] bf16 bits (the encoder's last-block output; shared by heads and layers).
+ * For query token i and every frame g: cos_ij = (f_i . f_j) / (|f_i| |f_j|) for the T tokens j of frame g (0 if a norm < 1e-20),
+ * double accumulation, stored fp32; keep the K best under (score desc, index asc); emit ascending.
+ * DESIGN.md reading A19: every token of every frame is a candidate, the query's own frame and the query itself included
+ * (cos = 1 ranks it first in its own frame); special tokens are ordinary tokens (reading A7).  Requires 1 <= K <= T.
+ * idx_out: int32 [(i1 - i0)][S][K], global token indices.  Rows i in [i0, i1). */
+void orc_token_topk_per_frame(const uint16_t *feat, int64_t S, int64_t T, int32_t D, int64_t K, int64_t i0, int64_t i1,
+                              int32_t *idx_out) {
+  const int64_t N = S * T;
+  double *nrm = (double *)malloc(sizeof(double) * (size_t)N);
+  for (int64_t t = 0; t < N; ++t) {
+    double nn = 0.0;
+    for (int d = 0; d < D; ++d) { double x = bf16_to_f32(feat[t * D + d]); nn += x * x; }
+    nrm[t] = sqrt(nn);
+  }
+#pragma omp parallel for schedule(dynamic, 4)
+  for (int64_t i = i0; i < i1; ++i) {
+    float *cosr = (float *)malloc(sizeof(float) * (size_t)T);
+    int32_t *cand = (int32_t *)malloc(sizeof(int32_t) * (size_t)T);
+    uint8_t *keep = (uint8_t *)malloc((size_t)T);
+    for (int64_t g = 0; g < S; ++g) {
+      for (int64_t p = 0; p < T; ++p) {
+        const int64_t j = g * T + p;
+        double dot = 0.0;
+        for (int d = 0; d < D; ++d) dot += (double)bf16_to_f32(feat[i * D + d]) * (double)bf16_to_f32(feat[j * D + d]);
+        const double den = nrm[i] * nrm[j];
+        cosr[p] = (nrm[i] < 1e-20 || nrm[j] < 1e-20) ? 0.0f : (float)(dot / den);
+        cand[p] = (int32_t)p;
+        keep[p] = 0;
+      }
+      topn_mark_sorted(cosr, cand, T, K, keep);
+      int64_t c = 0;
+      for (int64_t p = 0; p < T; ++p)
+        if (keep[p]) idx_out[((i - i0) * S + g) * K + c++] = (int32_t)(g * T + p);
+    }
+    free(cosr); free(cand); free(keep);
+  }
+  free(nrm);
+}
+
+/* the cosine row of one query against ALL tokens (for the near-tie rule of the GPU-vs-oracle comparison and for pin P19) */
+void orc_token_cosine_row(const uint16_t *feat, int64_t N, int32_t D, int64_t i, float *cos_out) {
+  double ni = 0.0;
+  for (int d = 0; d < D; ++d) { double x = bf16_to_f32(feat[i * D + d]); ni += x * x; }
+  ni = sqrt(ni);
+  for (int64_t j = 0; j < N; ++j) {
+    double nj = 0.0, dot = 0.0;
+    for (int d = 0; d < D; ++d) {
+      double x = bf16_to_f32(feat[j * D + d]);
+      nj += x * x;
+      dot += (double)bf16_to_f32(feat[i * D + d]) * x;
+    }
+    nj = sqrt(nj);
+    cos_out[j] = (ni < 1e-20 || nj < 1e-20) ? 0.0f : (float)(dot / (ni * nj));
+  }
+}
+
+/* O4 with PER-QUERY key lists ("... as the keys and values for attention"): query i (rows [i0, i1)) attends the key
+ * tokens idx[(i - i0) * L + 0 .. L); entries < 0 are padding and ignored.  o_i = sum_j softmax_j(q_i.k_j / sqrt(D)) v_j over its
+ * list; an empty list gives o_i = 0, lse_i = -inf.  Two passes, as the formulas read. */
+void orc_attn_token_lists(const uint16_t *q, const uint16_t *k, const uint16_t *v, int64_t N, int32_t D, const int32_t *idx, int64_t L,
+                          int64_t i0, int64_t i1, float *out, float *lse) {
+  const double scale = 1.0 / sqrt((double)D);
+  (void)N;
+#pragma omp parallel for schedule(dynamic, 8)
+  for (int64_t i = i0; i < i1; ++i) {
+    const int32_t *row = idx + (i - i0) * L;
+    double m = -INFINITY;
+    int64_t nk = 0;
+    for (int64_t e = 0; e < L; ++e) {
+      if (row[e] < 0) continue;
+      const int64_t j = row[e];
+      double z = 0.0;
+      for (int d = 0; d < D; ++d) z += (double)bf16_to_f32(q[i * D + d]) * (double)bf16_to_f32(k[j * D + d]);
+      z *= scale;
+      if (z > m) m = z;
+      ++nk;
+    }
+    if (nk == 0) {
+      for (int d = 0; d < D; ++d) out[i * D + d] = 0.0f;
+      if (lse) lse[i] = -INFINITY;
+      continue;
+    }
+    double l = 0.0, acc[256];
+    for (int d = 0; d < D; ++d) acc[d] = 0.0;
+    for (int64_t e = 0; e < L; ++e) {
+      if (row[e] < 0) continue;
+      const int64_t j = row[e];
+      double z = 0.0;
+      for (int d = 0; d < D; ++d) z += (double)bf16_to_f32(q[i * D + d]) * (double)bf16_to_f32(k[j * D + d]);
+      const double w = exp(z * scale - m);
+      l += w;
+      for (int d = 0; d < D; ++d) acc[d] += w * (double)bf16_to_f32(v[j * D + d]);
+    }
+    for (int d = 0; d < D; ++d) out[i * D + d] = (float)(acc[d] / l);
+    if (lse) lse[i] = (float)(m + log(l));
+  }
 }
 
 /* ---- Static kernel, "broadcasting the first frame's local attention map to other frames" ----

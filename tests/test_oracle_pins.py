@@ -584,3 +584,65 @@ def test_p18_broadcast_of_frame0_local_map():
     q2[T:], k2[T:] = rand_bits(rng, (N - T, D)), rand_bits(rng, (N - T, D))
     o5, _ = orc.attn_broadcast_frame0(q2, k2, v, S, T)
     assert np.array_equal(o5, out)
+
+
+# ---------------------------------------------------------------- P19 (NEXT-2 iii: token-wise per-frame Top-K)
+def test_p19_token_topk_per_frame_and_per_query_attention():
+    """orc_token_topk_per_frame / orc_token_cosine_row / orc_attn_token_lists against numpy:
+    (a) the cosine row equals the normalised float64 Gram matrix; (b) per query and per frame the kept set equals numpy's stable
+    argsort of (-cos) cut at K, with planted EXACT ties (duplicated feature rows) going to the lower index; (c) the kept fraction is
+    K/T, the paper's printed 0.2 % / 0.4 % for K = 2 / 4 (tests/golden/paper_key_fractions.txt, PAPER.md:L242, L249);
+    (d) K = T keeps every token and the per-query attention equals the separately written dense function; (e) the per-query
+    attention equals the brute-force masked softmax with the explicit N x N boolean mask; (f) identical lists for all queries
+    reduce to orc_attn_tokens; padding entries (-1) are ignored and an all-padding list gives 0 / -inf."""
+    rng = np.random.default_rng(19)
+    S, T, D, K = 4, 23, 8, 3
+    N = S * T
+    feat = rand_bits(rng, (N, D))
+    feat[T + 5] = feat[T + 2]                                   # exact ties inside frame 1 ...
+    feat[2 * T + 7] = feat[2 * T + 1]
+    feat[2 * T + 9] = feat[2 * T + 1]                           # ... and a triple inside frame 2
+    ff = sy.bf16_bits_to_f32(feat).astype(np.float64)
+    fn = ff / np.linalg.norm(ff, axis=1, keepdims=True)
+    G = fn @ fn.T
+    for i in (0, T + 2, N - 1):
+        assert np.abs(orc.token_cosine_row(feat, i) - G[i]).max() <= 1e-6                      # (a)
+    idx = orc.token_topk_per_frame(feat, S, T, K)
+    assert idx.shape == (N, S, K)
+    for i in range(N):
+        c32 = orc.token_cosine_row(feat, i)                    # ranking happens on the stored fp32 values
+        for g in range(S):
+            order = np.argsort(-c32[g * T:(g + 1) * T], kind="stable")[:K]
+            assert np.array_equal(idx[i, g], np.sort(order) + g * T), (i, g)                   # (b)
+            assert np.all(np.diff(idx[i, g]) > 0)
+        assert i in idx[i, i // T]                              # reading A19: the query itself is its own best match
+    # planted ties: for a query outside frame 2 with K = 1.. the lower index of an exact tie wins
+    one = orc.token_topk_per_frame(feat, S, T, 1)
+    i = 2 * T + 7                                               # its own frame holds two exact copies (indices 2T+1, 2T+7, 2T+9 all cos = 1)
+    assert one[i, 2, 0] == 2 * T + 1
+    lines = [l.split() for l in open(os.path.join(GOLD, "paper_key_fractions.txt")) if l.strip() and not l.startswith("#")]
+    gold = {l[0]: l[1:] for l in lines}                         # (c)
+    Tp = int(round(32 * 2 * float(gold["stride32_vs_k2_sparsity_ratio"][0])))   # (1/32) / (2/T) = 16  =>  T = 1024 (PAPER.md:L259)
+    for key, kk in (("topk_k2_fraction_percent", 2), ("topk_k4_fraction_percent", 4)):
+        full_count = orc.token_topk_per_frame(rand_bits(rng, (2 * Tp, D)), 2, Tp, kk, 0, 1).size    # keys of one query: S * K
+        assert abs(100.0 * full_count / (2 * Tp) - float(gold[key][0])) < 0.05
+    assert idx.shape[1] * idx.shape[2] / N == K / T
+    q, k, v = rand_bits(rng, (N, D), 1.5), rand_bits(rng, (N, D), 1.5), rand_bits(rng, (N, D))
+    full = orc.token_topk_per_frame(feat, S, T, T)              # (d)
+    assert np.array_equal(full.reshape(N, N), np.tile(np.arange(N, dtype=np.int32), (N, 1)))
+    o1, l1 = orc.attn_token_lists(q, k, v, full.reshape(N, -1))
+    o2, l2 = orc.attn_dense(q, k, v)
+    assert np.abs(o1 - o2).max() <= 1e-6 and np.abs(l1 - l2).max() <= 1e-5
+    mask = np.zeros((N, N), bool)                               # (e)
+    for i in range(N):
+        mask[i, idx[i].ravel()] = True
+    o3, l3 = orc.attn_token_lists(q, k, v, idx.reshape(N, -1))
+    ref, ref_lse = brute_masked_attention(q, k, v, mask)
+    assert np.abs(o3 - ref).max() <= 2e-6 and np.abs(l3 - ref_lse).max() <= 2e-6
+    same = np.sort(rng.choice(N, 11, replace=False)).astype(np.int32)                          # (f)
+    lists = np.tile(np.concatenate([same, [-1, -1]]).astype(np.int32), (N, 1))
+    o4, l4 = orc.attn_token_lists(q, k, v, lists)
+    o5, l5 = orc.attn_tokens(q, k, v, same.astype(np.int64))
+    assert np.abs(o4 - o5).max() <= 1e-6 and np.abs(l4 - l5).max() <= 1e-5
+    o6, l6 = orc.attn_token_lists(q, k, v, np.full((N, 4), -1, np.int32))
+    assert np.all(o6 == 0) and np.all(np.isneginf(l6))
