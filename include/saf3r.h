@@ -199,6 +199,44 @@ saf3r_status saf3r_token_set_attn(saf3r_ctx *ctx, const void *q_dev, const void 
                                   size_t workspace_bytes, void *out_dev, int out_is_fp32, float *lse_dev_or_null,
                                   void *cuda_stream);
 
+/* ---- Token-wise per-frame Top-K: the paper's primary definition of the DINO Top-K kernel (SURVEY 8(f) NEXT-2 iii) ----------------
+ * "we pre-compute the cosine similarity between each patch token and all other patch tokens using the DINO features, and select
+ * the Top-K most similar tokens from each frame as the keys and values for attention"; the indices are computed
+ * once per sequence, "cached and reused by all subsequent DINO Top-K kernels" (L126); K = 16..128 per frame (L161), K = 2 / 4
+ * attend 0.2 % / 0.4 % of the keys (L242, L249).  Reading A19: every token of every frame is a candidate, the query's
+ * own frame and the query itself included.
+ *
+ * saf3r_token_topk_select: features feat_dev [N][64] bf16 (per sequence, shared by heads and layers; shape->stride_token is the
+ *   row stride, num_heads / stride_head / block are ignored) -> idx_dev int32 [N][S][K]: for query token i and frame g the K tokens
+ *   of frame g with the largest cosine similarity (score desc, index asc), ascending.  The N x N similarity runs on the tensor
+ *   cores a strip of query tiles at a time (strip keys in the workspace); 1 + 2 * ceil(NB128 / strips) launches.
+ * saf3r_token_lists_count / _fill: turn idx into what the attention kernel consumes, per q-tile of `block` queries: the union of
+ *   its queries' keys, packed over the frames into tiles of `block` gathered key tokens (key_idx, -1 = padding), and one bit per
+ *   (query row, key column) of every tile (mask: [tile][block][block/32] uint32).  Tile counts depend on the data: _count writes
+ *   tile_ptr_dev[0 .. NB] (offsets; tile_ptr_dev[NB] = total tiles), the caller sizes key_idx (total * block int32) and mask from it
+ *   (or from the worst case *max_tiles of saf3r_token_topk_query_sizes) and calls _fill with the same tile_ptr.  A q-tile that does
+ *   not fit capacity_tiles is left unwritten.  Both depend only on idx: once per sequence, shared by all heads and layers.
+ * saf3r_token_lists_attn: o_i = sum_j softmax_j(q_i.k_j/sqrt(D)) v_j over the keys j of query i's own list: the block-sparse kernel
+ *   with K/V rows gathered by index (cp.async) and the bit mask applied before the row max; q, k, v, out, lse as in
+ *   saf3r_sparse_attn; the lists are shared by all heads of the call. */
+typedef struct {
+  int64_t *tile_ptr;       /* dev, [NB + 1]: tiles of q-tile I = [tile_ptr[I], tile_ptr[I+1]) */
+  int32_t *key_idx;        /* dev, [capacity_tiles * block]: gathered key token of every tile column, -1 = padding */
+  uint32_t *mask;          /* dev, [capacity_tiles][block][block/32]: bit c of row r = query r of the q-tile keeps column c */
+  int64_t capacity_tiles;
+} saf3r_token_lists;
+saf3r_status saf3r_token_topk_query_sizes(const saf3r_shape *shape, int32_t K, size_t *select_workspace_bytes, int64_t *idx_entries,
+                                          int64_t *max_tiles);
+saf3r_status saf3r_token_topk_select(saf3r_ctx *ctx, const void *feat_dev, const saf3r_shape *shape, int32_t K, void *workspace_dev,
+                                     size_t workspace_bytes, int32_t *idx_dev, void *cuda_stream);
+saf3r_status saf3r_token_lists_count(saf3r_ctx *ctx, const saf3r_shape *shape, int32_t K, const int32_t *idx_dev,
+                                     int64_t *tile_ptr_dev, void *cuda_stream);
+saf3r_status saf3r_token_lists_fill(saf3r_ctx *ctx, const saf3r_shape *shape, int32_t K, const int32_t *idx_dev,
+                                    const saf3r_token_lists *lists, void *cuda_stream);
+saf3r_status saf3r_token_lists_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_dev, const void *v_dev,
+                                    const saf3r_shape *shape, const saf3r_token_lists *lists, void *out_dev, int out_is_fp32,
+                                    float *lse_dev_or_null, void *cuda_stream);
+
 /* ---- Static kernel, "broadcast the first frame's local attention map" -----------------
  * Reading (A18): the attention of a position head is content-independent and "fixed across all image blocks", so
  * every T x T image block (f, g) of the N x N map is frame 0's local map P0 = softmax(Q0 K0^T / sqrt(D)) (rows normalised over

@@ -28,7 +28,8 @@ EXPORTS = ("saf3r_create", "saf3r_destroy", "saf3r_last_error", "saf3r_query_siz
            "saf3r_dense_attn", "saf3r_layer_host_scratch_bytes", "saf3r_layer_host", "saf3r_launch_count",
            "saf3r_set_stage_timing", "saf3r_last_select_stage_ms", "saf3r_select_cached", "saf3r_token_stride_attn",
            "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn", "saf3r_check_lists", "saf3r_select_plan", "saf3r_union_lists",
-           "saf3r_static_broadcast_workspace_bytes", "saf3r_static_broadcast_attn")
+           "saf3r_static_broadcast_workspace_bytes", "saf3r_static_broadcast_attn", "saf3r_token_topk_query_sizes",
+           "saf3r_token_topk_select", "saf3r_token_lists_count", "saf3r_token_lists_fill", "saf3r_token_lists_attn")
 
 
 class Saf3rError(RuntimeError):
@@ -50,6 +51,10 @@ class ShapeC(C.Structure):
 
 class ListsC(C.Structure):
     _fields_ = [("row_ptr", C.c_void_p), ("col_idx", C.c_void_p), ("capacity", C.c_int64)]
+
+
+class TokenListsC(C.Structure):
+    _fields_ = [("tile_ptr", C.c_void_p), ("key_idx", C.c_void_p), ("mask", C.c_void_p), ("capacity_tiles", C.c_int64)]
 
 
 _lib = None
@@ -86,6 +91,11 @@ def load_library():
         L.saf3r_union_lists.argtypes = [vp, C.POINTER(ShapeC), C.POINTER(ListsC), C.POINTER(ListsC), C.POINTER(ListsC), vp]
         L.saf3r_static_broadcast_workspace_bytes.argtypes = [C.POINTER(ShapeC), C.POINTER(C.c_size_t)]
         L.saf3r_static_broadcast_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), vp, C.c_size_t, vp, i32, vp, vp]
+        L.saf3r_token_topk_query_sizes.argtypes = [C.POINTER(ShapeC), C.c_int32, C.POINTER(C.c_size_t), C.POINTER(i64), C.POINTER(i64)]
+        L.saf3r_token_topk_select.argtypes = [vp, vp, C.POINTER(ShapeC), C.c_int32, vp, C.c_size_t, vp, vp]
+        L.saf3r_token_lists_count.argtypes = [vp, C.POINTER(ShapeC), C.c_int32, vp, vp, vp]
+        L.saf3r_token_lists_fill.argtypes = [vp, C.POINTER(ShapeC), C.c_int32, vp, C.POINTER(TokenListsC), vp]
+        L.saf3r_token_lists_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(TokenListsC), vp, i32, vp, vp]
         L.saf3r_launch_count.argtypes = [vp]
         L.saf3r_launch_count.restype = i64
         L.saf3r_set_stage_timing.argtypes = [vp, i32]
@@ -110,6 +120,17 @@ def make_shape(S: int, T: int, H: int, D: int, B: int, stride_head: int | None =
     st = D if stride_token is None else stride_token
     sh = S * T * st if stride_head is None else stride_head
     return ShapeC(S, T, H, D, B, sh, st)
+
+
+@dataclass
+class TokenLists:
+    tile_ptr: "torch.Tensor"  # int64 [NB+1], device
+    key_idx: "torch.Tensor"   # int32 [tiles*block], device
+    mask: "torch.Tensor"      # int32 [tiles][block][block/32], device (bit patterns)
+    tiles: int
+
+    def c(self) -> TokenListsC:
+        return TokenListsC(self.tile_ptr.data_ptr(), self.key_idx.data_ptr(), self.mask.data_ptr(), self.tiles)
 
 
 @dataclass
@@ -304,6 +325,52 @@ class Context:
                                                   lse.data_ptr() if lse is not None else None, _stream_ptr(stream)))
         return (out, lse) if want_lse else out
 
+    # ---- token-wise per-frame Top-K: saf3r_token_topk_select / saf3r_token_lists_count / _fill / _attn
+    def token_topk_select(self, feat, shape: ShapeC, K: int, workspace=None, idx=None, stream=None):
+        """feat: [N][64] bf16 device tensor (per-sequence features).  Returns idx int32 [N][S][K]: per query and frame the K most
+        cosine-similar tokens of that frame, ascending."""
+        import torch
+        ws_bytes, _, _ = token_topk_query_sizes(shape, K)
+        N = shape.num_frames * shape.tokens_per_frame
+        if workspace is None:
+            workspace = torch.empty(ws_bytes, dtype=torch.uint8, device=feat.device)
+            _on_stream(stream, workspace)
+        if idx is None:
+            idx = torch.empty((N, shape.num_frames, K), dtype=torch.int32, device=feat.device)
+            _on_stream(stream, idx)
+        fshape = ShapeC(shape.num_frames, shape.tokens_per_frame, 1, shape.head_dim, shape.block, N * feat.stride(0), feat.stride(0))
+        self._check(self.lib.saf3r_token_topk_select(self.h, feat.data_ptr(), C.byref(fshape), int(K), workspace.data_ptr(),
+                                                     workspace.numel(), idx.data_ptr(), _stream_ptr(stream)))
+        return idx
+
+    def token_lists_build(self, shape: ShapeC, idx, stream=None) -> TokenLists:
+        """Per q-tile union of the queries' keys + per-(query, key) masks (once per sequence).  Counts first, reads the total back
+        (one synchronisation), allocates exactly, then fills."""
+        import torch
+        K = int(idx.shape[2])
+        N = shape.num_frames * shape.tokens_per_frame
+        NB = (N + shape.block - 1) // shape.block
+        tile_ptr = torch.empty(NB + 1, dtype=torch.int64, device=idx.device)
+        _on_stream(stream, tile_ptr)
+        self._check(self.lib.saf3r_token_lists_count(self.h, C.byref(shape), K, idx.data_ptr(), tile_ptr.data_ptr(), _stream_ptr(stream)))
+        (torch.cuda.current_stream() if stream is None else stream).synchronize()
+        tiles = int(tile_ptr[-1].item())
+        B = shape.block
+        lists = TokenLists(tile_ptr, torch.empty(max(tiles, 1) * B, dtype=torch.int32, device=idx.device),
+                           torch.empty((max(tiles, 1), B, B // 32), dtype=torch.int32, device=idx.device), tiles)
+        _on_stream(stream, lists.key_idx, lists.mask)
+        lc = lists.c()
+        self._check(self.lib.saf3r_token_lists_fill(self.h, C.byref(shape), K, idx.data_ptr(), C.byref(lc), _stream_ptr(stream)))
+        return lists
+
+    def token_lists_attn(self, q, k, v, shape: ShapeC, lists: TokenLists, out=None, out_fp32=False, want_lse=False, stream=None):
+        out, lse = self._out_lse(q, shape, out, out_fp32, want_lse, stream)
+        lc = lists.c()
+        self._check(self.lib.saf3r_token_lists_attn(self.h, q.data_ptr(), k.data_ptr(), v.data_ptr(), C.byref(shape), C.byref(lc),
+                                                    out.data_ptr(), int(out_fp32), lse.data_ptr() if lse is not None else None,
+                                                    _stream_ptr(stream)))
+        return (out, lse) if want_lse else out
+
     # ---- saf3r_static_broadcast_attn
     def static_broadcast_attn(self, q, k, v, shape: ShapeC, workspace=None, out=None, out_fp32=False, want_lse=False, stream=None):
         """Static kernel that broadcasts frame 0's local attention map to every frame pair."""
@@ -336,6 +403,16 @@ class Context:
                                               arr, scratch.data_ptr(), scratch.numel() * scratch.element_size(),
                                               out_host.data_ptr(), _stream_ptr(stream)))
         return out_host
+
+
+def token_topk_query_sizes(shape: ShapeC, K: int) -> tuple[int, int, int]:
+    """Host-only: (select workspace bytes, idx entries = N*S*K, worst-case tiles) of the token-wise per-frame Top-K calls."""
+    L = load_library()
+    a, b, c = C.c_size_t(), C.c_int64(), C.c_int64()
+    st = L.saf3r_token_topk_query_sizes(C.byref(shape), int(K), C.byref(a), C.byref(b), C.byref(c))
+    if st != OK:
+        raise Saf3rError(st, "saf3r_token_topk_query_sizes rejected (shape, K)")
+    return int(a.value), int(b.value), int(c.value)
 
 
 def token_query_sizes(shape: ShapeC, K: int) -> tuple[int, int]:

@@ -10,7 +10,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libsaf3r.so")
 SOURCES = ["saf3r_api.cu"]
-DEPS = ["saf3r_api.cu", "attn_kernel.cuh", "select_kernels.cuh", "token_kernels.cuh", "ptx.cuh", os.path.join(ROOT, "include", "saf3r.h")]
+DEPS = ["saf3r_api.cu", "attn_kernel.cuh", "select_kernels.cuh", "token_kernels.cuh", "tokenwise_kernels.cuh", "ptx.cuh", os.path.join(ROOT, "include", "saf3r.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--expt-relaxed-constexpr",
               "--expt-extended-lambda", "-Xcompiler", "-fPIC", "-shared", "-I", os.path.join(ROOT, "include")]
 

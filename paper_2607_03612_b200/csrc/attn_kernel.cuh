@@ -8,7 +8,8 @@
 //               pipes (no MUFU).  The two halves of a row exchange their partial row max through shared memory.
 //   warp  8     TMA producer: Q tile once, then K_J into a 3-stage ring and V_J into a 2-stage ring
 //   warp  9     TMEM allocator + MMA issuer (one thread): S = Q K_J^T (tcgen05 SS), O += P V_J (tcgen05 TS: P from TMEM)
-//   warps 10-11 idle (they only complete the third warpgroup so that setmaxnreg can hand its registers over)
+//   warps 10-11 idle (they only complete the third warpgroup so that setmaxnreg can hand its registers over); in the token-list
+//               mode warp 8 gathers the K tiles and warp 10 the V tiles with cp.async instead of TMA
 // Running max is lazy (moves only when a row max grows by more than 2^8), so O in TMEM is rescaled rarely.  And it is
 // FROZEN as soon as it provably cannot matter: by Cauchy-Schwarz every logit of row i is at most |q_i| * max_j |k_j| / sqrt(D)
 // (kmax[h] = max_j |k_j| comes from knorm_kernel, one streaming pass over K before the launch).  Once that bound is within
@@ -17,6 +18,8 @@
 // the exchange between the two halves and the named barrier altogether - about an eighth of the softmax instructions.
 // TMEM columns: S [0,B) fp32, O [128,192) fp32, P [192,192+B/2) packed bf16.
 #pragma once
+#include <type_traits>
+
 #include "ptx.cuh"
 #include "saf3r.h"
 
@@ -34,6 +37,13 @@ struct AttnParams {
   float scale_log2;  // (1/sqrt(D)) * log2(e)
   const float *kmax;  // [H] max_j |k_j|_2 over the head's key tokens (knorm_kernel), or nullptr: never freeze the max
   uint8_t head_order[SAF3R_MAX_HEADS];  // blockIdx.y -> head, longest lists first
+  // token-list mode (kTok; SURVEY 8(f) NEXT-2 iii): the k-tiles of q-tile I are tiles [tile_ptr[I], tile_ptr[I+1]) of B gathered key
+  // tokens each (key_idx, -1 = padding), shared by all heads; mask bit (row r, column c) of a tile says whether query r keeps key c
+  const int64_t *tile_ptr;
+  const int32_t *key_idx;
+  const uint32_t *mask;  // [tile][B rows][B/32 words]
+  const __nv_bfloat16 *k_base, *v_base;
+  int64_t kv_stride_head, kv_stride_token;
 };
 
 constexpr int kD = 64;  // head_dim (bf16: one 128-byte swizzle row)
@@ -61,7 +71,7 @@ struct AttnSmem {
 };
 
 // one softmax half: rows = TMEM lanes of this warp, columns [C0, C1) of the B-wide tile
-template <int B, int C0, int C1, bool kFma>
+template <int B, int C0, int C1, bool kFma, bool kTok>
 __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem, uint32_t tmem, int n_ent, int64_t e0, int h,
                                              int I, uint32_t bar_q, uint32_t bar_s_full, uint32_t bar_s_free,
                                              uint32_t bar_p_full, uint32_t bar_o_done) {
@@ -83,13 +93,13 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
   const float c = p.scale_log2;
   const float lazy_raw = kLazyLog2 / c;
   float m = -INFINITY, l = 0.f;
-  const int J_last = (n_ent > 0) ? (p.row_ptr ? p.col_idx[e0 + n_ent - 1] : p.NB_kv - 1) : -1;
-  const bool last_is_tail = (J_last == p.NB_kv - 1) && (tail < B);
+  const int J_last = (n_ent > 0 && !kTok) ? (p.row_ptr ? p.col_idx[e0 + n_ent - 1] : p.NB_kv - 1) : -1;
+  const bool last_is_tail = !kTok && (J_last == p.NB_kv - 1) && (tail < B);
   // Cauchy-Schwarz bound of this row's logits (in the units of m: raw scores), from the Q tile in shared memory.  Both halves
   // of a row read the same eight 16-byte chunks in the same (physical) order, so they get the same bits and take the same
   // freeze decision without talking to each other.
   float bound = INFINITY;
-  bool frozen = false;
+  bool frozen = false, noclamp = false;
   if (p.kmax != nullptr && n_ent > 1) {
     mbar_wait(bar_q, 0);
     const uint4 *qrow = reinterpret_cast<const uint4 *>(smem + L::kQ + r * 128);
@@ -124,6 +134,16 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
       for (int i = 0; i < NC; ++i)
         if (C0 + i >= tail) v[i] = 0xff800000u;  // -inf
     }
+    if (kTok) {  // per-(query, key) mask of this tile: keys the query did not select get -inf before the max
+      constexpr int W0 = C0 / 32, W1 = (C1 + 31) / 32;
+      uint32_t mw[W1 - W0];
+      const uint32_t *mrow = p.mask + ((e0 + e) * B + (r < B ? r : 0)) * (B / 32);
+#pragma unroll
+      for (int w = W0; w < W1; ++w) mw[w - W0] = r < B ? __ldg(mrow + w) : 0u;
+#pragma unroll
+      for (int i = 0; i < NC; ++i)
+        if (!((mw[(C0 + i) / 32 - W0] >> ((C0 + i) & 31)) & 1u)) v[i] = 0xff800000u;
+    }
     float alpha = 1.f;
     bool moved = false;
     if (!frozen) {
@@ -148,33 +168,39 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
       if (moved) {
         const float m_new = fmaxf(m, mx);
         alpha = ex2_approx((m - m_new) * c);
+        if (kTok && m_new == -INFINITY) alpha = 1.f;  // this row has seen no kept key yet (another row of the warp moved)
         m = m_new;
       }
       // no later logit of these 32 rows can exceed m by more than 2^kFreezeLog2: m stays where it is from now on
       frozen = __all_sync(0xffffffffu, bound <= m + freeze_raw);
+      if (kFma && frozen) noclamp = __all_sync(0xffffffffu, (bound + fabsf(m)) * c < 120.f);
     }
-    const float nmc = -m * c;
+    const float nmc = (kTok && m == -INFINITY) ? 0.f : -m * c;  // a row without a kept key so far: every x stays -inf, p = 0
     uint32_t pk[NC / 2];
-    uint64_t acc0 = 0ull, acc1 = 0ull;
+    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;  // row sum of the bf16-ROUNDED weights (what the PV product multiplies)
     const uint64_t c2 = pack_f32x2(c, c), nmc2 = pack_f32x2(nmc, nmc);
+    auto exp_tile = [&](auto clamp_tag) {
+      constexpr bool kClamp = decltype(clamp_tag)::value;
 #pragma unroll
-    for (int j = 0; j < NC / 2; ++j) {
-      const uint64_t x2 = fma_f32x2(pack_f32x2(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1])), c2, nmc2);
-      float p0, p1;
-      if (kFma) {
-        exp2_emu_f32x2(x2, p0, p1);
-      } else {
-        unpack_f32x2(x2, p0, p1);
-        p0 = ex2_approx(p0);
-        p1 = ex2_approx(p1);
+      for (int j = 0; j < NC / 2; ++j) {
+        const uint64_t x2 = fma_f32x2(pack_f32x2(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1])), c2, nmc2);
+        float p0, p1;
+        if (kFma) {
+          exp2_emu_f32x2<kClamp>(x2, p0, p1);
+        } else {
+          unpack_f32x2(x2, p0, p1);
+          p0 = ex2_approx(p0);
+          p1 = ex2_approx(p1);
+        }
+        pk[j] = pack_bf16x2(p0, p1);
+        if (j & 1) add_bf16x2_to_f32(pk[j], s2, s3);
+        else add_bf16x2_to_f32(pk[j], s0, s1);
       }
-      if (j & 1) acc1 = add_f32x2(acc1, pack_f32x2(p0, p1));
-      else acc0 = add_f32x2(acc0, pack_f32x2(p0, p1));
-      pk[j] = pack_bf16x2(p0, p1);
-    }
-    float s0, s1, s2, s3;
-    unpack_f32x2(acc0, s0, s1);
-    unpack_f32x2(acc1, s2, s3);
+    };
+    // the polynomial half needs its argument clamped at -126 unless every x of the tile is known to be above it: frozen max,
+    // |logit| <= bound for all 32 rows (Cauchy-Schwarz again: x >= -(bound + m) c), no masked (-inf) column in the tile
+    if (kFma && !kTok && noclamp && !(e == n_ent - 1 && last_is_tail)) exp_tile(std::false_type{});
+    else exp_tile(std::true_type{});
     l = l * alpha + ((s0 + s1) + (s2 + s3));
     // PV(e-1) must be complete before P is overwritten and O is rescaled
     if (e > 0) {
@@ -237,7 +263,25 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
   }
 }
 
+// token-list mode: one warp gathers the B key (or value) rows of a tile into a SWIZZLE_128B stage with 16-byte cp.async copies
+// (lane = 16-byte chunk (l & 7) of rows (l >> 3) + 4 i; padding rows are zero-filled); the stage's mbarrier (32 arrivals) completes
+// when every lane's copies have landed.
 template <int B>
+__device__ __forceinline__ void gather_tile(const __nv_bfloat16 *__restrict__ base, int64_t stride_token, const int32_t *__restrict__ idx,
+                                            uint32_t stage, uint32_t bar_full) {
+  const int lane = threadIdx.x & 31, ch = lane & 7, rr = lane >> 3;
+#pragma unroll 8
+  for (int it = 0; it < B / 4; ++it) {
+    const int row = it * 4 + rr;
+    const int j = __ldg(idx + row);
+    const uint32_t dst = stage + row * 128 + ((ch ^ (row & 7)) << 4);
+    const __nv_bfloat16 *src = base + (int64_t)(j < 0 ? 0 : j) * stride_token + ch * 8;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(j < 0 ? 0 : 16) : "memory");
+  }
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar_full) : "memory");
+}
+
+template <int B, bool kTok>
 __global__ void __launch_bounds__(kAttnThreads, 2)
 saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
                   const __grid_constant__ CUtensorMap map_v, const AttnParams p) {
@@ -262,7 +306,10 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
 
   int64_t e0 = 0;
   int n_ent = p.NB_kv;
-  if (p.row_ptr != nullptr) {
+  if (kTok) {
+    e0 = p.tile_ptr[I];
+    n_ent = (int)(p.tile_ptr[I + 1] - e0);
+  } else if (p.row_ptr != nullptr) {
     const int64_t r = (int64_t)h * p.NB + I;
     e0 = p.row_ptr[r];
     n_ent = (int)(p.row_ptr[r + 1] - e0);
@@ -271,8 +318,8 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
   if (threadIdx.x == 0) {
     if (sbase & 1023u) __trap();  // SWIZZLE_128B tiles need a 1024-byte aligned base
     mbar_init(bar_q, 1);
-    for (int s = 0; s < kKStages; ++s) { mbar_init(bar_k_full + 8 * s, 1); mbar_init(bar_k_empty + 8 * s, 1); }
-    for (int s = 0; s < kVStages; ++s) { mbar_init(bar_v_full + 8 * s, 1); mbar_init(bar_v_empty + 8 * s, 1); }
+    for (int s = 0; s < kKStages; ++s) { mbar_init(bar_k_full + 8 * s, kTok ? 32 : 1); mbar_init(bar_k_empty + 8 * s, 1); }
+    for (int s = 0; s < kVStages; ++s) { mbar_init(bar_v_full + 8 * s, kTok ? 32 : 1); mbar_init(bar_v_empty + 8 * s, 1); }
     mbar_init(bar_s_full, 1);
     mbar_init(bar_s_free, 256);
     mbar_init(bar_p_full, 256);
@@ -301,6 +348,15 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
           tma_load_3d(sbase + L::kQ, &map_q, bar_q, 0, I * B, h);
         }
         __syncwarp();
+        if (kTok) {  // warp 8 gathers the K tiles (warp 10 the V tiles, below)
+          const __nv_bfloat16 *kb = p.k_base + (int64_t)h * p.kv_stride_head;
+          int sk = 0, phk = 0;
+          for (int e = 0; e < n_ent; ++e) {
+            mbar_wait_relaxed<kSleepTma>(bar_k_empty + 8 * sk, phk ^ 1);
+            gather_tile<B>(kb, p.kv_stride_token, p.key_idx + (e0 + e) * B, sbase + L::kK + sk * B * 128, bar_k_full + 8 * sk);
+            if (++sk == kKStages) { sk = 0; phk ^= 1; }
+          }
+        } else {
         int Jn = p.row_ptr ? p.col_idx[e0] : 0;
         int sk = 0, phk = 0, sv = 0, phv = 0;
         for (int e = 0; e < n_ent; ++e) {
@@ -321,6 +377,16 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
           if (++sk == kKStages) { sk = 0; phk ^= 1; }
           if (++sv == kVStages) { sv = 0; phv ^= 1; }
         }
+        }
+      }
+    } else if (kTok && warp == 10) {
+      // ------------------------------------------------------------ token-list mode: gather producer of the V tiles
+      const __nv_bfloat16 *vb = p.v_base + (int64_t)h * p.kv_stride_head;
+      int sv = 0, phv = 0;
+      for (int e = 0; e < n_ent; ++e) {
+        mbar_wait_relaxed<kSleepTma>(bar_v_empty + 8 * sv, phv ^ 1);
+        gather_tile<B>(vb, p.kv_stride_token, p.key_idx + (e0 + e) * B, sbase + L::kV + sv * B * 128, bar_v_full + 8 * sv);
+        if (++sv == kVStages) { sv = 0; phv ^= 1; }
       }
     } else if (warp == 9) {
       // ------------------------------------------------------------ MMA issuer (warp-uniform loop, one elected lane issues)
@@ -332,6 +398,7 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
         int sk = 0, phk = 0;
         auto issue_qk = [&]() {
           mbar_wait_relaxed<kSleepMma>(bar_k_full + 8 * sk, phk);
+          if (kTok) fence_proxy_async_smem();  // the gathered tile was written through the generic proxy (cp.async)
           tc_fence_after();
           if (elect_one_sync()) {
             const uint64_t kdesc = umma_desc_sw128(sbase + L::kK + sk * B * 128);
@@ -352,6 +419,7 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
             issue_qk();
           }
           mbar_wait_relaxed<kSleepMma>(bar_v_full + 8 * sv, phv);
+          if (kTok) fence_proxy_async_smem();
           mbar_wait_relaxed<kSleepMma>(bar_p_full, e & 1);
           tc_fence_after();
           if (elect_one_sync()) {
@@ -369,10 +437,10 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
     }
   } else if (warp < 4) {
     setmaxnreg_inc<kRegsMufu>();
-    softmax_half<B, 0, L::kSplit, false>(p, smem, tmem, n_ent, e0, h, I, bar_q, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
+    softmax_half<B, 0, L::kSplit, false, kTok>(p, smem, tmem, n_ent, e0, h, I, bar_q, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
   } else {
     setmaxnreg_inc<kRegsFma>();
-    softmax_half<B, L::kSplit, B, true>(p, smem, tmem, n_ent, e0, h, I, bar_q, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
+    softmax_half<B, L::kSplit, B, true, kTok>(p, smem, tmem, n_ent, e0, h, I, bar_q, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
   }
 
   tc_fence_before();

@@ -235,6 +235,17 @@ __device__ __forceinline__ uint64_t mul_f32x2(uint64_t a, uint64_t b) {
   asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
   return d;
 }
+// acc += lo half (bf16) and acc2 += hi half (bf16) of a packed pair, in fp32 (sm_100 mixed-precision add: FHADD.BF16 reads the
+// half straight out of the packed register).  Used to sum the ROUNDED softmax weights: the row sum then matches what the PV
+// tensor-core product sees bit for bit, so the bf16 rounding of P perturbs o = sum(P v) / sum(P) only through (v_j - o), not v_j.
+__device__ __forceinline__ void add_bf16x2_to_f32(uint32_t pk, float &acc_lo, float &acc_hi) {
+  asm("{\n\t.reg .b16 lo, hi;\n\t"
+      "mov.b32 {lo, hi}, %2;\n\t"
+      "add.rn.f32.bf16 %0, lo, %0;\n\t"
+      "add.rn.f32.bf16 %1, hi, %1;\n\t}"
+      : "+f"(acc_lo), "+f"(acc_hi)
+      : "r"(pk));
+}
 __device__ __forceinline__ float max3(float a, float b, float c) {
   float d;
   asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
@@ -244,12 +255,17 @@ __device__ __forceinline__ float max3(float a, float b, float c) {
 // 2^x for a packed pair on the FMA/ALU pipes (no MUFU): Cody-Waite range reduction by the magic-number add
 // (round-to-nearest integer n lands in the low mantissa bits), degree-3 polynomial for 2^f on f in [-0.5, 0.5]
 // (max relative error 2.1e-4, below bf16 rounding of P), exponent inserted with an integer shift-add.
+// kClamp = false is for callers that KNOW x >= -126 (no masked / -inf inputs, bounded logits): it saves the two FMNMX.
+template <bool kClamp>
 __device__ __forceinline__ void exp2_emu_f32x2(uint64_t x2, float &p0, float &p1) {
-  float x0, x1;
-  unpack_f32x2(x2, x0, x1);
-  x0 = fmaxf(x0, -126.f);
-  x1 = fmaxf(x1, -126.f);
-  const uint64_t xc = pack_f32x2(x0, x1);
+  uint64_t xc = x2;
+  if (kClamp) {
+    float x0, x1;
+    unpack_f32x2(x2, x0, x1);
+    x0 = fmaxf(x0, -126.f);
+    x1 = fmaxf(x1, -126.f);
+    xc = pack_f32x2(x0, x1);
+  }
   const uint64_t t = add_f32x2(xc, pack_f32x2(12582912.f, 12582912.f));
   const uint64_t fl = add_f32x2(t, pack_f32x2(-12582912.f, -12582912.f));
   const uint64_t f = fma_f32x2(fl, pack_f32x2(-1.f, -1.f), xc);

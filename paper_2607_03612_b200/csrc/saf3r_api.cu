@@ -13,6 +13,7 @@
 #include "attn_kernel.cuh"
 #include "select_kernels.cuh"
 #include "token_kernels.cuh"
+#include "tokenwise_kernels.cuh"
 
 using namespace saf3r;
 
@@ -199,9 +200,12 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
     return SAF3R_ERR_UNSUPPORTED;
   }
   ctx->encode = (EncodeTiledFn)fn;
-  e = cudaFuncSetAttribute(saf3r_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128>::kTotal);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
+  e = cudaFuncSetAttribute(saf3r_attn_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128>::kTotal);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128>::kTotal);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(token_sim_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSimSmem);
   if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->counter_dev, sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->kmax_ring, sizeof(float) * kKmaxSlots * SAF3R_MAX_HEADS);
   if (e != cudaSuccess) {
@@ -542,10 +546,11 @@ static saf3r_status attn_common(saf3r_ctx *ctx, const void *q, const void *k, co
     p.kmax = slot;
   }
   dim3 grid(g.NB, g.H);
+  p.tile_ptr = nullptr; p.key_idx = nullptr; p.mask = nullptr; p.k_base = p.v_base = nullptr; p.kv_stride_head = p.kv_stride_token = 0;
   if (g.B == 128)
-    saf3r_attn_kernel<128><<<grid, kAttnThreads, AttnSmem<128>::kTotal, st>>>(mq, mk, mv, p);
+    saf3r_attn_kernel<128, false><<<grid, kAttnThreads, AttnSmem<128>::kTotal, st>>>(mq, mk, mv, p);
   else
-    saf3r_attn_kernel<64><<<grid, kAttnThreads, AttnSmem<64>::kTotal, st>>>(mq, mk, mv, p);
+    saf3r_attn_kernel<64, false><<<grid, kAttnThreads, AttnSmem<64>::kTotal, st>>>(mq, mk, mv, p);
   ctx->launches += 1;
   CU_CHECK(cudaGetLastError());
   return SAF3R_OK;
@@ -713,6 +718,150 @@ saf3r_status saf3r_token_set_attn(saf3r_ctx *ctx, const void *q, const void *k, 
   CU_CHECK(cudaGetLastError());
   const KvGeom kv{K, (int64_t)K * 64, 64};
   return attn_common(ctx, q, kc, vc, shape, nullptr, out, out_is_fp32, lse, stream_, &kv);
+}
+
+// ------------------------------------------------------------------------------------------------ token-wise per-frame Top-K (NEXT-2 iii)
+struct TokTopkWs { size_t rn, keys, total; int64_t ld; int strips; };
+static TokTopkWs toktopk_ws(int64_t N) {
+  TokTopkWs w;
+  const int64_t nb = (N + 127) / 128;
+  w.ld = nb * 128;
+  const int64_t strip_bytes = 128 * w.ld * 4;
+  int64_t strips = (48ll << 20) / strip_bytes;  // q-tiles per launch pair: keep the key strip L2-sized
+  if (strips < 1) strips = 1;
+  if (strips > 8) strips = 8;
+  if (strips > nb) strips = nb;
+  w.strips = (int)strips;
+  size_t off = 0;
+  w.rn = off; off = align256(off + (size_t)N * sizeof(float));
+  w.keys = off; off = align256(off + (size_t)strips * strip_bytes);
+  w.total = off;
+  return w;
+}
+static int64_t toktopk_max_tiles(const SelGeom &g, int K) {
+  const int64_t per_frame = i64min(g.T, (int64_t)g.B * K);  // distinct keys a q-tile of B queries can pick in one frame
+  return (int64_t)g.NB * (((int64_t)g.S * per_frame + g.B - 1) / g.B);
+}
+static const char *validate_toktopk(const saf3r_shape *shape, int K) {
+  if (const char *m = validate_shape(shape, false)) return m;
+  if (K < 1 || K > shape->tokens_per_frame) return "token-wise Top-K: need 1 <= K <= tokens_per_frame";
+  return nullptr;
+}
+
+saf3r_status saf3r_token_topk_query_sizes(const saf3r_shape *shape, int32_t K, size_t *select_ws, int64_t *idx_entries, int64_t *max_tiles) {
+  if (validate_toktopk(shape, K)) return SAF3R_ERR_INVALID_ARG;
+  if (unsupported_shape(shape)) return SAF3R_ERR_UNSUPPORTED;
+  const SelGeom g = make_geom(shape);
+  if (select_ws) *select_ws = toktopk_ws(g.N).total;
+  if (idx_entries) *idx_entries = g.N * g.S * K;
+  if (max_tiles) *max_tiles = toktopk_max_tiles(g, K);
+  return SAF3R_OK;
+}
+
+saf3r_status saf3r_token_topk_select(saf3r_ctx *ctx, const void *feat, const saf3r_shape *shape, int32_t K, void *ws, size_t ws_bytes,
+                                     int32_t *idx, void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_toktopk(shape, K)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  if (!feat || !ws || !idx) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  if (shape->stride_token < 64 || shape->stride_token % 8 || ((uintptr_t)feat & 15))
+    return fail(ctx, SAF3R_ERR_INVALID_ARG, "features: 16-byte aligned, stride_token a multiple of 8 elements and >= head_dim");
+  SelGeom g = make_geom(shape);
+  g.H = 1; g.B = 128; g.NB = (int32_t)((g.N + 127) / 128);
+  g.stride_head = g.N * g.stride_token;
+  const TokTopkWs w = toktopk_ws(g.N);
+  if (ws_bytes < w.total) return fail(ctx, SAF3R_ERR_CAPACITY, "workspace too small (saf3r_token_topk_query_sizes)");
+  CUtensorMap mf;
+  saf3r_status s;
+  if ((s = get_map(ctx, feat, g, &mf)) != SAF3R_OK) return s;
+  cudaStream_t st = (cudaStream_t)stream_;
+  float *rn = (float *)((uint8_t *)ws + w.rn);
+  uint32_t *keys = (uint32_t *)((uint8_t *)ws + w.keys);
+  feat_rnorm_kernel<<<(unsigned)((g.N + 31) / 32), 256, 0, st>>>((const __nv_bfloat16 *)feat, g.N, g.stride_token, rn);
+  ctx->launches += 1;
+  for (int q0 = 0; q0 < g.NB; q0 += w.strips) {
+    const int nq = g.NB - q0 < w.strips ? g.NB - q0 : w.strips;
+    token_sim_kernel<<<dim3(g.NB, nq), 128, kSimSmem, st>>>(mf, rn, keys, g.N, w.ld, q0);
+    const int64_t warps = (int64_t)nq * 128 * g.S;
+    token_frame_topk_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(keys, w.ld, (int64_t)q0 * 128, nq * 128, g.N, g.S, g.T, K, idx);
+    ctx->launches += 2;
+  }
+  CU_CHECK(cudaGetLastError());
+  return SAF3R_OK;
+}
+
+static saf3r_status toklists_common(saf3r_ctx *ctx, const saf3r_shape *shape, int K, const int32_t *idx, int64_t *tile_ptr,
+                                    const saf3r_token_lists *lists, void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_toktopk(shape, K)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  if (!idx || !tile_ptr || (lists && (!lists->key_idx || !lists->mask))) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  const SelGeom g = make_geom(shape);
+  const size_t sm = 2 * (size_t)((g.T + 31) / 32) * sizeof(uint32_t);
+  if (sm > 48 * 1024) return fail(ctx, SAF3R_ERR_UNSUPPORTED, "tokens_per_frame too large for the union kernel");
+  cudaStream_t st = (cudaStream_t)stream_;
+  if (!lists) {
+    token_union_kernel<false><<<g.NB, 256, sm, st>>>(idx, g.N, g.S, g.T, K, g.B, tile_ptr, nullptr, nullptr, 0);
+    scan_row_ptr_kernel<<<1, 1024, 0, st>>>(tile_ptr, g.NB);
+    ctx->launches += 2;
+  } else {
+    CU_CHECK(cudaMemsetAsync(lists->mask, 0, (size_t)lists->capacity_tiles * g.B * (g.B / 32) * sizeof(uint32_t), st));
+    token_union_kernel<true><<<g.NB, 256, sm, st>>>(idx, g.N, g.S, g.T, K, g.B, tile_ptr, lists->key_idx, lists->mask, lists->capacity_tiles);
+    ctx->launches += 1;
+  }
+  CU_CHECK(cudaGetLastError());
+  return SAF3R_OK;
+}
+
+saf3r_status saf3r_token_lists_count(saf3r_ctx *ctx, const saf3r_shape *shape, int32_t K, const int32_t *idx, int64_t *tile_ptr, void *stream) {
+  return toklists_common(ctx, shape, K, idx, tile_ptr, nullptr, stream);
+}
+
+saf3r_status saf3r_token_lists_fill(saf3r_ctx *ctx, const saf3r_shape *shape, int32_t K, const int32_t *idx, const saf3r_token_lists *lists,
+                                    void *stream) {
+  if (!lists) return fail(ctx, SAF3R_ERR_INVALID_ARG, "lists is null");
+  return toklists_common(ctx, shape, K, idx, lists->tile_ptr, lists, stream);
+}
+
+saf3r_status saf3r_token_lists_attn(saf3r_ctx *ctx, const void *q, const void *k, const void *v, const saf3r_shape *shape,
+                                    const saf3r_token_lists *lists, void *out, int out_is_fp32, float *lse, void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_shape(shape, true)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  if (!q || !k || !v || !out || !lists || !lists->tile_ptr || !lists->key_idx || !lists->mask)
+    return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  if (((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) return fail(ctx, SAF3R_ERR_INVALID_ARG, "q/k/v/out must be 16-byte aligned");
+  const SelGeom g = make_geom(shape);
+  CUtensorMap mq;
+  saf3r_status s;
+  if ((s = get_map(ctx, q, g, &mq)) != SAF3R_OK) return s;
+  AttnParams p;
+  memset(&p, 0, sizeof p);
+  p.out = out; p.lse = lse;
+  p.out_stride_head = shape->stride_head; p.out_stride_token = shape->stride_token;
+  p.N = (int32_t)g.N; p.NB = g.NB; p.H = g.H; p.N_kv = (int32_t)g.N; p.NB_kv = g.NB;
+  p.out_fp32 = out_is_fp32 ? 1 : 0;
+  p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)shape->head_dim));
+  for (int h = 0; h < g.H; ++h) p.head_order[h] = (uint8_t)h;
+  p.tile_ptr = lists->tile_ptr; p.key_idx = lists->key_idx; p.mask = lists->mask;
+  p.k_base = (const __nv_bfloat16 *)k; p.v_base = (const __nv_bfloat16 *)v;
+  p.kv_stride_head = g.stride_head; p.kv_stride_token = g.stride_token;
+  cudaStream_t st = (cudaStream_t)stream_;
+  float *slot = ctx->kmax_ring + (size_t)(ctx->kmax_next++ % kKmaxSlots) * SAF3R_MAX_HEADS;
+  CU_CHECK(cudaMemsetAsync(slot, 0, sizeof(float) * g.H, st));
+  knorm_kernel<<<dim3((unsigned)((g.N + kKnormRows - 1) / kKnormRows), g.H), 256, 0, st>>>((const __nv_bfloat16 *)k, g.N, g.stride_head, g.stride_token, slot);
+  p.kmax = slot;
+  dim3 grid(g.NB, g.H);
+  if (g.B == 128)
+    saf3r_attn_kernel<128, true><<<grid, kAttnThreads, AttnSmem<128>::kTotal, st>>>(mq, mq, mq, p);
+  else
+    saf3r_attn_kernel<64, true><<<grid, kAttnThreads, AttnSmem<64>::kTotal, st>>>(mq, mq, mq, p);
+  ctx->launches += 2;
+  CU_CHECK(cudaGetLastError());
+  return SAF3R_OK;
 }
 
 // ------------------------------------------------------------------------------------------------ static broadcast (NEXT-4)

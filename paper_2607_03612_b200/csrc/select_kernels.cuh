@@ -124,7 +124,7 @@ __device__ __forceinline__ uint32_t score_key(float s) {
 // splits the row into exactly n and NB-n keys), then an ordered ballot compaction emits {key > tau} plus the first
 // `need` (by index) of {key == tau}.
 template <int kKeysPerLaneReg>  // 0: keys stay in shared memory
-__device__ __forceinline__ void warp_topn_bisect_impl(const uint32_t *key, int NB, int n, int32_t *out) {
+__device__ __forceinline__ void warp_topn_bisect_impl(const uint32_t *key, int NB, int n, int32_t *out, int base) {
   constexpr bool kRegs = kKeysPerLaneReg > 0;
   const int lane = threadIdx.x & 31;
   uint32_t kk[kRegs ? kKeysPerLaneReg : 1];
@@ -178,7 +178,7 @@ __device__ __forceinline__ void warp_topn_bisect_impl(const uint32_t *key, int N
       const bool take = kk[i] > tau;
       const uint32_t tb = __ballot_sync(0xffffffffu, take);
       int32_t *dst = out + written + __popc(tb & lt);
-      asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u32 [%0], %1;\n\t}" ::"l"(dst), "r"(lane + 32 * i), "r"((uint32_t)take) : "memory");
+      asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u32 [%0], %1;\n\t}" ::"l"(dst), "r"(base + lane + 32 * i), "r"((uint32_t)take) : "memory");
       written += __popc(tb);
     }
     return;
@@ -190,15 +190,16 @@ __device__ __forceinline__ void warp_topn_bisect_impl(const uint32_t *key, int N
     const uint32_t eqb = __ballot_sync(0xffffffffu, eq);
     const bool take = gt || (eq && eq_seen + __popc(eqb & lt) < need);
     const uint32_t tb = __ballot_sync(0xffffffffu, take);
-    if (take) out[written + __popc(tb & lt)] = j;
+    if (take) out[written + __popc(tb & lt)] = base + j;
     written += __popc(tb);
     eq_seen += __popc(eqb);
   }
 }
-__device__ __forceinline__ void warp_topn_bisect(const uint32_t *key, int NB, int n, int32_t *out) {
-  if (NB <= 32 * 36) warp_topn_bisect_impl<36>(key, NB, n, out);
-  else if (NB <= 32 * 72) warp_topn_bisect_impl<72>(key, NB, n, out);
-  else warp_topn_bisect_impl<0>(key, NB, n, out);
+// `base` is added to every index written (the keys may be a window of a longer row)
+__device__ __forceinline__ void warp_topn_bisect(const uint32_t *key, int NB, int n, int32_t *out, int base = 0) {
+  if (NB <= 32 * 36) warp_topn_bisect_impl<36>(key, NB, n, out, base);
+  else if (NB <= 32 * 72) warp_topn_bisect_impl<72>(key, NB, n, out, base);
+  else warp_topn_bisect_impl<0>(key, NB, n, out, base);
 }
 
 // One warp: per-frame top-k (PER_FRAME scope): in every frame's candidate range keep the kf best; ascending output.

@@ -730,3 +730,98 @@ def test_static_broadcast_attn_matches_oracle(env, S, G, B, H):
         check_attention(out[h].cpu().numpy(), ref, f"broadcast head {h} ({gens[h]}) S={S}")
         assert np.abs(lse[h].cpu().numpy() - ref_lse).max() <= 1e-2
         assert np.abs(out_bf[h].float().cpu().numpy() - ref).max() <= 2e-2
+
+
+# ------------------------------------------------------------------------------------------------ token-wise per-frame Top-K (NEXT-2 iii)
+def _check_token_topk(feat, gi, S, T, K, rows):
+    """GPU idx rows against the oracle: bit-exact except near-ties of the cut (reading A11 on the cosine row)."""
+    ties = 0
+    for i in rows:
+        oi = orc.token_topk_per_frame(feat, S, T, K, i, i + 1)[0]
+        if np.array_equal(gi[i], oi):
+            continue
+        c = orc.token_cosine_row(feat, i)
+        for g in range(S):
+            a, b = gi[i, g], oi[g]
+            assert np.all(np.diff(a) > 0) and a[0] >= g * T and a[-1] < (g + 1) * T, f"query {i} frame {g}: not ascending / outside the frame"
+            if np.array_equal(a, b):
+                continue
+            fr = c[g * T:(g + 1) * T]
+            tau = float(np.sort(fr)[::-1][K - 1])
+            for j in np.setxor1d(a, b):
+                assert abs(float(c[j]) - tau) <= 1e-4 * max(abs(tau), float(np.abs(fr).max())), f"query {i} frame {g}: token {j} is not a near-tie"
+                ties += 1
+    return ties
+
+
+@pytest.mark.parametrize("S,G,B,K", [(4, 16, 64, 3), (5, 17, 128, 16), (3, 9, 128, 86), (6, 16, 128, 1)])
+def test_token_topk_per_frame_select_and_attention(env, S, G, B, K):
+    """token-wise DINO Top-K.  (1) saf3r_token_topk_select against orc_token_topk_per_frame on every query
+    (planted exact ties: duplicated feature rows); (2) the union / mask structure: every query's kept columns are exactly its keys;
+    (3) saf3r_token_lists_attn against orc_attn_token_lists on the GPU's own index lists, all heads."""
+    sf, ctx, torch = env
+    H = 3
+    gens = [sy.GEN_SAME_POSITION, sy.GEN_UNIFORM, sy.GEN_SINK]
+    L = small_layer(S, G, H, B, gens, [sy.cfg(type=sy.HEAD_DENSE)] * H, seed=121)
+    sh = L.shape
+    T, N = sh.T, sh.N
+    feat = sy.make_features(sh, seed=122)
+    feat[T + 9] = feat[T + 4]                                     # exact ties inside frame 1
+    feat[T + 11] = feat[T + 4]
+    shape = c_shape(sf, sh)
+    fdev = to_dev(feat)
+    idx = ctx.token_topk_select(fdev, shape, K)
+    torch.cuda.synchronize()
+    gi = idx.cpu().numpy()
+    ties = _check_token_topk(feat, gi, S, T, K, range(N))
+    print(f"token-wise top-K S={S} T={T} K={K}: near-ties {ties} of {gi.size} entries")
+    assert ties <= max(2, gi.size // 1000)
+    lists = ctx.token_lists_build(shape, idx)
+    tp, kidx, mask = lists.tile_ptr.cpu().numpy(), lists.key_idx.cpu().numpy(), lists.mask.cpu().numpy().view(np.uint32)
+    assert tp[0] == 0 and tp[-1] == lists.tiles and np.all(np.diff(tp) >= 1)
+    for I in range(sh.NB):
+        keys = kidx[tp[I] * B:tp[I + 1] * B]
+        real = keys[keys >= 0]
+        assert np.all(np.diff(real) > 0), "union of a q-tile must be ascending and unique"
+        assert set(real.tolist()) == set(gi[I * B:(I + 1) * B].ravel().tolist())
+        m = mask[tp[I]:tp[I + 1]]                                  # [tiles][B][B/32]
+        bits = ((m[:, :, :, None] >> np.arange(32, dtype=np.uint32)) & 1).reshape(m.shape[0], B, B).astype(bool)
+        for r in range(min(B, N - I * B)):
+            kept = keys.reshape(-1, B)[bits[:, r, :]]
+            assert np.array_equal(np.sort(kept), np.sort(gi[I * B + r].ravel())), f"q-tile {I} row {r}: mask does not match the query's keys"
+    q, k, v = upload(L)
+    out, lse = ctx.token_lists_attn(q, k, v, shape, lists, out_fp32=True, want_lse=True)
+    torch.cuda.synchronize()
+    for h in range(H):
+        ref, ref_lse = orc.attn_token_lists(L.q[h], L.k[h], L.v[h], gi.reshape(N, -1))
+        check_attention(out[h].cpu().numpy(), ref, f"tokenwise head {h} ({gens[h]}) K={K}")
+        assert np.abs(lse[h].cpu().numpy() - ref_lse).max() <= 1e-2
+
+
+def test_token_topk_per_frame_at_c2_size_sampled(env):
+    """C2 size (N = 43 968, S = 32, T = 1374) with the paper's K = 16 per frame: sampled queries of the index lists
+    against the oracle, the kept fraction K/T, sampled rows of the attention of three heads against the oracle on the GPU's lists."""
+    sf, ctx, torch = env
+    sh = sy.Shape(S=32, G=37, H=3, D=64, B=128)
+    K = 16
+    gens = [sy.GEN_SAME_POSITION, sy.GEN_SINK, sy.GEN_UNIFORM]
+    L = sy.make_layer(sh, gens, [sy.cfg(type=sy.HEAD_DENSE)] * 3, seed=131)
+    feat = sy.make_features(sh, seed=132)
+    shape = c_shape(sf, sh)
+    idx = ctx.token_topk_select(to_dev(feat), shape, K)
+    lists = ctx.token_lists_build(shape, idx)
+    q, k, v = upload(L)
+    out = ctx.token_lists_attn(q, k, v, shape, lists, out_fp32=True)
+    torch.cuda.synchronize()
+    gi = idx.cpu().numpy()
+    assert gi.shape == (sh.N, sh.S, K) and abs(gi.shape[1] * K / sh.N - K / sh.T) < 1e-12
+    rows = [0, 5, sh.T + 700, sh.N // 2, sh.N - 1]
+    ties = _check_token_topk(feat, gi, sh.S, sh.T, K, rows)
+    print(f"C2-size token-wise top-K: near-ties {ties} in {len(rows)} sampled queries; union tiles {lists.tiles} "
+          f"({lists.tiles / (sh.NB * sh.NB):.3%} of the dense tiles)")
+    assert ties <= 4
+    for h in range(3):
+        for i0 in (0, sh.N // 2 - 64, sh.N - 100):
+            i1 = min(sh.N, i0 + 128)
+            ref, _ = orc.attn_token_lists(L.q[h], L.k[h], L.v[h], gi[i0:i1].reshape(i1 - i0, -1), i0, i1)
+            check_attention(out[h].cpu().numpy(), ref, f"tokenwise-C2 head {h} ({gens[h]})")
