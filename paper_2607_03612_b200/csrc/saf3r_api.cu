@@ -141,7 +141,7 @@ static const char *validate_cfg(const SelGeom &g, const saf3r_head_cfg *cfg, int
 }
 
 struct WsLayout {
-  size_t qt, kt, qpart, probe, total;
+  size_t qt, kt, qpart, probe, counters, total;
 };
 static WsLayout ws_layout(const SelGeom &g) {
   WsLayout w;
@@ -150,6 +150,7 @@ static WsLayout ws_layout(const SelGeom &g) {
   w.kt = off; off = align256(off + (size_t)g.H * kt_stride(g.NB) * 64 * sizeof(float));
   w.qpart = off; off = align256(off + (size_t)g.H * ((g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask) * 64 * sizeof(float));
   w.probe = off; off = align256(off + (size_t)g.H * g.NB * sizeof(int32_t));
+  w.counters = off; off = align256(off + kSelCounters * sizeof(int));  // ticket counters and per-head flags of the fused kernel
   w.total = off;
   return w;
 }
@@ -204,7 +205,7 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(select_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(token_sim_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSimSmem);
   if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->counter_dev, sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->kmax_ring, sizeof(float) * kKmaxSlots * SAF3R_MAX_HEADS);
@@ -276,7 +277,7 @@ static SelPlan select_plan(const SelGeom &g, int n_block, int n_probe, int sm_co
   const size_t row = (size_t)kt_stride(g.NB) * 4;
   if (n_block > 0) {
     const size_t qbytes = 64 * kSelRows * 4;
-    size_t budget = 108 * 1024 - qbytes;
+    size_t budget = 108 * 1024 - qbytes;  // two CTAs per SM
     if (row > budget) budget = 220 * 1024 - qbytes;
     if (row > budget) { p.unsupported = "NB too large for the select kernel"; return p; }
     while ((size_t)p.R * row > budget) --p.R;
@@ -284,9 +285,10 @@ static SelPlan select_plan(const SelGeom &g, int n_block, int n_probe, int sm_co
     p.smem = (size_t)p.R * row + qbytes;
   }
   if (n_probe > 0) {
-    if (row > 200 * 1024) { p.unsupported = "NB too large for the probe stage"; return p; }
-    if (p.smem < row) p.smem = row;
+    if (row + kSelScratch > 220 * 1024) { p.unsupported = "NB too large for the probe stage"; return p; }
+    if (p.smem < row + kSelScratch) p.smem = row + kSelScratch;
   }
+  if (p.smem < 4096) p.smem = 4096;  // scratch of the pool / row_ptr tasks
   return p;
 }
 
@@ -357,11 +359,11 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
     base += hint.len[h];
   }
   plan.head_base[g.H] = base;
-  // pool jobs: QUERY_PROBE heads first (their probe CTAs come first in launch 2 and overlap with its score CTAs)
+  // pool jobs: BLOCK_TOPK heads first (their score strips then run under the pooling of the QUERY_PROBE heads)
   for (int pass = 0; pass < 2; ++pass)
     for (int h = 0; h < g.H; ++h) {
       const bool probe = cfg[h].type == SAF3R_HEAD_QUERY_PROBE_TOPK, block = cfg[h].type == SAF3R_HEAD_BLOCK_TOPK;
-      if (!(pass == 0 ? probe : block)) continue;
+      if (!(pass == 0 ? block : probe)) continue;
       for (int which = 0; which < 2; ++which) {
         jobs.head[jobs.n] = (uint8_t)h;
         jobs.which[jobs.n] = (uint8_t)which;
@@ -370,50 +372,48 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
         ++jobs.n;
       }
     }
-  // launch 2's plan first: an UNSUPPORTED shape must be reported before anything is enqueued (saf3r.h "Asynchrony")
+  // the launch plan first: an UNSUPPORTED shape must be reported before anything is enqueued (saf3r.h "Asynchrony")
   const SelPlan sp = select_plan(g, sets.n_block, sets.n_probe, ctx->sm_count);
   if (sp.unsupported) return fail(ctx, SAF3R_ERR_UNSUPPORTED, sp.unsupported);
-  const int R = sp.R;
-  const size_t sm = sp.smem;
-  // launch 1: pooling (one warp per token block of every tensor a rule reads) + one row_ptr CTA per head + the lists of the
-  // constant-length closed-form heads
-  const int pool_tasks = jobs.n * ((g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask);
-  // persistent pool CTAs, at most 4 per SM; with few rounds, as many as give every CTA the SAME number of tasks (2.76 tasks per
-  // CTA would run as long as 3: launch tasks/3 CTAs instead)
-  int pool_ctas = pool_tasks;
-  if (pool_tasks > 4 * ctx->sm_count) {
-    const int per_cta = (pool_tasks + 4 * ctx->sm_count - 1) / (4 * ctx->sm_count);
-    pool_ctas = per_cta <= 4 ? (pool_tasks + per_cta - 1) / per_cta : 4 * ctx->sm_count;  // many rounds: keep every slot busy
-  }
+  const int tasks_per_job = (g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask;
   const int light_chunks = (g.NB + kLightRows - 1) / kLightRows;
-  if (ctx->stage_timing) cudaEventRecord(ctx->ev[0], st);
-  pool_rowptr_kernel<<<pool_ctas + g.H + sets.n_emit * light_chunks, 256, 0, st>>>(
-      (const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart, lists->row_ptr, lists->col_idx, g, jobs, plan, ca, sets,
-      pool_ctas, pool_tasks);
-  ctx->launches += 1;
-  CU_CHECK(cudaGetLastError());
-  if (ctx->stage_timing) cudaEventRecord(ctx->ev[1], st);
-  // launch 2: probe CTAs, score + select CTAs (R rows each), light CTAs of the per-row-length STATIC heads and of CACHED heads
-  const int sel_ctas = sets.n_probe + sets.n_block * ((g.NB + R - 1) / R) + (sets.n_light + sets.n_cached) * light_chunks;
-  if (sel_ctas > 0) {
-    cudaLaunchConfig_t lc;
-    memset(&lc, 0, sizeof lc);
-    lc.gridDim = dim3(sel_ctas);
-    lc.blockDim = dim3(256);
-    lc.dynamicSmemBytes = sm;
-    lc.stream = st;
-    cudaLaunchAttribute attr;
-    attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;  // may start while the pool grid drains (see the kernels)
-    attr.val.programmaticStreamSerializationAllowed = 1;
-    lc.attrs = &attr;
-    lc.numAttrs = 1;
-    CU_CHECK(cudaLaunchKernelEx(&lc, select_kernel, (const float *)qt, (const float *)kt, (const int32_t *)probe,
-                                (const int64_t *)lists->row_ptr, (const float *)qpart, probe, lists->col_idx,
-                                (const int64_t *)(cache ? cache->row_ptr : nullptr), (const int32_t *)(cache ? cache->col_idx : nullptr),
-                                g, ca, sets, R));
+  FusedPlan fp;
+  memset(&fp, 0, sizeof fp);
+  fp.R = sp.R;
+  fp.strips = (g.NB + sp.R - 1) / sp.R;
+  fp.light_chunks = light_chunks;
+  fp.pool_need = 2 * tasks_per_job;
+  fp.n_rowptr = g.H;
+  fp.n_pool_a = 2 * sets.n_block * tasks_per_job;   // jobs are ordered BLOCK_TOPK heads first (see above)
+  fp.n_pool_b = 2 * sets.n_probe * tasks_per_job;
+  fp.n_x = sets.n_block * fp.strips;                // score strips: mixed into the pooling of the QUERY_PROBE heads
+  fp.n_probe = sets.n_probe;                        // everything below follows ALL pool tasks
+  fp.n_light = (sets.n_light + sets.n_cached) * light_chunks;
+  fp.n_emit = sets.n_emit * light_chunks;
+  fp.n_rep = sets.n_probe * light_chunks;
+  fp.period = fp.n_x > 0 && fp.n_pool_b / fp.n_x > 1 ? fp.n_pool_b / fp.n_x : 1;
+  const int n_tasks = fp.n_rowptr + fp.n_pool_a + fp.n_pool_b + fp.n_x + fp.n_probe + fp.n_light + fp.n_emit + fp.n_rep;
+  int *counters = (int *)(wsb + w.counters);
+  CU_CHECK(cudaMemsetAsync(counters, 0, kSelCounters * sizeof(int), st));
+  auto launch = [&](int t_begin, int t_end, int counter) {
+    fp.t_begin = t_begin; fp.t_end = t_end; fp.counter = counter;
+    const int ctas = t_end - t_begin < 2 * ctx->sm_count ? t_end - t_begin : 2 * ctx->sm_count;
+    if (ctas <= 0) return;
+    select_fused_kernel<<<ctas, 256, sp.smem, st>>>((const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart, probe, lists->row_ptr,
+                                                   lists->col_idx, (const int64_t *)(cache ? cache->row_ptr : nullptr),
+                                                   (const int32_t *)(cache ? cache->col_idx : nullptr), counters, g, jobs, plan, ca, sets, fp);
     ctx->launches += 1;
-  }
-  if (ctx->stage_timing) {
+  };
+  if (!ctx->stage_timing) {
+    launch(0, n_tasks, 0);   // ONE launch: the dependent tasks run under the pooling of the QUERY_PROBE heads
+  } else {
+    // measurement aid: the same kernel as two launches, pooling (+ row_ptr) first, everything else second, with events around them
+    fp.period = fp.n_pool_b + 1;  // no mixing: all pool tasks come before the first dependent task
+    const int n_first = fp.n_rowptr + fp.n_pool_a + fp.n_pool_b;
+    cudaEventRecord(ctx->ev[0], st);
+    launch(0, n_first, 0);
+    cudaEventRecord(ctx->ev[1], st);
+    launch(n_first, n_tasks, 1);
     cudaEventRecord(ctx->ev[2], st);
     ctx->ev_valid = true;
   }

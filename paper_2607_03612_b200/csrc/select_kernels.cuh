@@ -1,10 +1,11 @@
 // Online pattern adaptation at block granularity (steps a-1..a-3 of DESIGN.md):
-//   pool_rowptr_kernel  Q,K bf16 -> Qtilde,Ktilde fp32 block means and per-task token sums of Q (HBM-bound stream); in extra
-//                       CTAs of the same launch, row_ptr from the closed-form row lengths and the lists of the constant-length
-//                       closed-form heads
-//   select_kernel       one probe CTA per QUERY_PROBE head: qbar = (1/N) sum_t q_t, p[J] = qbar . Ktilde_J /
-//                       sqrt(D), top-n -> the head's lists; score CTAs per (BLOCK_TOPK head, strip of q-blocks): score rows +
-//                       top-n / per-frame top-k; light CTAs: per-row closed forms and copies from the index cache
+//   select_fused_kernel  ONE persistent launch; its CTAs draw tasks in a fixed order from a ticket counter:
+//     pool tasks    Q,K bf16 -> Qtilde,Ktilde fp32 block means and per-task token sums of Q (the HBM-bound stream)
+//     row_ptr tasks closed-form row lengths -> offsets
+//     score strips  per (BLOCK_TOPK head, strip of q-blocks): score rows in shared memory + top-n / per-frame top-k
+//     probe tasks   per QUERY_PROBE head: qbar = (1/N) sum_t q_t, p[J] = qbar . Ktilde_J / sqrt(D), top-n -> lists
+//     light / emit  per-row closed forms, copies from the index cache, constant-length closed-form lists
+//   the dependent tasks are interleaved with the pool tasks of the heads pooled later, so they run under the HBM stream
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -335,7 +336,7 @@ struct HeadSets {
 //                            rows all have the same length, a block scan of the closed-form lengths otherwise.
 //   remaining CTAs          : the lists of the closed-form heads whose rows all have the same length (DENSE, UNIFORM_STRIDE,
 //                            STATIC/ANCHOR): 32 rows per CTA, written under the pooling's HBM time.
-constexpr int kPoolBlocksPerTask = 2;
+constexpr int kPoolBlocksPerTask = 8;  // one block per warp
 struct PoolJobs {
   int32_t n;                            // number of (tensor, head) jobs
   uint8_t head[2 * SAF3R_MAX_HEADS];
@@ -354,25 +355,32 @@ __device__ __forceinline__ uint4 ld_stream_16(const void *p) {
   return r;
 }
 
-// Probe of one QUERY_PROBE head, run by a whole CTA (256 threads) of the select launch: qbar = (1/N) sum_t q_t from the
+// Probe of one QUERY_PROBE head, run by a whole CTA (256 threads): qbar = (1/N) sum_t q_t from the
 // per-CTA token sums of the pool launch, p[J] = qbar . Ktilde_J / sqrt(D), top-n -> probe_list[h][0..n).
-__device__ inline void probe_head(const float *qpart, const float *kt, int32_t *probe_list, int32_t *head_lists, const SelGeom &g,
-                                  int h, int n, uint32_t *key /* dynamic smem, NB */, float (*part)[64], float *qb) {
+__device__ inline void probe_head(const float *qpart, const float *kt, int32_t *probe_list, const SelGeom &g, int h, int n,
+                                  uint32_t *key /* dynamic smem, NB */, float (*part)[64], float *qb) {
   const int nparts = (g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask;
   {
-    const int d = threadIdx.x & 63, grp = threadIdx.x >> 6;
-    const float *base = qpart + (int64_t)h * nparts * 64 + d;
-    float a0 = 0.f;
-    for (int c0 = grp; c0 < nparts; c0 += 32) {  // eight loads in flight, summed in a fixed order
-      float t[8];
+    // 16 groups of 16 threads; a thread owns four dimensions and every 16th partial sum (independent 16-byte loads, eight in flight);
+    // the groups are folded in a fixed order, so qbar does not depend on scheduling
+    const int d4 = threadIdx.x & 15, grp = threadIdx.x >> 4;
+    const float4 *base = reinterpret_cast<const float4 *>(qpart + (int64_t)h * nparts * 64) + d4;
+    float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int c0 = grp; c0 < nparts; c0 += 16 * 8) {
+      float4 t[8];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) t[i] = (c0 + 4 * i < nparts) ? __ldcg(base + (int64_t)(c0 + 4 * i) * 64) : 0.f;
+      for (int i = 0; i < 8; ++i) t[i] = (c0 + 16 * i < nparts) ? __ldcg(base + (int64_t)(c0 + 16 * i) * 16) : make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-      for (int i = 0; i < 8; ++i) a0 += t[i];
+      for (int i = 0; i < 8; ++i) { a.x += t[i].x; a.y += t[i].y; a.z += t[i].z; a.w += t[i].w; }
     }
-    part[grp][d] = a0;
+    *reinterpret_cast<float4 *>(&part[grp][4 * d4]) = a;
     __syncthreads();
-    if (threadIdx.x < 64) qb[threadIdx.x] = ((part[0][threadIdx.x] + part[1][threadIdx.x]) + (part[2][threadIdx.x] + part[3][threadIdx.x])) / (float)g.N;
+    if (threadIdx.x < 64) {
+      float sum = 0.f;
+#pragma unroll
+      for (int gq = 0; gq < 16; ++gq) sum += part[gq][threadIdx.x];
+      qb[threadIdx.x] = sum / (float)g.N;
+    }
     __syncthreads();
   }
   const int64_t ld = kt_stride(g.NB);
@@ -391,95 +399,62 @@ __device__ inline void probe_head(const float *qpart, const float *kt, int32_t *
   }
   __syncthreads();
   if (threadIdx.x < 32) warp_topn_bisect(key, g.NB, n, probe_list + (int64_t)h * g.NB);
-  __syncthreads();
-  // every q-block of the head gets the same list: its NB rows of n entries are contiguous in col_idx, so the region is the
-  // list repeated NB times; written here with coalesced stores while the score CTAs of the launch are still busy
-  int32_t *list = reinterpret_cast<int32_t *>(key);
-  for (int i = threadIdx.x; i < n; i += 256) list[i] = __ldcg(probe_list + (int64_t)h * g.NB + i);  // this CTA's own global writes
-  __syncthreads();
-  const int64_t total = (int64_t)g.NB * n;
-  int m = (int)(threadIdx.x % (unsigned)n);
-  const int step = 256 % n;
-  for (int64_t idx = threadIdx.x; idx < total; idx += 256) {
-    head_lists[idx] = list[m];
-    m += step;
-    if (m >= n) m -= n;
-  }
 }
 
-__global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
-                                                          float *__restrict__ qt, float *__restrict__ kt, float *__restrict__ qpart,
-                                                          int64_t *__restrict__ row_ptr, int32_t *__restrict__ col_idx, SelGeom g, PoolJobs jobs, RowPtrPlan plan,
-                                                          HeadCfgArray cfg, HeadSets sets, int pool_ctas, int pool_tasks) {
-  // programmatic dependent launch: let the select launch that follows become resident as this grid drains; it waits
-  // (griddepcontrol.wait) for this grid's completion before it reads anything written here
-  asm volatile("griddepcontrol.launch_dependents;");
-  if ((int)blockIdx.x >= pool_ctas + g.H) {
-    // ---------------------------------------------------------------- lists of a constant-length closed-form head
-    const int chunks = (g.NB + kLightRows - 1) / kLightRows;
-    const int e = (int)blockIdx.x - pool_ctas - g.H;
-    const int h = sets.emit[e / chunks];
-    const int I0 = (e % chunks) * kLightRows;
-    const int warp = threadIdx.x >> 5;
-    for (int r = warp; r < kLightRows && I0 + r < g.NB; r += 8)
-      emit_light_row(g, cfg.c[h], h, I0 + r, col_idx + plan.head_base[h] + (int64_t)(I0 + r) * plan.const_len[h], nullptr);
-    return;
-  }
-  if ((int)blockIdx.x >= pool_ctas) {
-    // ---------------------------------------------------------------- row_ptr of one head
-    const int h = blockIdx.x - pool_ctas;
-    int64_t *rp = row_ptr + (int64_t)h * g.NB;
-    const int64_t base = plan.head_base[h];
-    if (plan.const_len[h] >= 0) {
-      for (int I = threadIdx.x; I < g.NB; I += 256) rp[I] = base + (int64_t)I * plan.const_len[h];
-    } else {
-      __shared__ int64_t sums[256];
-      const int per = (g.NB + 255) / 256;
-      const int a = min(g.NB, (int)threadIdx.x * per), b = min(g.NB, a + per);
-      int64_t s = 0;
-      for (int I = a; I < b; ++I) s += row_length(g, cfg.c[h], I);
-      sums[threadIdx.x] = s;
+// row_ptr entries of head h (one task of the fused kernel, whole CTA)
+__device__ inline void rowptr_task(int64_t *__restrict__ row_ptr, const SelGeom &g, const RowPtrPlan &plan, const HeadCfgArray &cfg, int h,
+                                   int64_t *sums /* shared, 256 */) {
+  int64_t *rp = row_ptr + (int64_t)h * g.NB;
+  const int64_t base = plan.head_base[h];
+  if (plan.const_len[h] >= 0) {
+    for (int I = threadIdx.x; I < g.NB; I += 256) rp[I] = base + (int64_t)I * plan.const_len[h];
+  } else {
+    const int per = (g.NB + 255) / 256;
+    const int a = min(g.NB, (int)threadIdx.x * per), b = min(g.NB, a + per);
+    int64_t s = 0;
+    for (int I = a; I < b; ++I) s += row_length(g, cfg.c[h], I);
+    sums[threadIdx.x] = s;
+    __syncthreads();
+    for (int off = 1; off < 256; off <<= 1) {
+      int64_t v = (int)threadIdx.x >= off ? sums[threadIdx.x - off] : 0;
       __syncthreads();
-      for (int off = 1; off < 256; off <<= 1) {
-        int64_t v = (int)threadIdx.x >= off ? sums[threadIdx.x - off] : 0;
-        __syncthreads();
-        sums[threadIdx.x] += v;
-        __syncthreads();
-      }
-      int64_t run = base + (threadIdx.x ? sums[threadIdx.x - 1] : 0);
-      for (int I = a; I < b; ++I) {
-        rp[I] = run;
-        run += row_length(g, cfg.c[h], I);
-      }
+      sums[threadIdx.x] += v;
+      __syncthreads();
     }
-    if (h == g.H - 1 && threadIdx.x == 0) row_ptr[(int64_t)g.H * g.NB] = plan.head_base[g.H];
-    return;
+    int64_t run = base + (threadIdx.x ? sums[threadIdx.x - 1] : 0);
+    for (int I = a; I < b; ++I) {
+      rp[I] = run;
+      run += row_length(g, cfg.c[h], I);
+    }
   }
-  // ------------------------------------------------------------------ pool: four warps per token block, two blocks per task
-  // Task t of a job covers blocks 2t, 2t+1 (jobs are padded to a multiple of 2 blocks, so a task never straddles jobs); warp w
-  // takes quarter (w & 3) of block (w >> 2): B/4 token rows, one round of at most eight 16-byte loads per lane.  Small tasks
-  // keep the tail of the launch short (a warp that streams a whole 16 KB block alone needs four dependent DRAM round trips).
-  // The pool CTAs are persistent: pool_ctas <= 4 per SM of them stride over the pool_tasks tasks.
-  __shared__ float wsum[8][64];
+  if (h == g.H - 1 && threadIdx.x == 0) row_ptr[(int64_t)g.H * g.NB] = plan.head_base[g.H];
+}
+
+// One pool task (whole CTA): eight consecutive token blocks of one (tensor, head) job, ONE WARP PER BLOCK and no shared memory on
+// the way: a lane owns a 16-byte chunk (l & 7) of rows (l >> 3) + 4 i, eight independent 16-byte loads in flight per lane and
+// round of 32 rows, fp32 accumulate, optional per-token L2 normalisation (cosine), fold of the four row groups with shuffles,
+// mean -> Qtilde (row-major) or Ktilde^T (transposed).  The Q job of a QUERY_PROBE head also leaves each warp's token sum in
+// wsum for the task's partial sum of qbar, written by the caller after its barrier.
+__device__ __forceinline__ void pool_task(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k, float *__restrict__ qt,
+                                          float *__restrict__ kt, const SelGeom &g, const PoolJobs &jobs, int job, int task_in_job,
+                                          float (*wsum)[64]) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int tasks_per_job = (g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask;
   const int sub = lane & 7, rg = lane >> 3;
-  const int rows_q = g.B / 4;  // token rows per warp
-  for (int task = blockIdx.x; task < pool_tasks; task += pool_ctas) {
-    const int job = task / tasks_per_job, task_in_job = task % tasks_per_job;
-    const int J = task_in_job * kPoolBlocksPerTask + (warp >> 2);
-    const int h = jobs.head[job], which = jobs.which[job];
-    const bool want_part = jobs.probe[job] != 0 && which == 0;  // Q of a QUERY_PROBE head: also emit the task's token sum (qbar)
-    const bool cosine = jobs.cosine[job] != 0;
-    float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    if (J < g.NB) {
-      const int64_t t0 = (int64_t)J * g.B + (warp & 3) * rows_q;
-      const int cnt = (int)i64max(0, i64min(rows_q, g.N - t0));
-      const __nv_bfloat16 *src = (which ? k : q) + (int64_t)h * g.stride_head + t0 * g.stride_token + sub * 8;
+  const int J = task_in_job * kPoolBlocksPerTask + warp;
+  const int h = jobs.head[job], which = jobs.which[job];
+  const bool want_part = jobs.probe[job] != 0 && which == 0;
+  const bool cosine = jobs.cosine[job] != 0;
+  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (J < g.NB) {
+    const int64_t t0 = (int64_t)J * g.B;
+    const int cnt = (int)i64min(g.B, g.N - t0);
+    const __nv_bfloat16 *src = (which ? k : q) + (int64_t)h * g.stride_head + t0 * g.stride_token + sub * 8;
+#pragma unroll 1
+    for (int r0 = 0; r0 < cnt; r0 += 32) {
       uint4 raw[8];
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
-        const int r = rg + 4 * i;
+        const int r = r0 + rg + 4 * i;
         raw[i] = make_uint4(0, 0, 0, 0);
         if (r < cnt) raw[i] = ld_stream_16(src + (int64_t)r * g.stride_token);
       }
@@ -506,34 +481,27 @@ __global__ void __launch_bounds__(256, 4) pool_rowptr_kernel(const __nv_bfloat16
 #pragma unroll
         for (int c = 0; c < 8; ++c) acc[c] = fmaf(v[c], inv, acc[c]);
       }
+    }
 #pragma unroll
-      for (int c = 0; c < 8; ++c) {
-        acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 8);
-        acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 16);
-      }
+    for (int c = 0; c < 8; ++c) {
+      acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 8);
+      acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], 16);
     }
     if (rg == 0) {
+      if (which == 0) {
+        float4 *dst = reinterpret_cast<float4 *>(qt + ((int64_t)h * g.NB + J) * 64 + sub * 8);  // Qtilde row-major [H][NB][64]
+        dst[0] = make_float4(acc[0] / (float)cnt, acc[1] / (float)cnt, acc[2] / (float)cnt, acc[3] / (float)cnt);
+        dst[1] = make_float4(acc[4] / (float)cnt, acc[5] / (float)cnt, acc[6] / (float)cnt, acc[7] / (float)cnt);
+      } else {
+        float *dst = kt + ((int64_t)h * 64 + sub * 8) * kt_stride(g.NB) + J;                    // Ktilde transposed [H][64][NBp]
 #pragma unroll
-      for (int c = 0; c < 8; ++c) wsum[warp][sub * 8 + c] = acc[c];  // zero for warps past the last block / token
-    }
-    __syncthreads();
-    if (threadIdx.x < 64 * kPoolBlocksPerTask) {  // block sums in a fixed order (quarters 0..3), mean, store
-      const int bb = threadIdx.x >> 6, d = threadIdx.x & 63;
-      const int Jb = task_in_job * kPoolBlocksPerTask + bb;
-      if (Jb < g.NB) {
-        const float sum = (wsum[4 * bb][d] + wsum[4 * bb + 1][d]) + (wsum[4 * bb + 2][d] + wsum[4 * bb + 3][d]);
-        const float mean = sum / (float)i64min(g.B, g.N - (int64_t)Jb * g.B);
-        if (which == 0) qt[((int64_t)h * g.NB + Jb) * 64 + d] = mean;                    // Qtilde row-major [H][NB][64]
-        else kt[((int64_t)h * 64 + d) * kt_stride(g.NB) + Jb] = mean;                   // Ktilde transposed [H][64][NBp]
+        for (int c = 0; c < 8; ++c) dst[(int64_t)c * kt_stride(g.NB)] = acc[c] / (float)cnt;
       }
-    } else if (want_part && threadIdx.x >= 192) {  // the task's token sum, for qbar
-      const int d = threadIdx.x - 192;
-      float t = 0.f;
-#pragma unroll
-      for (int w = 0; w < 8; ++w) t += wsum[w][d];
-      qpart[((int64_t)h * tasks_per_job + task_in_job) * 64 + d] = t;
     }
-    __syncthreads();  // wsum is reused by this CTA's next task
+  }
+  if (want_part && rg == 0) {
+#pragma unroll
+    for (int c = 0; c < 8; ++c) wsum[warp][sub * 8 + c] = acc[c];  // zero for warps past the last block
   }
 }
 
@@ -558,6 +526,9 @@ __device__ __forceinline__ uint64_t sel_fma2(uint64_t a, uint64_t b, uint64_t c)
   return d;
 }
 
+// (Qtilde / Ktilde^T were written earlier in the SAME launch by other CTAs.  Reading them through L1 / the read-only path is safe
+// here: no thread of this SM touches a line of head h before the acquire that follows the head's last pool task, L1 is empty of
+// them at kernel start, and the GPU never prefetches into L1 - so the first touch fetches the finished line from L2.)
 // Score rows I0 .. I0+rows-1 (rows <= RT) of head h against every k-block: keys[r][J] = key(Qtilde_{I0+r} . Ktilde_J * cs).
 // Groups of 1024 columns: each thread owns four consecutive columns (one 16-byte load of Ktilde^T per d, coalesced across
 // the warp) and RT rows, 4*RT accumulators as packed row pairs.  The columns left over (< 1024) are spread over all threads
@@ -657,68 +628,192 @@ __device__ __forceinline__ void score_rows(const float *__restrict__ qt, const f
   }
 }
 
-__global__ void __launch_bounds__(256, 2) select_kernel(const float *__restrict__ qt, const float *__restrict__ kt,
-                                                        const int32_t *__restrict__ probe_list, const int64_t *__restrict__ row_ptr,
-                                                        const float *__restrict__ qpart, int32_t *__restrict__ probe_out,
-                                                        int32_t *__restrict__ col_idx, const int64_t *__restrict__ cache_row_ptr,
-                                                        const int32_t *__restrict__ cache_col_idx, SelGeom g, HeadCfgArray cfg,
-                                                        HeadSets sets, int R) {
-  const int warp = threadIdx.x >> 5;
-  extern __shared__ float sm[];
-  __shared__ float part[4][64];
-  __shared__ float qb[64];
-  asm volatile("griddepcontrol.wait;" ::: "memory");  // the pool launch has completed and its writes are visible
-  const int strips = (g.NB + R - 1) / R;
-  const int probe_ctas = sets.n_probe;
-  const int heavy_ctas = sets.n_block * strips;
-  if ((int)blockIdx.x < probe_ctas) {
-    const int h = sets.probe[blockIdx.x];
-    probe_head(qpart, kt, probe_out, col_idx + row_ptr[(int64_t)h * g.NB], g, h, (int)i64min(cfg.c[h].keep_blocks, g.NB),
-               reinterpret_cast<uint32_t *>(sm), part, qb);
-    return;
-  }
-  const int bid = (int)blockIdx.x - probe_ctas;
-  if (bid >= heavy_ctas) {
-    // light CTAs come last in launch order, 32 rows each: per-row-length STATIC heads, then CACHED heads
-    const int chunks = (g.NB + kLightRows - 1) / kLightRows;
-    const int e = bid - heavy_ctas;
-    const int I0 = (e % chunks) * kLightRows;
-    if (e / chunks >= sets.n_light) {
-      const int h = sets.cached[e / chunks - sets.n_light];
-      const int src = cfg.c[h].offset;
-      const int lane = threadIdx.x & 31;
-      for (int r = warp; r < kLightRows && I0 + r < g.NB; r += 8) {
-        const int64_t a = cache_row_ptr[(int64_t)src * g.NB + I0 + r], b = cache_row_ptr[(int64_t)src * g.NB + I0 + r + 1];
-        const int64_t o = row_ptr[(int64_t)h * g.NB + I0 + r], cap = row_ptr[(int64_t)h * g.NB + I0 + r + 1] - o;
-        const int64_t n = i64min(b - a, cap);  // equal when cfg repeats the source rule; never write past the row
-        for (int64_t i = lane; i < n; i += 32) col_idx[o + i] = cache_col_idx[a + i];
-      }
-      return;
-    }
-    const int h = sets.light[e / chunks];
-    for (int r = warp; r < kLightRows && I0 + r < g.NB; r += 8)
-      emit_light_row(g, cfg.c[h], h, I0 + r, col_idx + row_ptr[(int64_t)h * g.NB + I0 + r], probe_list);
-    return;
-  }
-  const int h = sets.block[bid / strips];
-  const saf3r_head_cfg c = cfg.c[h];
-  const int I0 = (bid % strips) * R;
-  const int rows = (int)i64min(R, g.NB - I0);
+// ------------------------------------------------------------------------------------------------ the fused selection kernel
+// ONE persistent launch for the whole of saf3r_select.  CTAs (256 threads, <= 2 per SM) draw tickets from a device counter; the
+// ticket order is a host-side closed form of (shape, cfg):
+//   [row_ptr task per head] [pool tasks of the BLOCK_TOPK heads] [MIX: pool tasks of the QUERY_PROBE heads with one score strip
+//   after every `period` of them] [what is left of either] [probe tasks] [light chunks] [emit chunks] [probe-list copies]
+// score strip: R q-block rows of a BLOCK_TOPK head (scores in shared memory, top-n / per-frame top-k); probe task: one per
+// QUERY_PROBE head (qbar, probe row, top-n -> the head's list); light chunk: 32 rows of a per-row STATIC rule or of a CACHED head;
+// emit chunk: 32 rows of a constant-length closed-form list; copy chunk: 32 of the NB identical rows of a QUERY_PROBE head.  So the score + select work of the BLOCK_TOPK heads and every list
+// write run UNDER the HBM stream of the remaining pooling instead of after it, and nothing is launched twice.
+// A task that needs the pooled tensors of head h spins (one thread, ld.acquire) on pooled[h]; every pool task ends with a
+// release increment of it.  All tasks a waiter depends on have SMALLER tickets, i.e. were drawn by CTAs that are running and never
+// wait on larger tickets: no deadlock whatever the grid size.  Light / CACHED tasks wait the same way for the head's row_ptr.
+struct FusedPlan {
+  int32_t t_begin, t_end;                 // tickets this launch serves (two launches when the stages are timed separately)
+  int32_t n_rowptr, n_pool_a, n_pool_b;   // tasks per segment
+  int32_t n_x, period;                    // score strips (mixed into the pool-B tasks, one after every `period` of them, >= 1)
+  int32_t n_probe, n_light, n_emit, n_rep;  // after ALL pool tasks: probe tasks, light chunks, emit chunks, probe-list copies
+  int32_t strips, R, light_chunks;
+  int32_t pool_need;                      // pool tasks per head = 2 jobs * tasks_per_job
+  int32_t counter;                        // which ticket counter (0 / 1)
+};
+constexpr int kSelScratch = 17 * 64 * 4;  // bytes of task scratch besides the keys of a probe task (partial sums of qbar, qbar)
+constexpr int kSelCounters = 2 + 3 * SAF3R_MAX_HEADS;  // int32: 2 ticket counters, pooled[h], rowptr_done[h], probe_done[h]
 
-  uint32_t *keys = reinterpret_cast<uint32_t *>(sm);   // [R][NBp]
-  const int64_t ld = kt_stride(g.NB);                  // key rows are padded like Ktilde^T
-  float *qT = sm + (size_t)R * ld;                     // [64][RT] (rows past `rows` are zero)
-  const float cs = c.score_mode == SAF3R_SCORE_COSINE ? 1.f : 0.125f;
-  if (R <= 4) score_rows<4>(qt, kt, keys, qT, g, h, I0, rows, cs);
-  else if (R <= 8) score_rows<8>(qt, kt, keys, qT, g, h, I0, rows, cs);
-  else score_rows<kSelRows>(qt, kt, keys, qT, g, h, I0, rows, cs);
+__device__ __forceinline__ void wait_count(const int *ctr, int need) {
+  if (threadIdx.x == 0) {
+    int v;
+    do {
+      asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+      if (v < need) __nanosleep(200);
+    } while (v < need);
+  }
   __syncthreads();
-  for (int r = warp; r < rows; r += 8) {
-    int32_t *out = col_idx + row_ptr[(int64_t)h * g.NB + I0 + r];
-    if (c.topk_scope == SAF3R_SCOPE_GLOBAL)
-      warp_topn_bisect(keys + (size_t)r * ld, g.NB, (int)i64min(c.keep_blocks, g.NB), out);
-    else
-      warp_per_frame_emit(keys + (size_t)r * ld, g, c.topk_per_frame, out);
+}
+__device__ __forceinline__ void signal_count(int *ctr) {
+  __syncthreads();  // all threads of the CTA have issued their stores
+  if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(ctr) : "memory");  // release: cumulative over the barrier
+}
+
+__global__ void __launch_bounds__(256, 2) select_fused_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
+                                                              float *__restrict__ qt, float *__restrict__ kt, float *__restrict__ qpart,
+                                                              int32_t *__restrict__ probe_list, int64_t *__restrict__ row_ptr,
+                                                              int32_t *__restrict__ col_idx, const int64_t *__restrict__ cache_row_ptr,
+                                                              const int32_t *__restrict__ cache_col_idx, int *__restrict__ counters,
+                                                              SelGeom g, PoolJobs jobs, RowPtrPlan plan, HeadCfgArray cfg, HeadSets sets,
+                                                              FusedPlan fp) {
+  extern __shared__ __align__(16) float sm[];  // per task: score keys + Qtilde^T | probe keys | the scratch below (>= kSelScratch bytes)
+  float(*wsum)[64] = reinterpret_cast<float(*)[64]>(sm);      // pool task: [8][64]
+  int64_t *sums = reinterpret_cast<int64_t *>(sm);             // row_ptr task: [256]
+  __shared__ int s_ticket;
+  int *pooled = counters + 2, *rp_done = counters + 2 + SAF3R_MAX_HEADS, *probe_done = counters + 2 + 2 * SAF3R_MAX_HEADS;
+  const int warp = threadIdx.x >> 5;
+  // thread 0 always holds the NEXT ticket: its atomic is issued a whole task ahead, so its latency never shows
+  int next = 0;
+  if (threadIdx.x == 0) next = fp.t_begin + atomicAdd(counters + fp.counter, 1);
+  for (;;) {
+    __syncthreads();  // the previous task is finished with the shared buffers (and with s_ticket)
+    if (threadIdx.x == 0) s_ticket = next;
+    __syncthreads();
+    int t = s_ticket;
+    if (t >= fp.t_end) break;
+    if (threadIdx.x == 0) next = fp.t_begin + atomicAdd(counters + fp.counter, 1);
+    // ---------------------------------------------------------------- decode the ticket
+    int pool_task_id = -1, x = -1;
+    if (t < fp.n_rowptr) {
+      rowptr_task(row_ptr, g, plan, cfg, t, sums);
+      signal_count(rp_done + t);
+      continue;
+    }
+    t -= fp.n_rowptr;
+    if (t < fp.n_pool_a) {
+      pool_task_id = t;
+    } else {
+      t -= fp.n_pool_a;
+      const int groups = min(fp.n_x, fp.n_pool_b / fp.period);  // full (period pool tasks, one dependent task) groups
+      const int mixed = groups * (fp.period + 1);
+      if (t < mixed) {
+        const int gi = t / (fp.period + 1), r = t % (fp.period + 1);
+        if (r < fp.period) pool_task_id = fp.n_pool_a + gi * fp.period + r;
+        else x = gi;
+      } else {
+        t -= mixed;
+        const int rest_pool = fp.n_pool_b - groups * fp.period;
+        if (t < rest_pool) pool_task_id = fp.n_pool_a + groups * fp.period + t;
+        else x = groups + (t - rest_pool);  // past n_x: the probe tasks
+      }
+    }
+    if (pool_task_id >= 0) {
+      const int tasks_per_job = (g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask;
+      const int job = pool_task_id / tasks_per_job, task_in_job = pool_task_id % tasks_per_job;
+      pool_task(q, k, qt, kt, g, jobs, job, task_in_job, wsum);
+      if (jobs.probe[job] != 0 && jobs.which[job] == 0) {  // the task's token sum for qbar, warps in a fixed order
+        __syncthreads();
+        if (threadIdx.x < 64) {
+          float tsum = 0.f;
+#pragma unroll
+          for (int w = 0; w < 8; ++w) tsum += wsum[w][threadIdx.x];
+          qpart[((int64_t)jobs.head[job] * tasks_per_job + task_in_job) * 64 + threadIdx.x] = tsum;
+        }
+      }
+      signal_count(pooled + jobs.head[job]);
+      continue;
+    }
+    // ---------------------------------------------------------------- dependent tasks
+    if (x < fp.n_x) {
+      const int h = sets.block[x / fp.strips];
+      const saf3r_head_cfg c = cfg.c[h];
+      const int R = fp.R, I0 = (x % fp.strips) * R;
+      const int rows = (int)i64min(R, g.NB - I0);
+      wait_count(pooled + h, fp.pool_need);
+      uint32_t *keys = reinterpret_cast<uint32_t *>(sm);   // [R][NBp]
+      const int64_t ld = kt_stride(g.NB);
+      float *qT = sm + (size_t)R * ld;                     // [64][RT] (rows past `rows` are zero)
+      const float cs = c.score_mode == SAF3R_SCORE_COSINE ? 1.f : 0.125f;
+      if (R <= 4) score_rows<4>(qt, kt, keys, qT, g, h, I0, rows, cs);
+      else if (R <= 8) score_rows<8>(qt, kt, keys, qT, g, h, I0, rows, cs);
+      else score_rows<kSelRows>(qt, kt, keys, qT, g, h, I0, rows, cs);
+      __syncthreads();
+      const int64_t base = plan.head_base[h];  // BLOCK_TOPK rows all have the same length: offsets are a closed form
+      const int len = plan.const_len[h];
+      for (int r = warp; r < rows; r += 8) {
+        int32_t *out = col_idx + base + (int64_t)(I0 + r) * len;
+        if (c.topk_scope == SAF3R_SCOPE_GLOBAL) warp_topn_bisect(keys + (size_t)r * ld, g.NB, (int)i64min(c.keep_blocks, g.NB), out);
+        else warp_per_frame_emit(keys + (size_t)r * ld, g, c.topk_per_frame, out);
+      }
+      continue;
+    }
+    x -= fp.n_x;
+    if (x < fp.n_probe) {
+      const int h = sets.probe[x];
+      wait_count(pooled + h, fp.pool_need);
+      float(*part)[64] = reinterpret_cast<float(*)[64]>(sm + kt_stride(g.NB));  // behind the NB probe keys: [16][64], then qbar [64]
+      probe_head(qpart, kt, probe_list, g, h, (int)i64min(cfg.c[h].keep_blocks, g.NB), reinterpret_cast<uint32_t *>(sm), part,
+                 sm + kt_stride(g.NB) + 16 * 64);
+      signal_count(probe_done + h);
+      continue;
+    }
+    x -= fp.n_probe;
+    if (x < fp.n_light) {
+      const int I0 = (x % fp.light_chunks) * kLightRows, hi = x / fp.light_chunks;
+      if (hi >= sets.n_light) {  // CACHED head: rows copied from the index cache
+        const int h = sets.cached[hi - sets.n_light];
+        wait_count(rp_done + h, 1);
+        const int src = cfg.c[h].offset, lane = threadIdx.x & 31;
+        for (int r = warp; r < kLightRows && I0 + r < g.NB; r += 8) {
+          const int64_t a = cache_row_ptr[(int64_t)src * g.NB + I0 + r], b = cache_row_ptr[(int64_t)src * g.NB + I0 + r + 1];
+          const int64_t o = row_ptr[(int64_t)h * g.NB + I0 + r], cap = row_ptr[(int64_t)h * g.NB + I0 + r + 1] - o;
+          const int64_t n = i64min(b - a, cap);  // equal when cfg repeats the source rule; never write past the row
+          for (int64_t i = lane; i < n; i += 32) col_idx[o + i] = cache_col_idx[a + i];
+        }
+      } else {
+        const int h = sets.light[hi];
+        wait_count(rp_done + h, 1);
+        for (int r = warp; r < kLightRows && I0 + r < g.NB; r += 8)
+          emit_light_row(g, cfg.c[h], h, I0 + r, col_idx + row_ptr[(int64_t)h * g.NB + I0 + r], nullptr);
+      }
+      continue;
+    }
+    x -= fp.n_light;
+    if (x < fp.n_emit) {  // constant-length closed-form head: no dependence at all
+      const int h = sets.emit[x / fp.light_chunks];
+      const int I0 = (x % fp.light_chunks) * kLightRows;
+      for (int r = warp; r < kLightRows && I0 + r < g.NB; r += 8)
+        emit_light_row(g, cfg.c[h], h, I0 + r, col_idx + plan.head_base[h] + (int64_t)(I0 + r) * plan.const_len[h], nullptr);
+      continue;
+    }
+    x -= fp.n_emit;
+    {  // 32 of the NB identical rows of a QUERY_PROBE head: the region is the head's list repeated, written with coalesced stores
+      const int h = sets.probe[x / fp.light_chunks];
+      const int I0 = (x % fp.light_chunks) * kLightRows;
+      const int n = (int)i64min(cfg.c[h].keep_blocks, g.NB);
+      wait_count(probe_done + h, 1);
+      int32_t *list = reinterpret_cast<int32_t *>(sm);
+      for (int i = threadIdx.x; i < n; i += 256) list[i] = __ldcg(probe_list + (int64_t)h * g.NB + i);
+      __syncthreads();
+      const int nrows = min(kLightRows, g.NB - I0);
+      int32_t *dst = col_idx + plan.head_base[h] + (int64_t)I0 * n;
+      const int64_t total = (int64_t)nrows * n;
+      int m = (int)(((int64_t)threadIdx.x) % n);
+      const int step = 256 % n;
+      for (int64_t idx = threadIdx.x; idx < total; idx += 256) {
+        dst[idx] = list[m];
+        m += step;
+        if (m >= n) m -= n;
+      }
+    }
   }
 }
 
