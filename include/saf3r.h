@@ -252,6 +252,14 @@ saf3r_status saf3r_static_broadcast_attn(saf3r_ctx *ctx, const void *q_dev, cons
                                          const saf3r_shape *shape, void *workspace_dev, size_t workspace_bytes, void *out_dev,
                                          int out_is_fp32, float *lse_dev_or_null, void *cuda_stream);
 
+/* ---- Offline head profiling aid (Eq. 1) ------------------------------------------------
+ * E(c) = E_calib[ ||O_full - O_sparse||^2 / ||O_full||^2 ] per head.  saf3r_nmse_accumulate ADDS, for every head h of the call,
+ * sum (o_full - o_sparse)^2 to num_den_dev[h] and sum o_full^2 to num_den_dev[H + h] (double accumulators, caller-zeroed, so that
+ * several calibration samples can be accumulated); the caller divides.  o_full / o_sparse: two attention outputs with the
+ * layout of `shape` (both bf16 or both fp32).  One launch; enqueues and returns. */
+saf3r_status saf3r_nmse_accumulate(saf3r_ctx *ctx, const void *o_full_dev, const void *o_sparse_dev, const saf3r_shape *shape,
+                                   int is_fp32, double *num_den_dev, void *cuda_stream);
+
 /* Measurement aid ("select ms split into pool and score+select stages").  When enabled, saf3r_select records
  * CUDA events on its stream before the pool launch, between the two launches and after the select launch (three
  * cudaEventRecord calls, no synchronisation).  saf3r_last_select_stage_ms blocks until the last timed saf3r_select has

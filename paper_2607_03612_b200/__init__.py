@@ -29,7 +29,7 @@ EXPORTS = ("saf3r_create", "saf3r_destroy", "saf3r_last_error", "saf3r_query_siz
            "saf3r_set_stage_timing", "saf3r_last_select_stage_ms", "saf3r_select_cached", "saf3r_token_stride_attn",
            "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn", "saf3r_check_lists", "saf3r_select_plan", "saf3r_union_lists",
            "saf3r_static_broadcast_workspace_bytes", "saf3r_static_broadcast_attn", "saf3r_token_topk_query_sizes",
-           "saf3r_token_topk_select", "saf3r_token_lists_count", "saf3r_token_lists_fill", "saf3r_token_lists_attn")
+           "saf3r_token_topk_select", "saf3r_token_lists_count", "saf3r_token_lists_fill", "saf3r_token_lists_attn", "saf3r_nmse_accumulate")
 
 
 class Saf3rError(RuntimeError):
@@ -96,6 +96,7 @@ def load_library():
         L.saf3r_token_lists_count.argtypes = [vp, C.POINTER(ShapeC), C.c_int32, vp, vp, vp]
         L.saf3r_token_lists_fill.argtypes = [vp, C.POINTER(ShapeC), C.c_int32, vp, C.POINTER(TokenListsC), vp]
         L.saf3r_token_lists_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(TokenListsC), vp, i32, vp, vp]
+        L.saf3r_nmse_accumulate.argtypes = [vp, vp, vp, C.POINTER(ShapeC), i32, vp, vp]
         L.saf3r_launch_count.argtypes = [vp]
         L.saf3r_launch_count.restype = i64
         L.saf3r_set_stage_timing.argtypes = [vp, i32]
@@ -370,6 +371,19 @@ class Context:
                                                     out.data_ptr(), int(out_fp32), lse.data_ptr() if lse is not None else None,
                                                     _stream_ptr(stream)))
         return (out, lse) if want_lse else out
+
+    # ---- saf3r_nmse_accumulate
+    def nmse(self, o_full, o_sparse, shape: ShapeC, stream=None) -> list[float]:
+        """Eq. 1 per head for one sample: ||O_full - O_sparse||^2 / ||O_full||^2, both sums in the library."""
+        import torch
+        acc = torch.zeros(2 * shape.num_heads, dtype=torch.float64, device=o_full.device)
+        _on_stream(stream, acc)
+        assert o_full.dtype == o_sparse.dtype
+        self._check(self.lib.saf3r_nmse_accumulate(self.h, o_full.data_ptr(), o_sparse.data_ptr(), C.byref(shape),
+                                                   int(o_full.dtype == torch.float32), acc.data_ptr(), _stream_ptr(stream)))
+        a = acc.cpu().tolist()
+        H = shape.num_heads
+        return [a[h] / a[H + h] for h in range(H)]
 
     # ---- saf3r_static_broadcast_attn
     def static_broadcast_attn(self, q, k, v, shape: ShapeC, workspace=None, out=None, out_fp32=False, want_lse=False, stream=None):

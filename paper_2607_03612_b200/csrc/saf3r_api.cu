@@ -720,6 +720,22 @@ saf3r_status saf3r_token_set_attn(saf3r_ctx *ctx, const void *q, const void *k, 
   return attn_common(ctx, q, kc, vc, shape, nullptr, out, out_is_fp32, lse, stream_, &kv);
 }
 
+saf3r_status saf3r_nmse_accumulate(saf3r_ctx *ctx, const void *o_full, const void *o_sparse, const saf3r_shape *shape, int is_fp32,
+                                   double *num_den, void *stream_) {
+  if (!ctx) return SAF3R_ERR_INVALID_ARG;
+  if (ctx->sticky_cuda) return SAF3R_ERR_CUDA;
+  if (const char *m = validate_shape(shape, true)) return fail(ctx, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
+  if (!o_full || !o_sparse || !num_den) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  if (((uintptr_t)o_full | (uintptr_t)o_sparse) & 15) return fail(ctx, SAF3R_ERR_INVALID_ARG, "outputs must be 16-byte aligned");
+  const SelGeom g = make_geom(shape);
+  nmse_kernel<<<dim3(4 * ctx->sm_count / (g.H < 4 ? g.H : 4) + 1, g.H), 256, 0, (cudaStream_t)stream_>>>(
+      (const uint8_t *)o_full, (const uint8_t *)o_sparse, g.N, g.stride_head, g.stride_token, is_fp32 ? 1 : 0, num_den, num_den + g.H);
+  ctx->launches += 1;
+  CU_CHECK(cudaGetLastError());
+  return SAF3R_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ token-wise per-frame Top-K (NEXT-2 iii)
 struct TokTopkWs { size_t rn, keys, total; int64_t ld; int strips; };
 static TokTopkWs toktopk_ws(int64_t N) {

@@ -326,4 +326,55 @@ __global__ void __launch_bounds__(256) frame_broadcast_kernel(uint8_t *__restric
   if (lse != nullptr && c == 0) lse[(int64_t)h * g.N + (int64_t)f * g.T + p] = lse0[(int64_t)h * g.T + p] + logf((float)g.S);
 }
 
+// ------------------------------------------------------------------------------------------------ Eq. 1 (NEXT-3)
+// num[h] += sum (o_full - o_sparse)^2, den[h] += sum o_full^2 over one head's [N][64] outputs (bf16 or fp32), double accumulators;
+// E(c) = num / den (Eq. 1).  grid (chunks, H), 256 threads, grid-stride over 16-byte chunks, one atomicAdd(double)
+// pair per CTA (the two sums are order-dependent only in the last bits of a double).
+__global__ void __launch_bounds__(256) nmse_kernel(const uint8_t *__restrict__ a, const uint8_t *__restrict__ b, int64_t N, int64_t stride_head,
+                                                   int64_t stride_token, int is_fp32, double *__restrict__ num, double *__restrict__ den) {
+  const int h = blockIdx.y;
+  const int per_row = is_fp32 ? 16 : 8;  // 16-byte chunks per 64-element row
+  const int esz = is_fp32 ? 4 : 2;
+  double n = 0.0, d = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < N * per_row; i += (int64_t)gridDim.x * 256) {
+    const int64_t off = ((int64_t)h * stride_head + (i / per_row) * stride_token) * esz + (i % per_row) * 16;
+    const uint4 ra = *reinterpret_cast<const uint4 *>(a + off), rb = *reinterpret_cast<const uint4 *>(b + off);
+    if (is_fp32) {
+      const float fa[4] = {__uint_as_float(ra.x), __uint_as_float(ra.y), __uint_as_float(ra.z), __uint_as_float(ra.w)};
+      const float fb[4] = {__uint_as_float(rb.x), __uint_as_float(rb.y), __uint_as_float(rb.z), __uint_as_float(rb.w)};
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const double x = fa[c], y = fb[c];
+        n += (x - y) * (x - y);
+        d += x * x;
+      }
+    } else {
+      float fa[8], fb[8];
+      bf16x8_to_f32(ra, fa);
+      bf16x8_to_f32(rb, fb);
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        const double x = fa[c], y = fb[c];
+        n += (x - y) * (x - y);
+        d += x * x;
+      }
+    }
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    n += __shfl_xor_sync(0xffffffffu, n, off);
+    d += __shfl_xor_sync(0xffffffffu, d, off);
+  }
+  __shared__ double sn[8], sd[8];
+  if ((threadIdx.x & 31) == 0) { sn[threadIdx.x >> 5] = n; sd[threadIdx.x >> 5] = d; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tn = 0.0, td = 0.0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) { tn += sn[w]; td += sd[w]; }
+    atomicAdd(num + h, tn);
+    atomicAdd(den + h, td);
+  }
+}
+
 }  // namespace saf3r

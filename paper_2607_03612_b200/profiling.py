@@ -9,7 +9,7 @@ and keep   c* = argmin_{c in C_h + {c_base}} E(c)  s.t.  Omega(c) <= Omega(c_bas
 
 with Omega = executed FLOP of the block-sparse attention (4*B^2*D per listed block pair, a closed form of (shape, c)).
 O_full comes from saf3r_dense_attn, O_sparse from saf3r_select + saf3r_sparse_attn; heads are independent, so one call
-evaluates a candidate on every head at once.  The reductions of Eq. 1 use torch (offline tooling, not the hot path).
+evaluates a candidate on every head at once.  The two sums of Eq. 1 run in the library too (saf3r_nmse_accumulate).
 The paper's calibration data (10 ETH3D sequences) is not available; callers pass their own layers.
 """
 from __future__ import annotations
@@ -61,13 +61,10 @@ def candidate_set(shape: ShapeC, sigma: float) -> list[dict]:
     return out
 
 
-def nmse_per_head(o_full, o_sparse):
-    """Eq. 1 for one calibration sample: ||O_full - O_sparse||_F^2 / ||O_full||_F^2 per head ([H][N][D] tensors)."""
-    import torch
-    a, b = o_full.float(), o_sparse.float()
-    num = (a - b).pow(2).sum(dim=(1, 2), dtype=torch.float64)
-    den = a.pow(2).sum(dim=(1, 2), dtype=torch.float64)
-    return (num / den).cpu().tolist()
+def nmse_per_head(ctx: Context, o_full, o_sparse, shape: ShapeC):
+    """Eq. 1 for one calibration sample: ||O_full - O_sparse||_F^2 / ||O_full||_F^2 per head ([H][N][D] tensors); both sums run in
+    the library (saf3r_nmse_accumulate, double accumulators)."""
+    return ctx.nmse(o_full, o_sparse, shape)
 
 
 @dataclass
@@ -97,7 +94,7 @@ def profile_heads(ctx: Context, layers, shape: ShapeC, sigma: float = 0.85, cand
                 continue
             lists = ctx.select(q, k, shape, [c] * H)
             o = ctx.sparse_attn(q, k, v, shape, lists, out_fp32=True)
-            e = nmse_per_head(o_full, o)
+            e = nmse_per_head(ctx, o_full, o, shape)
             for h in range(H):
                 err[ci][h] += e[h] / len(layers)
         torch.cuda.synchronize()
