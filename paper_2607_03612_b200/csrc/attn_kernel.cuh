@@ -36,7 +36,7 @@ struct AttnParams {
   int32_t out_fp32;
   float scale_log2;  // (1/sqrt(D)) * log2(e)
   const float *kmax;  // [H] max_j |k_j|_2 over the head's key tokens (knorm_kernel), or nullptr: never freeze the max
-  uint8_t head_order[SAF3R_MAX_HEADS];  // blockIdx.y -> head, longest lists first
+  const uint8_t *head_order;  // dev, blockIdx.y -> head, longest lists first (knorm_kernel); nullptr: identity
   // token-list mode (kTok; SURVEY 8(f) NEXT-2 iii): the k-tiles of q-tile I are tiles [tile_ptr[I], tile_ptr[I+1]) of B gathered key
   // tokens each (key_idx, -1 = padding), shared by all heads; mask bit (row r, column c) of a tile says whether query r keeps key c
   const int64_t *tile_ptr;
@@ -289,7 +289,7 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
   using L = AttnSmem<B>;
   const uint32_t sbase = smem_u32(smem);
   const int warp = threadIdx.x >> 5;
-  const int I = blockIdx.x, h = p.head_order[blockIdx.y];
+  const int I = blockIdx.x, h = p.head_order ? p.head_order[blockIdx.y] : (int)blockIdx.y;
 
   const uint32_t bar = sbase + L::kBar;
   const uint32_t bar_q = bar + 0;
@@ -454,11 +454,30 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
 // kmax[h] = max over the head's key tokens of |k_j|_2 (the Cauchy-Schwarz factor of the freeze test above).  One streaming pass
 // over K: grid (chunks, H), 256 threads, 8 lanes per 128-byte token row with eight 16-byte loads in flight per lane; the norms
 // are non-negative, so the maximum of their bit patterns as unsigned integers is the maximum of the floats (atomicMax into a
-// zeroed slot).
+// zeroed slot).  Thread 0 of CTA (0, 0) also writes the head order of the attention launch.
 constexpr int kKnormRows = 1024;  // token rows per CTA
 __global__ void __launch_bounds__(256) knorm_kernel(const __nv_bfloat16 *__restrict__ k, int64_t n_kv, int64_t stride_head,
-                                                    int64_t stride_token, float *__restrict__ kmax) {
+                                                    int64_t stride_token, float *__restrict__ kmax, const int64_t *__restrict__ row_ptr,
+                                                    int NB, uint8_t *__restrict__ head_order) {
   const int h = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) {
+    // scheduling aid for the attention launch that follows: heads by total list length, longest first (stable insertion sort of
+    // at most SAF3R_MAX_HEADS entries; dense mode / token lists: identity)
+    const int H = gridDim.y;
+    int64_t len[SAF3R_MAX_HEADS];
+    uint8_t ord[SAF3R_MAX_HEADS];
+    for (int i = 0; i < H; ++i) {
+      len[i] = row_ptr ? row_ptr[(int64_t)(i + 1) * NB] - row_ptr[(int64_t)i * NB] : 0;
+      ord[i] = (uint8_t)i;
+    }
+    for (int a = 1; a < H; ++a)
+      for (int b = a; b > 0 && len[ord[b - 1]] < len[ord[b]]; --b) {
+        const uint8_t t = ord[b];
+        ord[b] = ord[b - 1];
+        ord[b - 1] = t;
+      }
+    for (int i = 0; i < H; ++i) head_order[i] = ord[i];
+  }
   const int sub = lane & 7, rg = lane >> 3;
   const int64_t t0 = (int64_t)blockIdx.x * kKnormRows + warp * (kKnormRows / 8);
   const __nv_bfloat16 *src = k + (int64_t)h * stride_head + sub * 8;

@@ -32,6 +32,7 @@ struct MapKey {
 
 constexpr size_t kMapCacheEntries = 512;
 constexpr uint32_t kKmaxSlots = 256;
+constexpr size_t kKmaxSlotFloats = SAF3R_MAX_HEADS + SAF3R_MAX_HEADS / 4;  // kmax[H] floats + head_order[H] bytes
 
 struct saf3r_ctx {
   int device = 0;
@@ -51,9 +52,6 @@ struct saf3r_ctx {
   cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};  // select: start, after the pool launch, after the select launch
   bool ev_valid = false;
   std::vector<std::pair<MapKey, CUtensorMap>> maps;  // LRU cache, most recently used last (a 24-layer stack holds 72 q/k/v keys)
-  // per-head list totals of the lists saf3r_select last wrote into a given row_ptr buffer (scheduling hint only)
-  struct LenHint { const int64_t *row_ptr; int32_t H, NB; int64_t len[SAF3R_MAX_HEADS]; };
-  std::vector<LenHint> hints;
   struct SizeMemo { int32_t H, S, T, B; saf3r_head_cfg cfg[SAF3R_MAX_HEADS]; int64_t len[SAF3R_MAX_HEADS]; int64_t total; };
   std::vector<SizeMemo> sizes;
 };
@@ -208,7 +206,7 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(select_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(token_sim_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSimSmem);
   if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->counter_dev, sizeof(unsigned long long));
-  if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->kmax_ring, sizeof(float) * kKmaxSlots * SAF3R_MAX_HEADS);
+  if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->kmax_ring, sizeof(float) * kKmaxSlots * kKmaxSlotFloats);
   if (e != cudaSuccess) {
     fprintf(stderr, "saf3r_create: cudaFuncSetAttribute / cudaMalloc failed: %s\n", cudaGetErrorString(e));
     delete ctx;
@@ -306,7 +304,7 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
   if (!q || !k || !ws || !lists || !lists->row_ptr || !lists->col_idx) return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
   if (((uintptr_t)q | (uintptr_t)k) & 15) return fail(ctx, SAF3R_ERR_INVALID_ARG, "q/k must be 16-byte aligned");
   const WsLayout w = ws_layout(g);
-  saf3r_ctx::LenHint hint;
+  struct { int64_t len[SAF3R_MAX_HEADS]; } hint;  // per-head list totals (closed forms)
   memset(&hint, 0, sizeof hint);
   // list sizes are a closed form of (shape, cfg); the per-row-length STATIC rules cost O(NB) .. O(NB*S) host work, so the last
   // few (shape, cfg) -> sizes results are memoised
@@ -418,14 +416,6 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
     ctx->ev_valid = true;
   }
   CU_CHECK(cudaGetLastError());
-  hint.row_ptr = lists->row_ptr; hint.H = g.H; hint.NB = g.NB;
-  bool found = false;
-  for (auto &hh : ctx->hints)
-    if (hh.row_ptr == hint.row_ptr) { hh = hint; found = true; }
-  if (!found) {
-    if (ctx->hints.size() >= 32) ctx->hints.erase(ctx->hints.begin());
-    ctx->hints.push_back(hint);
-  }
   return SAF3R_OK;
 }
 
@@ -519,31 +509,20 @@ static saf3r_status attn_common(saf3r_ctx *ctx, const void *q, const void *k, co
   p.N_kv = (int32_t)gk.N; p.NB_kv = gk.NB;
   p.out_fp32 = out_is_fp32 ? 1 : 0;
   p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)shape->head_dim));
-  // heads with the longest lists first (list lengths are per-head nearly uniform; dense mode: identity)
-  {
-    const int64_t *head_len = nullptr;
-    if (lists)
-      for (auto &hh : ctx->hints)
-        if (hh.row_ptr == lists->row_ptr && hh.H == g.H && hh.NB == g.NB) head_len = hh.len;
-    int64_t len[SAF3R_MAX_HEADS];
-    for (int h = 0; h < g.H; ++h) len[h] = head_len ? head_len[h] : 0;
-    for (int h = 0; h < g.H; ++h) p.head_order[h] = (uint8_t)h;
-    for (int a = 1; a < g.H; ++a)  // insertion sort, descending, stable
-      for (int b = a; b > 0 && len[p.head_order[b - 1]] < len[p.head_order[b]]; --b) {
-        uint8_t t = p.head_order[b]; p.head_order[b] = p.head_order[b - 1]; p.head_order[b - 1] = t;
-      }
-  }
   cudaStream_t st = (cudaStream_t)stream_;
   // max key norm per head (one streaming pass over K) for the kernel's frozen-max fast path; worth it from a few k-tiles per
   // q-block on (the pass reads K once, the attention reads it NB times through L2)
+  // The same launch orders the heads by list length, longest first (one CTA reads row_ptr; hand-made lists are balanced too).
   p.kmax = nullptr;
+  p.head_order = nullptr;
   if (gk.NB >= 4) {
-    float *slot = ctx->kmax_ring + (size_t)(ctx->kmax_next++ % kKmaxSlots) * SAF3R_MAX_HEADS;
+    float *slot = ctx->kmax_ring + (size_t)(ctx->kmax_next++ % kKmaxSlots) * kKmaxSlotFloats;
     CU_CHECK(cudaMemsetAsync(slot, 0, sizeof(float) * g.H, st));
-    knorm_kernel<<<dim3((unsigned)((gk.N + kKnormRows - 1) / kKnormRows), g.H), 256, 0, st>>>((const __nv_bfloat16 *)k, gk.N, gk.stride_head,
-                                                                                             gk.stride_token, slot);
+    knorm_kernel<<<dim3((unsigned)((gk.N + kKnormRows - 1) / kKnormRows), g.H), 256, 0, st>>>(
+        (const __nv_bfloat16 *)k, gk.N, gk.stride_head, gk.stride_token, slot, p.row_ptr, g.NB, reinterpret_cast<uint8_t *>(slot + SAF3R_MAX_HEADS));
     ctx->launches += 1;
     p.kmax = slot;
+    p.head_order = reinterpret_cast<const uint8_t *>(slot + SAF3R_MAX_HEADS);
   }
   dim3 grid(g.NB, g.H);
   p.tile_ptr = nullptr; p.key_idx = nullptr; p.mask = nullptr; p.k_base = p.v_base = nullptr; p.kv_stride_head = p.kv_stride_token = 0;
@@ -861,14 +840,15 @@ saf3r_status saf3r_token_lists_attn(saf3r_ctx *ctx, const void *q, const void *k
   p.N = (int32_t)g.N; p.NB = g.NB; p.H = g.H; p.N_kv = (int32_t)g.N; p.NB_kv = g.NB;
   p.out_fp32 = out_is_fp32 ? 1 : 0;
   p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)shape->head_dim));
-  for (int h = 0; h < g.H; ++h) p.head_order[h] = (uint8_t)h;
+  p.head_order = nullptr;
   p.tile_ptr = lists->tile_ptr; p.key_idx = lists->key_idx; p.mask = lists->mask;
   p.k_base = (const __nv_bfloat16 *)k; p.v_base = (const __nv_bfloat16 *)v;
   p.kv_stride_head = g.stride_head; p.kv_stride_token = g.stride_token;
   cudaStream_t st = (cudaStream_t)stream_;
-  float *slot = ctx->kmax_ring + (size_t)(ctx->kmax_next++ % kKmaxSlots) * SAF3R_MAX_HEADS;
+  float *slot = ctx->kmax_ring + (size_t)(ctx->kmax_next++ % kKmaxSlots) * kKmaxSlotFloats;
   CU_CHECK(cudaMemsetAsync(slot, 0, sizeof(float) * g.H, st));
-  knorm_kernel<<<dim3((unsigned)((g.N + kKnormRows - 1) / kKnormRows), g.H), 256, 0, st>>>((const __nv_bfloat16 *)k, g.N, g.stride_head, g.stride_token, slot);
+  knorm_kernel<<<dim3((unsigned)((g.N + kKnormRows - 1) / kKnormRows), g.H), 256, 0, st>>>((const __nv_bfloat16 *)k, g.N, g.stride_head, g.stride_token, slot,
+                                                                                          nullptr, g.NB, reinterpret_cast<uint8_t *>(slot + SAF3R_MAX_HEADS));
   p.kmax = slot;
   dim3 grid(g.NB, g.H);
   if (g.B == 128)
