@@ -139,7 +139,7 @@ static const char *validate_cfg(const SelGeom &g, const saf3r_head_cfg *cfg, int
 }
 
 struct WsLayout {
-  size_t qt, kt, qpart, probe, counters, total;
+  size_t qt, kt, qpart, probe, pkeys, counters, total;
 };
 static WsLayout ws_layout(const SelGeom &g) {
   WsLayout w;
@@ -148,6 +148,7 @@ static WsLayout ws_layout(const SelGeom &g) {
   w.kt = off; off = align256(off + (size_t)g.H * kt_stride(g.NB) * 64 * sizeof(float));
   w.qpart = off; off = align256(off + (size_t)g.H * ((g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask) * 64 * sizeof(float));
   w.probe = off; off = align256(off + (size_t)g.H * g.NB * sizeof(int32_t));
+  w.pkeys = off; off = align256(off + (size_t)g.H * g.NB * sizeof(uint32_t));  // probe rows as keys
   w.counters = off; off = align256(off + kSelCounters * sizeof(int));  // ticket counters and per-head flags of the fused kernel
   w.total = off;
   return w;
@@ -283,8 +284,9 @@ static SelPlan select_plan(const SelGeom &g, int n_block, int n_probe, int sm_co
     p.smem = (size_t)p.R * row + qbytes;
   }
   if (n_probe > 0) {
-    if (row + kSelScratch > 220 * 1024) { p.unsupported = "NB too large for the probe stage"; return p; }
-    if (p.smem < row + kSelScratch) p.smem = row + kSelScratch;
+    if (row > 220 * 1024) { p.unsupported = "NB too large for the probe stage"; return p; }
+    if (p.smem < row) p.smem = row;
+    if (p.smem < (size_t)kSelScratch) p.smem = kSelScratch;
   }
   if (p.smem < 4096) p.smem = 4096;  // scratch of the pool / row_ptr tasks
   return p;
@@ -385,19 +387,21 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
   fp.n_pool_a = 2 * sets.n_block * tasks_per_job;   // jobs are ordered BLOCK_TOPK heads first (see above)
   fp.n_pool_b = 2 * sets.n_probe * tasks_per_job;
   fp.n_x = sets.n_block * fp.strips;                // score strips: mixed into the pooling of the QUERY_PROBE heads
-  fp.n_probe = sets.n_probe;                        // everything below follows ALL pool tasks
+  fp.pchunks = (g.NB + kProbeChunk - 1) / kProbeChunk;
+  fp.n_pscore = sets.n_probe * fp.pchunks;          // everything from here on follows ALL pool tasks
+  fp.n_probe = sets.n_probe;
   fp.n_light = (sets.n_light + sets.n_cached) * light_chunks;
   fp.n_emit = sets.n_emit * light_chunks;
   fp.n_rep = sets.n_probe * light_chunks;
   fp.period = fp.n_x > 0 && fp.n_pool_b / fp.n_x > 1 ? fp.n_pool_b / fp.n_x : 1;
-  const int n_tasks = fp.n_rowptr + fp.n_pool_a + fp.n_pool_b + fp.n_x + fp.n_probe + fp.n_light + fp.n_emit + fp.n_rep;
+  const int n_tasks = fp.n_rowptr + fp.n_pool_a + fp.n_pool_b + fp.n_x + fp.n_pscore + fp.n_probe + fp.n_light + fp.n_emit + fp.n_rep;
   int *counters = (int *)(wsb + w.counters);
   CU_CHECK(cudaMemsetAsync(counters, 0, kSelCounters * sizeof(int), st));
   auto launch = [&](int t_begin, int t_end, int counter) {
     fp.t_begin = t_begin; fp.t_end = t_end; fp.counter = counter;
     const int ctas = t_end - t_begin < 2 * ctx->sm_count ? t_end - t_begin : 2 * ctx->sm_count;
     if (ctas <= 0) return;
-    select_fused_kernel<<<ctas, 256, sp.smem, st>>>((const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart, probe, lists->row_ptr,
+    select_fused_kernel<<<ctas, 256, sp.smem, st>>>((const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart, (uint32_t *)(wsb + w.pkeys), probe, lists->row_ptr,
                                                    lists->col_idx, (const int64_t *)(cache ? cache->row_ptr : nullptr),
                                                    (const int32_t *)(cache ? cache->col_idx : nullptr), counters, g, jobs, plan, ca, sets, fp);
     ctx->launches += 1;

@@ -337,6 +337,7 @@ struct HeadSets {
 //   remaining CTAs          : the lists of the closed-form heads whose rows all have the same length (DENSE, UNIFORM_STRIDE,
 //                            STATIC/ANCHOR): 32 rows per CTA, written under the pooling's HBM time.
 constexpr int kPoolBlocksPerTask = 8;  // one block per warp
+constexpr int kPoolLoads = 16;         // independent 16-byte loads in flight per lane (64 token rows per round; 8 measured the same)
 struct PoolJobs {
   int32_t n;                            // number of (tensor, head) jobs
   uint8_t head[2 * SAF3R_MAX_HEADS];
@@ -355,10 +356,14 @@ __device__ __forceinline__ uint4 ld_stream_16(const void *p) {
   return r;
 }
 
-// Probe of one QUERY_PROBE head, run by a whole CTA (256 threads): qbar = (1/N) sum_t q_t from the
-// per-CTA token sums of the pool launch, p[J] = qbar . Ktilde_J / sqrt(D), top-n -> probe_list[h][0..n).
-__device__ inline void probe_head(const float *qpart, const float *kt, int32_t *probe_list, const SelGeom &g, int h, int n,
-                                  uint32_t *key /* dynamic smem, NB */, float (*part)[64], float *qb) {
+// Probe of a QUERY_PROBE head (qbar = (1/N) sum_t q_t, p[J] = qbar . Ktilde_J / sqrt(D)), as small tasks so that what
+// is left to do after the head's last pool task is short and parallel:
+//   probe_score_task  kProbeChunk k-blocks: qbar from the per-task token sums of the pool tasks (fixed order), the two halves of d by
+//                     the two halves of the CTA (every load independent), keys -> probe_keys[h][J]
+//   probe_topn_task   the head's NB keys -> shared memory, one warp runs the top-n -> probe_list[h][0..n)
+constexpr int kProbeChunk = 128;
+__device__ inline void probe_score_task(const float *qpart, const float *kt, uint32_t *probe_keys, const SelGeom &g, int h, int chunk,
+                                        float (*part)[64], float *qb, float *ph /* [2][kProbeChunk] */) {
   const int nparts = (g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask;
   {
     // 16 groups of 16 threads; a thread owns four dimensions and every 16th partial sum (independent 16-byte loads, eight in flight);
@@ -384,19 +389,27 @@ __device__ inline void probe_head(const float *qpart, const float *kt, int32_t *
     __syncthreads();
   }
   const int64_t ld = kt_stride(g.NB);
-  for (int J = threadIdx.x; J < g.NB; J += 256) {
-    const float *kc = kt + (int64_t)h * 64 * ld + J;
-    float acc = 0.f;
+  const int col = threadIdx.x & (kProbeChunk - 1), half = threadIdx.x / kProbeChunk;
+  const int J = chunk * kProbeChunk + col;
+  float acc = 0.f;
+  if (J < g.NB) {
+    const float *kc = kt + ((int64_t)h * 64 + 32 * half) * ld + J;
 #pragma unroll
-    for (int d0 = 0; d0 < 64; d0 += 16) {
+    for (int d0 = 0; d0 < 32; d0 += 16) {
       float t[16];
 #pragma unroll
       for (int i = 0; i < 16; ++i) t[i] = __ldcg(kc + (int64_t)(d0 + i) * ld);
 #pragma unroll
-      for (int i = 0; i < 16; ++i) acc = fmaf(qb[d0 + i], t[i], acc);
+      for (int i = 0; i < 16; ++i) acc = fmaf(qb[32 * half + d0 + i], t[i], acc);
     }
-    key[J] = score_key(acc * 0.125f);
   }
+  ph[half * kProbeChunk + col] = acc;
+  __syncthreads();
+  if (half == 0 && J < g.NB) probe_keys[(int64_t)h * g.NB + J] = score_key((ph[col] + ph[kProbeChunk + col]) * 0.125f);
+}
+__device__ inline void probe_topn_task(const uint32_t *probe_keys, int32_t *probe_list, const SelGeom &g, int h, int n,
+                                       uint32_t *key /* dynamic smem, NB */) {
+  for (int J = threadIdx.x; J < g.NB; J += 256) key[J] = __ldcg(probe_keys + (int64_t)h * g.NB + J);
   __syncthreads();
   if (threadIdx.x < 32) warp_topn_bisect(key, g.NB, n, probe_list + (int64_t)h * g.NB);
 }
@@ -431,8 +444,8 @@ __device__ inline void rowptr_task(int64_t *__restrict__ row_ptr, const SelGeom 
 }
 
 // One pool task (whole CTA): eight consecutive token blocks of one (tensor, head) job, ONE WARP PER BLOCK and no shared memory on
-// the way: a lane owns a 16-byte chunk (l & 7) of rows (l >> 3) + 4 i, eight independent 16-byte loads in flight per lane and
-// round of 32 rows, fp32 accumulate, optional per-token L2 normalisation (cosine), fold of the four row groups with shuffles,
+// the way: a lane owns a 16-byte chunk (l & 7) of rows (l >> 3) + 4 i, kPoolLoads independent 16-byte loads in flight per lane and
+// round of 4 * kPoolLoads rows, fp32 accumulate, optional per-token L2 normalisation (cosine), fold of the four row groups with shuffles,
 // mean -> Qtilde (row-major) or Ktilde^T (transposed).  The Q job of a QUERY_PROBE head also leaves each warp's token sum in
 // wsum for the task's partial sum of qbar, written by the caller after its barrier.
 __device__ __forceinline__ void pool_task(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k, float *__restrict__ qt,
@@ -450,16 +463,16 @@ __device__ __forceinline__ void pool_task(const __nv_bfloat16 *__restrict__ q, c
     const int cnt = (int)i64min(g.B, g.N - t0);
     const __nv_bfloat16 *src = (which ? k : q) + (int64_t)h * g.stride_head + t0 * g.stride_token + sub * 8;
 #pragma unroll 1
-    for (int r0 = 0; r0 < cnt; r0 += 32) {
-      uint4 raw[8];
+    for (int r0 = 0; r0 < cnt; r0 += 4 * kPoolLoads) {
+      uint4 raw[kPoolLoads];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
+      for (int i = 0; i < kPoolLoads; ++i) {
         const int r = r0 + rg + 4 * i;
         raw[i] = make_uint4(0, 0, 0, 0);
         if (r < cnt) raw[i] = ld_stream_16(src + (int64_t)r * g.stride_token);
       }
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
+      for (int i = 0; i < kPoolLoads; ++i) {
         const uint32_t w[4] = {raw[i].x, raw[i].y, raw[i].z, raw[i].w};
         float v[8];
 #pragma unroll
@@ -632,9 +645,10 @@ __device__ __forceinline__ void score_rows(const float *__restrict__ qt, const f
 // ONE persistent launch for the whole of saf3r_select.  CTAs (256 threads, <= 2 per SM) draw tickets from a device counter; the
 // ticket order is a host-side closed form of (shape, cfg):
 //   [row_ptr task per head] [pool tasks of the BLOCK_TOPK heads] [MIX: pool tasks of the QUERY_PROBE heads with one score strip
-//   after every `period` of them] [what is left of either] [probe tasks] [light chunks] [emit chunks] [probe-list copies]
-// score strip: R q-block rows of a BLOCK_TOPK head (scores in shared memory, top-n / per-frame top-k); probe task: one per
-// QUERY_PROBE head (qbar, probe row, top-n -> the head's list); light chunk: 32 rows of a per-row STATIC rule or of a CACHED head;
+//   after every `period` of them] [what is left of either] [probe-score chunks] [probe top-n tasks] [light chunks] [emit chunks]
+//   [probe-list copies]
+// score strip: R q-block rows of a BLOCK_TOPK head (scores in shared memory, top-n / per-frame top-k); probe-score chunk: qbar and
+// 128 entries of the probe row of a QUERY_PROBE head; probe top-n: one per QUERY_PROBE head (the row's top-n -> the head's list); light chunk: 32 rows of a per-row STATIC rule or of a CACHED head;
 // emit chunk: 32 rows of a constant-length closed-form list; copy chunk: 32 of the NB identical rows of a QUERY_PROBE head.  So the score + select work of the BLOCK_TOPK heads and every list
 // write run UNDER the HBM stream of the remaining pooling instead of after it, and nothing is launched twice.
 // A task that needs the pooled tensors of head h spins (one thread, ld.acquire) on pooled[h]; every pool task ends with a
@@ -644,13 +658,14 @@ struct FusedPlan {
   int32_t t_begin, t_end;                 // tickets this launch serves (two launches when the stages are timed separately)
   int32_t n_rowptr, n_pool_a, n_pool_b;   // tasks per segment
   int32_t n_x, period;                    // score strips (mixed into the pool-B tasks, one after every `period` of them, >= 1)
-  int32_t n_probe, n_light, n_emit, n_rep;  // after ALL pool tasks: probe tasks, light chunks, emit chunks, probe-list copies
+  int32_t n_pscore, n_probe, n_light, n_emit, n_rep;  // after ALL pool tasks: probe-score chunks, probe top-n, light, emit, list copies
+  int32_t pchunks;                        // probe-score chunks per QUERY_PROBE head
   int32_t strips, R, light_chunks;
   int32_t pool_need;                      // pool tasks per head = 2 jobs * tasks_per_job
   int32_t counter;                        // which ticket counter (0 / 1)
 };
-constexpr int kSelScratch = 17 * 64 * 4;  // bytes of task scratch besides the keys of a probe task (partial sums of qbar, qbar)
-constexpr int kSelCounters = 2 + 3 * SAF3R_MAX_HEADS;  // int32: 2 ticket counters, pooled[h], rowptr_done[h], probe_done[h]
+constexpr int kSelScratch = 17 * 64 * 4 + 2 * kProbeChunk * 4;  // bytes of scratch of a probe-score task (partial sums of qbar, qbar, half sums)
+constexpr int kSelCounters = 2 + 4 * SAF3R_MAX_HEADS;  // int32: 2 ticket counters, pooled[h], rowptr_done[h], probe_done[h], pscore_done[h]
 
 __device__ __forceinline__ void wait_count(const int *ctr, int need) {
   if (threadIdx.x == 0) {
@@ -669,7 +684,7 @@ __device__ __forceinline__ void signal_count(int *ctr) {
 
 __global__ void __launch_bounds__(256, 2) select_fused_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
                                                               float *__restrict__ qt, float *__restrict__ kt, float *__restrict__ qpart,
-                                                              int32_t *__restrict__ probe_list, int64_t *__restrict__ row_ptr,
+                                                              uint32_t *__restrict__ probe_keys, int32_t *__restrict__ probe_list, int64_t *__restrict__ row_ptr,
                                                               int32_t *__restrict__ col_idx, const int64_t *__restrict__ cache_row_ptr,
                                                               const int32_t *__restrict__ cache_col_idx, int *__restrict__ counters,
                                                               SelGeom g, PoolJobs jobs, RowPtrPlan plan, HeadCfgArray cfg, HeadSets sets,
@@ -678,7 +693,8 @@ __global__ void __launch_bounds__(256, 2) select_fused_kernel(const __nv_bfloat1
   float(*wsum)[64] = reinterpret_cast<float(*)[64]>(sm);      // pool task: [8][64]
   int64_t *sums = reinterpret_cast<int64_t *>(sm);             // row_ptr task: [256]
   __shared__ int s_ticket;
-  int *pooled = counters + 2, *rp_done = counters + 2 + SAF3R_MAX_HEADS, *probe_done = counters + 2 + 2 * SAF3R_MAX_HEADS;
+  int *pooled = counters + 2, *rp_done = counters + 2 + SAF3R_MAX_HEADS, *probe_done = counters + 2 + 2 * SAF3R_MAX_HEADS,
+      *pscore_done = counters + 2 + 3 * SAF3R_MAX_HEADS;
   const int warp = threadIdx.x >> 5;
   // thread 0 always holds the NEXT ticket: its atomic is issued a whole task ahead, so its latency never shows
   int next = 0;
@@ -756,12 +772,19 @@ __global__ void __launch_bounds__(256, 2) select_fused_kernel(const __nv_bfloat1
       continue;
     }
     x -= fp.n_x;
+    if (x < fp.n_pscore) {
+      const int h = sets.probe[x / fp.pchunks];
+      wait_count(pooled + h, fp.pool_need);
+      float(*part)[64] = reinterpret_cast<float(*)[64]>(sm);  // [16][64], then qbar [64], then the half sums [2][kProbeChunk]
+      probe_score_task(qpart, kt, probe_keys, g, h, x % fp.pchunks, part, sm + 16 * 64, sm + 17 * 64);
+      signal_count(pscore_done + h);
+      continue;
+    }
+    x -= fp.n_pscore;
     if (x < fp.n_probe) {
       const int h = sets.probe[x];
-      wait_count(pooled + h, fp.pool_need);
-      float(*part)[64] = reinterpret_cast<float(*)[64]>(sm + kt_stride(g.NB));  // behind the NB probe keys: [16][64], then qbar [64]
-      probe_head(qpart, kt, probe_list, g, h, (int)i64min(cfg.c[h].keep_blocks, g.NB), reinterpret_cast<uint32_t *>(sm), part,
-                 sm + kt_stride(g.NB) + 16 * 64);
+      wait_count(pscore_done + h, fp.pchunks);
+      probe_topn_task(probe_keys, probe_list, g, h, (int)i64min(cfg.c[h].keep_blocks, g.NB), reinterpret_cast<uint32_t *>(sm));
       signal_count(probe_done + h);
       continue;
     }
