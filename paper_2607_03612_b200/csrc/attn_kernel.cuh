@@ -50,52 +50,60 @@ constexpr int kD = 64;  // head_dim (bf16: one 128-byte swizzle row)
 constexpr int kAttnThreads = 384;
 constexpr int kKStages = 3, kVStages = 2;
 constexpr int kTmemCols = 256;
-constexpr int kTmemO = 128;  // first O column
-constexpr int kTmemP = 192;  // first P column
+constexpr int kTmemO = 128;  // first O column (64 fp32 columns)
+constexpr int kTmemL = 192;  // row sums of P: 16 identical fp32 columns written by the ones-MMA (column 0 is read)
+constexpr int kTmemP = 208;  // P of ONE 64-key half of the tile, packed bf16 (32 columns)
 constexpr float kLazyLog2 = 8.f;
 constexpr int kSleepTma = 128, kSleepMma = 48;  // ns between two mbarrier polls of the producer / issuer warps
 constexpr float kFreezeLog2 = 64.f;  // freeze the reference max when no logit can exceed it by more than 2^64
-constexpr int kSplit128 = 80;  // columns of a 128-wide tile whose exponentials use the MUFU (rest: FMA-pipe polynomial); any multiple of 8
+constexpr int kSplitHalf128 = 40;  // columns of every 64-key half whose exponentials use the MUFU (rest: FMA-pipe polynomial); multiple of 8
 constexpr int kRegsMufu = 112, kRegsFma = 88, kRegsIdle = 40;  // 128*(112+88+40) = 30720 = 384 threads * 80 registers
 
 template <int B>
 struct AttnSmem {
-  static constexpr int kSplit = (B == 128) ? kSplit128 : 32;  // columns whose exponentials use the MUFU (rest: FMA-pipe polynomial)
+  static constexpr int kSplitHalf = (B == 128) ? kSplitHalf128 : 32;
   static constexpr int kQ = 0;                          // 128 x 64 bf16 (only the first B rows are loaded)
   static constexpr int kK = kQ + 128 * 128;             // kKStages x (B x 64 bf16)
   static constexpr int kV = kK + kKStages * B * 128;    // kVStages x (B x 64 bf16)
-  static constexpr int kMax = kV + kVStages * B * 128;  // float [2 parity][2 half][128 rows]
-  static constexpr int kSum = kMax + 2 * 2 * 128 * 4;   // float [2 half][128 rows]
-  static constexpr int kBar = kSum + 2 * 128 * 4;
-  static constexpr int kTotal = kBar + 128;
+  static constexpr int kOnes = kV + kVStages * B * 128; // 16 x 64 bf16 ones (K-major B operand of the row-sum MMA; 1024-byte aligned)
+  static constexpr int kMax = kOnes + 2048;             // float [2 parity][2 half][128 rows]
+  static constexpr int kBar = kMax + 2 * 2 * 128 * 4;
+  static constexpr int kTotal = kBar + 256;
 };
 
-// one softmax half: rows = TMEM lanes of this warp, columns [C0, C1) of the B-wide tile
-template <int B, int C0, int C1, bool kFma, bool kTok>
+// one softmax group: rows = TMEM lanes of this warp; of every 64-key half of the B-wide tile it owns the columns
+// [C0h, C0h + NCH): the MUFU group the first kSplitHalf, the FMA group the rest.  P goes to TMEM one 64-key half at a time (the
+// 32-column P buffer is handed back by the PV MMAs of the previous half), and the row sum of the bf16-ROUNDED weights is an MMA of
+// its own (P x ones, N = 16) into kTmemL: no per-element add in these warps, and the sum matches what the PV product multiplies.
+template <int B, bool kFma, bool kTok>
 __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem, uint32_t tmem, int n_ent, int64_t e0, int h,
                                              int I, uint32_t bar_q, uint32_t bar_s_full, uint32_t bar_s_free,
-                                             uint32_t bar_p_full, uint32_t bar_o_done) {
+                                             uint32_t bar_p_full /* [NH] */, uint32_t bar_pv0_done, uint32_t bar_o_done) {
   using L = AttnSmem<B>;
-  constexpr int NC = C1 - C0;
-  static_assert(NC % 8 == 0 && C0 % 8 == 0, "column split must be a multiple of 8");
+  constexpr int NH = B / 64;                       // 64-key halves of a tile
+  constexpr int kS = L::kSplitHalf;
+  constexpr int C0h = kFma ? kS : 0;               // first column of this group inside a half
+  constexpr int NCH = kFma ? 64 - kS : kS;         // columns of this group per half
+  constexpr int NC = NCH * NH;
+  static_assert(NCH % 8 == 0 && NCH > 0 && NCH < 64, "column split must be a multiple of 8");
   constexpr int kHalf = kFma ? 1 : 0;
   const int r = threadIdx.x & 127;
   const int pair_bar = 1 + (r >> 5);  // named barrier shared by the two warps that own these 32 rows
   // TMEM lane block of this warp; the shuffle makes it warp-uniform by construction so that ptxas keeps the tcgen05.ld/st
   // addresses in uniform registers instead of re-deriving them (R2UR) every iteration
   const uint32_t lane_off = (uint32_t)(__shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0) & 3) << 21;
-  const uint32_t tS = tmem + lane_off + C0, tO = tmem + lane_off + kTmemO + 32 * kHalf, tP = tmem + lane_off + kTmemP + C0 / 2;
+  const uint32_t tS = tmem + lane_off + C0h, tO = tmem + lane_off + kTmemO + 32 * kHalf, tP = tmem + lane_off + kTmemP + C0h / 2;
+  const uint32_t tL = tmem + lane_off + kTmemL;
   float *smax = reinterpret_cast<float *>(smem + L::kMax);
-  float *ssum = reinterpret_cast<float *>(smem + L::kSum);
   const int tail = p.N_kv - (p.NB_kv - 1) * B;  // valid keys in the last k-block
   const int64_t tok = (int64_t)I * B + r;
   const bool row_valid = (r < B) && (tok < p.N);
   const float c = p.scale_log2;
   const float lazy_raw = kLazyLog2 / c;
-  float m = -INFINITY, l = 0.f;
+  float m = -INFINITY;
   const int J_last = (n_ent > 0 && !kTok) ? (p.row_ptr ? p.col_idx[e0 + n_ent - 1] : p.NB_kv - 1) : -1;
   const bool last_is_tail = !kTok && (J_last == p.NB_kv - 1) && (tail < B);
-  // Cauchy-Schwarz bound of this row's logits (in the units of m: raw scores), from the Q tile in shared memory.  Both halves
+  // Cauchy-Schwarz bound of this row's logits (in the units of m: raw scores), from the Q tile in shared memory.  Both groups
   // of a row read the same eight 16-byte chunks in the same (physical) order, so they get the same bits and take the same
   // freeze decision without talking to each other.
   float bound = INFINITY;
@@ -120,34 +128,34 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
   const float freeze_raw = kFreezeLog2 / c;
 
   for (int e = 0; e < n_ent; ++e) {
-    uint32_t v[NC];
+    uint32_t v[NC];  // v[hh * NCH + i] = score of column 64 hh + C0h + i
     mbar_wait(bar_s_full, e & 1);
     tc_fence_after();
 #pragma unroll
-    for (int cb = 0; cb + 16 <= NC; cb += 16) tmem_ld16(tS + cb, *reinterpret_cast<uint32_t(*)[16]>(&v[cb]));
-    if (NC % 16) tmem_ld8(tS + NC - 8, *reinterpret_cast<uint32_t(*)[8]>(&v[NC - 8]));
+    for (int hh = 0; hh < NH; ++hh) tmem_ld_n<NCH>(tS + 64 * hh, &v[hh * NCH]);
     tmem_ld_wait();
     tc_fence_before();
     mbar_arrive(bar_s_free);
     if (e == n_ent - 1 && last_is_tail) {
 #pragma unroll
       for (int i = 0; i < NC; ++i)
-        if (C0 + i >= tail) v[i] = 0xff800000u;  // -inf
+        if ((i / NCH) * 64 + C0h + (i % NCH) >= tail) v[i] = 0xff800000u;  // -inf
     }
     if (kTok) {  // per-(query, key) mask of this tile: keys the query did not select get -inf before the max
-      constexpr int W0 = C0 / 32, W1 = (C1 + 31) / 32;
-      uint32_t mw[W1 - W0];
+      uint32_t mw[B / 32];
       const uint32_t *mrow = p.mask + ((e0 + e) * B + (r < B ? r : 0)) * (B / 32);
 #pragma unroll
-      for (int w = W0; w < W1; ++w) mw[w - W0] = r < B ? __ldg(mrow + w) : 0u;
+      for (int w = 0; w < B / 32; ++w) mw[w] = r < B ? __ldg(mrow + w) : 0u;
 #pragma unroll
-      for (int i = 0; i < NC; ++i)
-        if (!((mw[(C0 + i) / 32 - W0] >> ((C0 + i) & 31)) & 1u)) v[i] = 0xff800000u;
+      for (int i = 0; i < NC; ++i) {
+        const int col = (i / NCH) * 64 + C0h + (i % NCH);
+        if (!((mw[col / 32] >> (col & 31)) & 1u)) v[i] = 0xff800000u;
+      }
     }
     float alpha = 1.f;
     bool moved = false;
     if (!frozen) {
-      // partial row max over this half's columns, then exchange with the other half
+      // partial row max over this group's columns, then exchange with the other group
       float mx0 = __uint_as_float(v[0]), mx1 = __uint_as_float(v[1]), mx2 = __uint_as_float(v[2]), mx3 = __uint_as_float(v[3]);
 #pragma unroll
       for (int i = 4; i < NC; i += 8) {
@@ -163,7 +171,7 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
       slot[kHalf * 128 + r] = mx;
       named_bar_sync(pair_bar, 64);
       mx = fmaxf(mx, slot[(1 - kHalf) * 128 + r]);
-      // lazy running max (identical decision in both halves: same rows, same combined max)
+      // lazy running max (identical decision in both groups: same rows, same combined max)
       moved = __any_sync(0xffffffffu, mx > m + lazy_raw);
       if (moved) {
         const float m_new = fmaxf(m, mx);
@@ -176,14 +184,18 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
       if (kFma && frozen) noclamp = __all_sync(0xffffffffu, (bound + fabsf(m)) * c < 120.f);
     }
     const float nmc = (kTok && m == -INFINITY) ? 0.f : -m * c;  // a row without a kept key so far: every x stays -inf, p = 0
-    uint32_t pk[NC / 2];
-    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;  // row sum of the bf16-ROUNDED weights (what the PV product multiplies)
     const uint64_t c2 = pack_f32x2(c, c), nmc2 = pack_f32x2(nmc, nmc);
-    auto exp_tile = [&](auto clamp_tag) {
+    // the polynomial group needs its argument clamped at -126 unless every x of the tile is known to be above it: frozen max,
+    // |logit| <= bound for all 32 rows (Cauchy-Schwarz again: x >= -(bound + m) c), no masked (-inf) column in the tile
+    const bool fast = kFma && !kTok && noclamp && !(e == n_ent - 1 && last_is_tail);
+    uint32_t pk[NCH / 2];
+    auto exp_half = [&](auto clamp_tag, auto hh_tag) {
       constexpr bool kClamp = decltype(clamp_tag)::value;
+      constexpr int hh = decltype(hh_tag)::value;
 #pragma unroll
-      for (int j = 0; j < NC / 2; ++j) {
-        const uint64_t x2 = fma_f32x2(pack_f32x2(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1])), c2, nmc2);
+      for (int j = 0; j < NCH / 2; ++j) {
+        const uint64_t x2 =
+            fma_f32x2(pack_f32x2(__uint_as_float(v[hh * NCH + 2 * j]), __uint_as_float(v[hh * NCH + 2 * j + 1])), c2, nmc2);
         float p0, p1;
         if (kFma) {
           exp2_emu_f32x2<kClamp>(x2, p0, p1);
@@ -193,55 +205,61 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
           p1 = ex2_approx(p1);
         }
         pk[j] = pack_bf16x2(p0, p1);
-        if (j & 1) add_bf16x2_to_f32(pk[j], s2, s3);
-        else add_bf16x2_to_f32(pk[j], s0, s1);
       }
     };
-    // the polynomial half needs its argument clamped at -126 unless every x of the tile is known to be above it: frozen max,
-    // |logit| <= bound for all 32 rows (Cauchy-Schwarz again: x >= -(bound + m) c), no masked (-inf) column in the tile
-    if (kFma && !kTok && noclamp && !(e == n_ent - 1 && last_is_tail)) exp_tile(std::false_type{});
-    else exp_tile(std::true_type{});
-    l = l * alpha + ((s0 + s1) + (s2 + s3));
-    // PV(e-1) must be complete before P is overwritten and O is rescaled
-    if (e > 0) {
-      mbar_wait(bar_o_done, (e - 1) & 1);
-      tc_fence_after();
-      if (moved) {  // this half rescales its 32 of the 64 O columns
-        uint32_t o[32];
-        tmem_ld32(tO, o);
-        tmem_ld_wait();
+    auto do_half = [&](auto hh_tag) {
+      constexpr int hh = decltype(hh_tag)::value;
+      if (fast) exp_half(std::false_type{}, hh_tag);
+      else exp_half(std::true_type{}, hh_tag);
+      if (hh == 0) {
+        // PV(e-1) must be complete before the P buffer is overwritten and O / the row sum are rescaled
+        if (e > 0) {
+          mbar_wait(bar_o_done, (e - 1) & 1);
+          tc_fence_after();
+          if (moved) {  // this group rescales its 32 of the 64 O columns (the MUFU group also the row sum)
+            uint32_t o[32];
+            uint32_t lsum = 0;
+            tmem_ld32(tO, o);
+            if (!kFma) tmem_ld1(tL, lsum);
+            tmem_ld_wait();
 #pragma unroll
-        for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-        tmem_st32(tO, o);
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+            tmem_st32(tO, o);
+            if (!kFma) tmem_st1(tL, __float_as_uint(__uint_as_float(lsum) * alpha));
+          }
+        }
+      } else {
+        mbar_wait(bar_pv0_done, e & 1);  // the MMAs of the first half have read the P buffer
+        tc_fence_after();
       }
-    }
-#pragma unroll
-    for (int cb = 0; cb + 8 <= NC / 2; cb += 8) tmem_st8(tP + cb, *reinterpret_cast<uint32_t(*)[8]>(&pk[cb]));
-    if ((NC / 2) % 8) tmem_st4(tP + NC / 2 - 4, *reinterpret_cast<uint32_t(*)[4]>(&pk[NC / 2 - 4]));
-    tmem_st_wait();
-    tc_fence_before();
-    mbar_arrive(bar_p_full);
+      tmem_st_n<NCH / 2>(tP, pk);
+      tmem_st_wait();
+      tc_fence_before();
+      mbar_arrive(bar_p_full + 8 * hh);
+    };
+    do_half(std::integral_constant<int, 0>{});
+    if constexpr (NH == 2) do_half(std::integral_constant<int, 1>{});
   }
 
   // ------------------------------------------------------------ epilogue: O / l -> global (32 of the 64 columns each)
-  ssum[kHalf * 128 + r] = l;
-  named_bar_sync(pair_bar, 64);
-  l += ssum[(1 - kHalf) * 128 + r];
   if (n_ent > 0) {
     mbar_wait(bar_o_done, (n_ent - 1) & 1);
     tc_fence_after();
   }
-  const float inv_l = (n_ent > 0) ? 1.f / l : 0.f;
   uint8_t *orow = reinterpret_cast<uint8_t *>(p.out) +
                   ((int64_t)h * p.out_stride_head + tok * p.out_stride_token + 32 * kHalf) * (p.out_fp32 ? 4 : 2);
   uint32_t o[32];
+  uint32_t lbits = 0;
   if (n_ent > 0) {
     tmem_ld32(tO, o);
+    tmem_ld1(tL, lbits);
     tmem_ld_wait();
   } else {
 #pragma unroll
     for (int i = 0; i < 32; ++i) o[i] = 0u;
   }
+  const float l = __uint_as_float(lbits);
+  const float inv_l = (n_ent > 0) ? 1.f / l : 0.f;
   if (row_valid) {
     if (p.out_fp32) {
       float4 *dst = reinterpret_cast<float4 *>(orow);
@@ -299,10 +317,12 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
   const uint32_t bar_v_empty = bar_v_full + 8 * kVStages;    // [kVStages]
   const uint32_t bar_s_full = bar_v_empty + 8 * kVStages;    // MMA -> softmax: S(e) is in TMEM
   const uint32_t bar_s_free = bar_s_full + 8;   // softmax -> MMA: S(e) has been read into registers (256 arrivals)
-  const uint32_t bar_p_full = bar_s_free + 8;   // softmax -> MMA: P(e) is in TMEM, O rescaled (256 arrivals)
-  const uint32_t bar_o_done = bar_p_full + 8;   // MMA -> softmax: PV(e) complete
-  static_assert(8 + 16 * (kKStages + kVStages) + 32 <= 120, "barrier area overflow");
-  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::kBar + 120);
+  const uint32_t bar_p_full = bar_s_free + 8;   // [2] softmax -> MMA: this 64-key half of P(e) is in TMEM, O rescaled (256 arrivals)
+  const uint32_t bar_pv0_done = bar_p_full + 16;  // MMA -> softmax: the MMAs of the first half of P(e) are complete (P buffer free)
+  const uint32_t bar_o_done = bar_pv0_done + 8;   // MMA -> softmax: PV(e) complete
+  static_assert(8 + 16 * (kKStages + kVStages) + 48 <= 240, "barrier area overflow");
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::kBar + 248);
+  constexpr int NH = B / 64;
 
   int64_t e0 = 0;
   int n_ent = p.NB_kv;
@@ -323,8 +343,15 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
     mbar_init(bar_s_full, 1);
     mbar_init(bar_s_free, 256);
     mbar_init(bar_p_full, 256);
+    mbar_init(bar_p_full + 8, 256);
+    mbar_init(bar_pv0_done, 1);
     mbar_init(bar_o_done, 1);
     fence_mbar_init();
+  }
+  // ones tile of the row-sum MMA: 16 rows x 64 bf16 of 1.0 (every 16-byte chunk is the same, so the 128-byte swizzle is a no-op)
+  if (threadIdx.x >= 256) {
+    reinterpret_cast<uint4 *>(smem + L::kOnes)[threadIdx.x - 256] = make_uint4(0x3f803f80u, 0x3f803f80u, 0x3f803f80u, 0x3f803f80u);
+    fence_proxy_async_smem();
   }
   if (warp == 9) {
     tmem_alloc(smem_u32(tmem_slot), kTmemCols);
@@ -413,6 +440,9 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
         mbar_wait_relaxed<kSleepMma>(bar_q, 0);
         issue_qk();
         int sv = 0, phv = 0;
+        constexpr uint32_t idesc_l = umma_idesc_bf16(16, false);
+        const uint64_t odesc = umma_desc_sw128(sbase + L::kOnes);
+        const uint32_t tL = tmem + kTmemL;
         for (int e = 0; e < n_ent; ++e) {
           if (e + 1 < n_ent) {
             mbar_wait_relaxed<kSleepMma>(bar_s_free, e & 1);  // S(e) is in registers -> overwrite it with S(e+1) while softmax(e) runs
@@ -420,27 +450,37 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
           }
           mbar_wait_relaxed<kSleepMma>(bar_v_full + 8 * sv, phv);
           if (kTok) fence_proxy_async_smem();
-          mbar_wait_relaxed<kSleepMma>(bar_p_full, e & 1);
-          tc_fence_after();
-          if (elect_one_sync()) {
-            const uint64_t vdesc = umma_desc_sw128(sbase + L::kV + sv * B * 128);
 #pragma unroll
-            for (int kk = 0; kk < B / 16; ++kk)
-              umma_ts(tO, tP + kk * 8, vdesc + (uint64_t)kk * 128, idesc_pv, (e > 0 || kk > 0) ? 1u : 0u);
-            umma_commit(bar_v_empty + 8 * sv);
-            umma_commit(bar_o_done);
+          for (int hh = 0; hh < NH; ++hh) {
+            mbar_wait_relaxed<kSleepMma>(bar_p_full + 8 * hh, e & 1);
+            tc_fence_after();
+            if (elect_one_sync()) {
+              const uint64_t vdesc = umma_desc_sw128(sbase + L::kV + sv * B * 128);
+#pragma unroll
+              for (int kk = 0; kk < 4; ++kk)   // O += P_half . V_half (K = 16 keys per MMA; P packed: 8 columns per step)
+                umma_ts(tO, tP + kk * 8, vdesc + (uint64_t)(hh * 4 + kk) * 128, idesc_pv, (e > 0 || hh > 0 || kk > 0) ? 1u : 0u);
+#pragma unroll
+              for (int kk = 0; kk < 4; ++kk)   // l += P_half . 1 (N = 16 identical columns)
+                umma_ts(tL, tP + kk * 8, odesc + 2 * kk, idesc_l, (e > 0 || hh > 0 || kk > 0) ? 1u : 0u);
+              if (hh + 1 < NH) {
+                umma_commit(bar_pv0_done);
+              } else {
+                umma_commit(bar_v_empty + 8 * sv);
+                umma_commit(bar_o_done);
+              }
+            }
+            __syncwarp();
           }
-          __syncwarp();
           if (++sv == kVStages) { sv = 0; phv ^= 1; }
         }
       }
     }
   } else if (warp < 4) {
     setmaxnreg_inc<kRegsMufu>();
-    softmax_half<B, 0, L::kSplit, false, kTok>(p, smem, tmem, n_ent, e0, h, I, bar_q, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
+    softmax_half<B, false, kTok>(p, smem, tmem, n_ent, e0, h, I, bar_q, bar_s_full, bar_s_free, bar_p_full, bar_pv0_done, bar_o_done);
   } else {
     setmaxnreg_inc<kRegsFma>();
-    softmax_half<B, L::kSplit, B, true, kTok>(p, smem, tmem, n_ent, e0, h, I, bar_q, bar_s_full, bar_s_free, bar_p_full, bar_o_done);
+    softmax_half<B, true, kTok>(p, smem, tmem, n_ent, e0, h, I, bar_q, bar_s_full, bar_s_free, bar_p_full, bar_pv0_done, bar_o_done);
   }
 
   tc_fence_before();

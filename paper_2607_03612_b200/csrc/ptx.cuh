@@ -192,9 +192,50 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&r)[8]) {
                : "r"(taddr)
                : "memory");
 }
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+      "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+      "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+      : "memory");
+}
+__device__ __forceinline__ void tmem_ld1(uint32_t taddr, uint32_t &r) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(r) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st1(uint32_t taddr, uint32_t r) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr), "r"(r) : "memory");
+}
+// N consecutive columns (N a sum of 32 / 16 / 8 chunks) of this warp's 32 lanes -> dst[0..N)
+template <int N>
+__device__ __forceinline__ void tmem_ld_n(uint32_t taddr, uint32_t *dst) {
+  static_assert(N % 8 == 0 && N > 0, "tmem_ld_n: multiples of 8 columns");
+  if constexpr (N >= 32) {
+    tmem_ld32(taddr, *reinterpret_cast<uint32_t(*)[32]>(dst));
+    if constexpr (N > 32) tmem_ld_n<N - 32>(taddr + 32, dst + 32);
+  } else if constexpr (N >= 16) {
+    tmem_ld16(taddr, *reinterpret_cast<uint32_t(*)[16]>(dst));
+    if constexpr (N > 16) tmem_ld_n<N - 16>(taddr + 16, dst + 16);
+  } else {
+    tmem_ld8(taddr, *reinterpret_cast<uint32_t(*)[8]>(dst));
+  }
+}
 __device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t (&r)[4]) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3])
                : "memory");
+}
+// N consecutive columns (N a sum of 16 / 8 / 4 chunks) <- src[0..N)
+template <int N>
+__device__ __forceinline__ void tmem_st_n(uint32_t taddr, const uint32_t *src) {
+  static_assert(N % 4 == 0 && N > 0, "tmem_st_n: multiples of 4 columns");
+  if constexpr (N >= 16) {
+    tmem_st16(taddr, *reinterpret_cast<const uint32_t(*)[16]>(src));
+    if constexpr (N > 16) tmem_st_n<N - 16>(taddr + 16, src + 16);
+  } else if constexpr (N >= 8) {
+    tmem_st8(taddr, *reinterpret_cast<const uint32_t(*)[8]>(src));
+    if constexpr (N > 8) tmem_st_n<N - 8>(taddr + 8, src + 8);
+  } else {
+    tmem_st4(taddr, *reinterpret_cast<const uint32_t(*)[4]>(src));
+  }
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
