@@ -56,12 +56,12 @@ constexpr int kTmemP = 208;  // P of ONE 64-key half of the tile, packed bf16 (3
 constexpr float kLazyLog2 = 8.f;
 constexpr int kSleepTma = 128, kSleepMma = 48;  // ns between two mbarrier polls of the producer / issuer warps
 constexpr float kFreezeLog2 = 64.f;  // freeze the reference max when no logit can exceed it by more than 2^64
-constexpr int kSplitHalf128 = 40;  // columns of every 64-key half whose exponentials use the MUFU (rest: FMA-pipe polynomial); multiple of 8
+constexpr int kSplitLo128 = 40, kSplitHi128 = 40;  // columns of the first / second 64-key half whose exponentials use the MUFU (rest: FMA-pipe polynomial); multiples of 8
 constexpr int kRegsMufu = 112, kRegsFma = 88, kRegsIdle = 40;  // 128*(112+88+40) = 30720 = 384 threads * 80 registers
 
 template <int B>
 struct AttnSmem {
-  static constexpr int kSplitHalf = (B == 128) ? kSplitHalf128 : 32;
+  static constexpr int split_of(int hh) { return (B == 128) ? (hh == 0 ? kSplitLo128 : kSplitHi128) : 32; }  // MUFU columns of half hh
   static constexpr int kQ = 0;                          // 128 x 64 bf16 (only the first B rows are loaded)
   static constexpr int kK = kQ + 128 * 128;             // kKStages x (B x 64 bf16)
   static constexpr int kV = kK + kKStages * B * 128;    // kVStages x (B x 64 bf16)
@@ -81,18 +81,20 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
                                              uint32_t bar_p_full /* [NH] */, uint32_t bar_pv0_done, uint32_t bar_o_done) {
   using L = AttnSmem<B>;
   constexpr int NH = B / 64;                       // 64-key halves of a tile
-  constexpr int kS = L::kSplitHalf;
-  constexpr int C0h = kFma ? kS : 0;               // first column of this group inside a half
-  constexpr int NCH = kFma ? 64 - kS : kS;         // columns of this group per half
-  constexpr int NC = NCH * NH;
-  static_assert(NCH % 8 == 0 && NCH > 0 && NCH < 64, "column split must be a multiple of 8");
+  // this group's columns of half hh: [64 hh + c0(hh), 64 hh + c0(hh) + nch(hh)); v[] holds half 0's columns, then half 1's
+  auto c0 = [](int hh) constexpr { return kFma ? L::split_of(hh) : 0; };
+  auto nch = [](int hh) constexpr { return kFma ? 64 - L::split_of(hh) : L::split_of(hh); };
+  constexpr int NCH0 = nch(0), NCH1 = (NH == 2) ? nch(1) : 0;
+  constexpr int NC = NCH0 + NCH1;
+  static_assert(NCH0 % 8 == 0 && NCH0 > 0 && NCH0 < 64 && NCH1 % 8 == 0 && (NH == 1 || (NCH1 > 0 && NCH1 < 64)), "column split must be a multiple of 8");
+  auto col_of = [&](int i) constexpr { return i < NCH0 ? c0(0) + i : 64 + c0(1) + (i - NCH0); };
   constexpr int kHalf = kFma ? 1 : 0;
   const int r = threadIdx.x & 127;
   const int pair_bar = 1 + (r >> 5);  // named barrier shared by the two warps that own these 32 rows
   // TMEM lane block of this warp; the shuffle makes it warp-uniform by construction so that ptxas keeps the tcgen05.ld/st
   // addresses in uniform registers instead of re-deriving them (R2UR) every iteration
   const uint32_t lane_off = (uint32_t)(__shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0) & 3) << 21;
-  const uint32_t tS = tmem + lane_off + C0h, tO = tmem + lane_off + kTmemO + 32 * kHalf, tP = tmem + lane_off + kTmemP + C0h / 2;
+  const uint32_t tS = tmem + lane_off, tO = tmem + lane_off + kTmemO + 32 * kHalf, tP = tmem + lane_off + kTmemP;
   const uint32_t tL = tmem + lane_off + kTmemL;
   float *smax = reinterpret_cast<float *>(smem + L::kMax);
   const int tail = p.N_kv - (p.NB_kv - 1) * B;  // valid keys in the last k-block
@@ -128,18 +130,18 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
   const float freeze_raw = kFreezeLog2 / c;
 
   for (int e = 0; e < n_ent; ++e) {
-    uint32_t v[NC];  // v[hh * NCH + i] = score of column 64 hh + C0h + i
+    uint32_t v[NC];  // v[i] = score of column col_of(i)
     mbar_wait(bar_s_full, e & 1);
     tc_fence_after();
-#pragma unroll
-    for (int hh = 0; hh < NH; ++hh) tmem_ld_n<NCH>(tS + 64 * hh, &v[hh * NCH]);
+    tmem_ld_n<NCH0>(tS + c0(0), v);
+    if constexpr (NH == 2) tmem_ld_n<(NCH1 > 0 ? NCH1 : 8)>(tS + 64 + c0(1), &v[NCH0]);
     tmem_ld_wait();
     tc_fence_before();
     mbar_arrive(bar_s_free);
     if (e == n_ent - 1 && last_is_tail) {
 #pragma unroll
       for (int i = 0; i < NC; ++i)
-        if ((i / NCH) * 64 + C0h + (i % NCH) >= tail) v[i] = 0xff800000u;  // -inf
+        if (col_of(i) >= tail) v[i] = 0xff800000u;  // -inf
     }
     if (kTok) {  // per-(query, key) mask of this tile: keys the query did not select get -inf before the max
       uint32_t mw[B / 32];
@@ -148,7 +150,7 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
       for (int w = 0; w < B / 32; ++w) mw[w] = r < B ? __ldg(mrow + w) : 0u;
 #pragma unroll
       for (int i = 0; i < NC; ++i) {
-        const int col = (i / NCH) * 64 + C0h + (i % NCH);
+        const int col = col_of(i);
         if (!((mw[col / 32] >> (col & 31)) & 1u)) v[i] = 0xff800000u;
       }
     }
@@ -188,14 +190,14 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
     // the polynomial group needs its argument clamped at -126 unless every x of the tile is known to be above it: frozen max,
     // |logit| <= bound for all 32 rows (Cauchy-Schwarz again: x >= -(bound + m) c), no masked (-inf) column in the tile
     const bool fast = kFma && !kTok && noclamp && !(e == n_ent - 1 && last_is_tail);
-    uint32_t pk[NCH / 2];
+    uint32_t pk[(NCH0 > NCH1 ? NCH0 : NCH1) / 2];
     auto exp_half = [&](auto clamp_tag, auto hh_tag) {
       constexpr bool kClamp = decltype(clamp_tag)::value;
       constexpr int hh = decltype(hh_tag)::value;
 #pragma unroll
-      for (int j = 0; j < NCH / 2; ++j) {
+      for (int j = 0; j < nch(hh) / 2; ++j) {
         const uint64_t x2 =
-            fma_f32x2(pack_f32x2(__uint_as_float(v[hh * NCH + 2 * j]), __uint_as_float(v[hh * NCH + 2 * j + 1])), c2, nmc2);
+            fma_f32x2(pack_f32x2(__uint_as_float(v[hh * NCH0 + 2 * j]), __uint_as_float(v[hh * NCH0 + 2 * j + 1])), c2, nmc2);
         float p0, p1;
         if (kFma) {
           exp2_emu_f32x2<kClamp>(x2, p0, p1);
@@ -232,7 +234,7 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
         mbar_wait(bar_pv0_done, e & 1);  // the MMAs of the first half have read the P buffer
         tc_fence_after();
       }
-      tmem_st_n<NCH / 2>(tP, pk);
+      tmem_st_n<nch(hh) / 2>(tP + c0(hh) / 2, pk);
       tmem_st_wait();
       tc_fence_before();
       mbar_arrive(bar_p_full + 8 * hh);
