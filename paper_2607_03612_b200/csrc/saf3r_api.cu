@@ -204,7 +204,8 @@ saf3r_status saf3r_create(saf3r_ctx **out, int device) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<128>::kTotal);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(saf3r_attn_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem<64>::kTotal);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(select_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(select_fused_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(select_fused_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 72 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(token_sim_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSimSmem);
   if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->counter_dev, sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->kmax_ring, sizeof(float) * kKmaxSlots * kKmaxSlotFloats);
@@ -270,9 +271,9 @@ saf3r_status saf3r_query_sizes(const saf3r_shape *shape, const saf3r_head_cfg *c
 // Launch plan of the score + select kernel: rows per score strip R (16; fewer when R*NB keys do not fit the shared-memory budget of
 // two CTAs per SM - then of one - or when the BLOCK_TOPK heads are few, so that the strips cover every SM twice) and the dynamic
 // shared memory.  A closed form of (shape, cfg, SM count), computed BEFORE anything is enqueued.
-struct SelPlan { int R; size_t smem; const char *unsupported; };
+struct SelPlan { int R; size_t smem; const char *unsupported; bool tail_stage; };
 static SelPlan select_plan(const SelGeom &g, int n_block, int n_probe, int sm_count) {
-  SelPlan p{kSelRows, 0, nullptr};
+  SelPlan p{kSelRows, 0, nullptr, false};
   const size_t row = (size_t)kt_stride(g.NB) * 4;
   if (n_block > 0) {
     const size_t qbytes = 64 * kSelRows * 4;
@@ -280,8 +281,12 @@ static SelPlan select_plan(const SelGeom &g, int n_block, int n_probe, int sm_co
     if (row > budget) budget = 220 * 1024 - qbytes;
     if (row > budget) { p.unsupported = "NB too large for the select kernel"; return p; }
     while ((size_t)p.R * row > budget) --p.R;
-    while (p.R > 8 && (int64_t)n_block * ((g.NB + p.R - 1) / p.R) < 2 * (int64_t)sm_count) p.R = (p.R + 1) / 2;
+    while (p.R > 8 && ((int64_t)n_block * ((g.NB + p.R - 1) / p.R) < 2 * (int64_t)sm_count || g.NB <= 1152)) p.R = (p.R + 1) / 2;  // NB <= 1152: 8-row strips, three CTAs per SM
     p.smem = (size_t)p.R * row + qbytes;
+    // staging of the columns left over after the groups of 1024 (score_rows), when they are few
+    const int64_t tail_cols = kt_stride(g.NB) - (g.NB / 1024) * 1024;
+    p.tail_stage = g.NB >= 1024 && tail_cols <= kSelTailCols && p.smem + 64 * tail_cols * 4 <= (p.smem <= 108 * 1024 ? 108 * 1024 : 220 * 1024);
+    if (p.tail_stage) p.smem += 64 * tail_cols * 4;
   }
   if (n_probe > 0) {
     if (row > 220 * 1024) { p.unsupported = "NB too large for the probe stage"; return p; }
@@ -380,6 +385,7 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
   FusedPlan fp;
   memset(&fp, 0, sizeof fp);
   fp.R = sp.R;
+  fp.tail_stage = sp.tail_stage ? 1 : 0;
   fp.strips = (g.NB + sp.R - 1) / sp.R;
   fp.light_chunks = light_chunks;
   fp.pool_need = 2 * tasks_per_job;
@@ -399,9 +405,13 @@ static saf3r_status select_impl(saf3r_ctx *ctx, const void *q, const void *k, co
   CU_CHECK(cudaMemsetAsync(counters, 0, kSelCounters * sizeof(int), st));
   auto launch = [&](int t_begin, int t_end, int counter) {
     fp.t_begin = t_begin; fp.t_end = t_end; fp.counter = counter;
-    const int ctas = t_end - t_begin < 2 * ctx->sm_count ? t_end - t_begin : 2 * ctx->sm_count;
+    // three CTAs per SM when the strips are short and the rows fit the 36-keys-per-lane register top-n (80 registers per thread):
+    // a CTA that is busy with a latency-bound score strip then leaves two CTAs of the SM streaming Q / K
+    const bool occ3 = sp.R <= 8 && g.NB <= 1152 && sp.smem <= 72 * 1024;
+    const int per_sm = occ3 ? 3 : 2;
+    const int ctas = t_end - t_begin < per_sm * ctx->sm_count ? t_end - t_begin : per_sm * ctx->sm_count;
     if (ctas <= 0) return;
-    select_fused_kernel<<<ctas, 256, sp.smem, st>>>((const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart, (uint32_t *)(wsb + w.pkeys), probe, lists->row_ptr,
+    (occ3 ? select_fused_kernel<3> : select_fused_kernel<2>)<<<ctas, 256, sp.smem, st>>>((const __nv_bfloat16 *)q, (const __nv_bfloat16 *)k, qt, kt, qpart, (uint32_t *)(wsb + w.pkeys), probe, lists->row_ptr,
                                                    lists->col_idx, (const int64_t *)(cache ? cache->row_ptr : nullptr),
                                                    (const int32_t *)(cache ? cache->col_idx : nullptr), counters, g, jobs, plan, ca, sets, fp);
     ctx->launches += 1;

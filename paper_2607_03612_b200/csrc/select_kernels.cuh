@@ -197,8 +197,10 @@ __device__ __forceinline__ void warp_topn_bisect_impl(const uint32_t *key, int N
   }
 }
 // `base` is added to every index written (the keys may be a window of a longer row)
+// kSmall: the caller guarantees NB <= 32 * 36 (the three-CTAs-per-SM build of the fused kernel: 80 registers per thread)
+template <bool kSmall = false>
 __device__ __forceinline__ void warp_topn_bisect(const uint32_t *key, int NB, int n, int32_t *out, int base = 0) {
-  if (NB <= 32 * 36) warp_topn_bisect_impl<36>(key, NB, n, out, base);
+  if (kSmall || NB <= 32 * 36) warp_topn_bisect_impl<36>(key, NB, n, out, base);
   else if (NB <= 32 * 72) warp_topn_bisect_impl<72>(key, NB, n, out, base);
   else warp_topn_bisect_impl<0>(key, NB, n, out, base);
 }
@@ -407,11 +409,12 @@ __device__ inline void probe_score_task(const float *qpart, const float *kt, uin
   __syncthreads();
   if (half == 0 && J < g.NB) probe_keys[(int64_t)h * g.NB + J] = score_key((ph[col] + ph[kProbeChunk + col]) * 0.125f);
 }
+template <bool kSmall>
 __device__ inline void probe_topn_task(const uint32_t *probe_keys, int32_t *probe_list, const SelGeom &g, int h, int n,
                                        uint32_t *key /* dynamic smem, NB */) {
   for (int J = threadIdx.x; J < g.NB; J += 256) key[J] = __ldcg(probe_keys + (int64_t)h * g.NB + J);
   __syncthreads();
-  if (threadIdx.x < 32) warp_topn_bisect(key, g.NB, n, probe_list + (int64_t)h * g.NB);
+  if (threadIdx.x < 32) warp_topn_bisect<kSmall>(key, g.NB, n, probe_list + (int64_t)h * g.NB);
 }
 
 // row_ptr entries of head h (one task of the fused kernel, whole CTA)
@@ -448,6 +451,7 @@ __device__ inline void rowptr_task(int64_t *__restrict__ row_ptr, const SelGeom 
 // round of 4 * kPoolLoads rows, fp32 accumulate, optional per-token L2 normalisation (cosine), fold of the four row groups with shuffles,
 // mean -> Qtilde (row-major) or Ktilde^T (transposed).  The Q job of a QUERY_PROBE head also leaves each warp's token sum in
 // wsum for the task's partial sum of qbar, written by the caller after its barrier.
+template <int kLoads>
 __device__ __forceinline__ void pool_task(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k, float *__restrict__ qt,
                                           float *__restrict__ kt, const SelGeom &g, const PoolJobs &jobs, int job, int task_in_job,
                                           float (*wsum)[64]) {
@@ -463,16 +467,16 @@ __device__ __forceinline__ void pool_task(const __nv_bfloat16 *__restrict__ q, c
     const int cnt = (int)i64min(g.B, g.N - t0);
     const __nv_bfloat16 *src = (which ? k : q) + (int64_t)h * g.stride_head + t0 * g.stride_token + sub * 8;
 #pragma unroll 1
-    for (int r0 = 0; r0 < cnt; r0 += 4 * kPoolLoads) {
-      uint4 raw[kPoolLoads];
+    for (int r0 = 0; r0 < cnt; r0 += 4 * kLoads) {
+      uint4 raw[kLoads];
 #pragma unroll
-      for (int i = 0; i < kPoolLoads; ++i) {
+      for (int i = 0; i < kLoads; ++i) {
         const int r = r0 + rg + 4 * i;
         raw[i] = make_uint4(0, 0, 0, 0);
         if (r < cnt) raw[i] = ld_stream_16(src + (int64_t)r * g.stride_token);
       }
 #pragma unroll
-      for (int i = 0; i < kPoolLoads; ++i) {
+      for (int i = 0; i < kLoads; ++i) {
         const uint32_t w[4] = {raw[i].x, raw[i].y, raw[i].z, raw[i].w};
         float v[8];
 #pragma unroll
@@ -546,16 +550,30 @@ __device__ __forceinline__ uint64_t sel_fma2(uint64_t a, uint64_t b, uint64_t c)
 // Groups of 1024 columns: each thread owns four consecutive columns (one 16-byte load of Ktilde^T per d, coalesced across
 // the warp) and RT rows, 4*RT accumulators as packed row pairs.  The columns left over (< 1024) are spread over all threads
 // as (four rows, four columns) tasks.  Every sum runs in the order d = 0..63 with fp32 FMAs, so both paths give the same bits.
+// When at most kSelTailCols columns are left over after the groups of 1024 (C3: NB = 1074 -> 52), their 64 x cols slice of
+// Ktilde^T is copied to shared memory (kl) with cp.async while the groups are computed, and the tail becomes (row, column quad)
+// tasks over all threads reading shared memory: one L2 round trip for the tail instead of a latency-bound pass of its own.
+constexpr int kSelTailCols = 128;
 template <int RT>
 __device__ __forceinline__ void score_rows(const float *__restrict__ qt, const float *__restrict__ kt, uint32_t *keys, float *qT,
-                                           const SelGeom &g, int h, int I0, int rows, float cs) {
+                                           const SelGeom &g, int h, int I0, int rows, float cs, float *kl) {
   for (int i = threadIdx.x; i < 64 * RT; i += blockDim.x) {
     const int d = i / RT, r = i % RT;
     qT[i] = r < rows ? qt[((int64_t)h * g.NB + I0 + r) * 64 + d] : 0.f;
   }
-  __syncthreads();
   const int64_t ld = kt_stride(g.NB);
   const float *kh = kt + (int64_t)h * 64 * ld;
+  const int Jtail = (g.NB / 1024) * 1024, tail_quads = (int)((ld - Jtail) / 4);
+  const bool staged = kl != nullptr && Jtail > 0 && tail_quads * 4 <= kSelTailCols;
+  if (staged) {
+    for (int i = threadIdx.x; i < 64 * tail_quads; i += blockDim.x) {
+      const int d = i / tail_quads, qd = i % tail_quads;
+      const uint32_t dst = (uint32_t)__cvta_generic_to_shared(kl + (d * tail_quads + qd) * 4);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(kh + (int64_t)d * ld + Jtail + 4 * qd) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  }
+  __syncthreads();
   int Jb = 0;
   for (; Jb + 1024 <= g.NB; Jb += 1024) {
     const int J = Jb + 4 * (int)threadIdx.x;
@@ -603,6 +621,24 @@ __device__ __forceinline__ void score_rows(const float *__restrict__ qt, const f
         *reinterpret_cast<uint4 *>(keys + (size_t)(2 * r2 + 1) * ld + J) =
             make_uint4(score_key(hi[0] * cs), score_key(hi[1] * cs), score_key(hi[2] * cs), score_key(hi[3] * cs));
     }
+  }
+  if (staged) {
+    // (row, column quad) tasks from shared memory; the same fp32 FMA chain d = 0..63 as the packed form above, so the same bits
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < rows * tail_quads; idx += blockDim.x) {
+      const int r = idx / tail_quads, qd = idx % tail_quads;
+      float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll 16
+      for (int d = 0; d < 64; ++d) {
+        const float4 kv = *reinterpret_cast<const float4 *>(kl + (d * tail_quads + qd) * 4);
+        const float qv = qT[d * RT + r];
+        a0 = fmaf(qv, kv.x, a0); a1 = fmaf(qv, kv.y, a1); a2 = fmaf(qv, kv.z, a2); a3 = fmaf(qv, kv.w, a3);
+      }
+      *reinterpret_cast<uint4 *>(keys + (size_t)r * ld + Jtail + 4 * qd) =
+          make_uint4(score_key(a0 * cs), score_key(a1 * cs), score_key(a2 * cs), score_key(a3 * cs));
+    }
+    return;
   }
   // left-over columns: (four rows, column quad) tasks; the padded columns NB..NBp-1 of Ktilde^T are never written, so their
   // scores are computed from garbage and stored into the row's padding, which nothing reads
@@ -663,6 +699,7 @@ struct FusedPlan {
   int32_t strips, R, light_chunks;
   int32_t pool_need;                      // pool tasks per head = 2 jobs * tasks_per_job
   int32_t counter;                        // which ticket counter (0 / 1)
+  int32_t tail_stage;                     // the strips have a shared-memory staging area for the left-over columns (score_rows)
 };
 constexpr int kSelScratch = 17 * 64 * 4 + 2 * kProbeChunk * 4;  // bytes of scratch of a probe-score task (partial sums of qbar, qbar, half sums)
 constexpr int kSelCounters = 2 + 4 * SAF3R_MAX_HEADS;  // int32: 2 ticket counters, pooled[h], rowptr_done[h], probe_done[h], pscore_done[h]
@@ -682,7 +719,8 @@ __device__ __forceinline__ void signal_count(int *ctr) {
   if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(ctr) : "memory");  // release: cumulative over the barrier
 }
 
-__global__ void __launch_bounds__(256, 2) select_fused_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
+template <int kOcc>  // CTAs per SM the register budget is sized for (3: only strips of <= 8 rows and rows of <= 1152 keys)
+__global__ void __launch_bounds__(256, kOcc) select_fused_kernel(const __nv_bfloat16 *__restrict__ q, const __nv_bfloat16 *__restrict__ k,
                                                               float *__restrict__ qt, float *__restrict__ kt, float *__restrict__ qpart,
                                                               uint32_t *__restrict__ probe_keys, int32_t *__restrict__ probe_list, int64_t *__restrict__ row_ptr,
                                                               int32_t *__restrict__ col_idx, const int64_t *__restrict__ cache_row_ptr,
@@ -734,7 +772,7 @@ __global__ void __launch_bounds__(256, 2) select_fused_kernel(const __nv_bfloat1
     if (pool_task_id >= 0) {
       const int tasks_per_job = (g.NB + kPoolBlocksPerTask - 1) / kPoolBlocksPerTask;
       const int job = pool_task_id / tasks_per_job, task_in_job = pool_task_id % tasks_per_job;
-      pool_task(q, k, qt, kt, g, jobs, job, task_in_job, wsum);
+      pool_task<(kOcc > 2 ? 8 : kPoolLoads)>(q, k, qt, kt, g, jobs, job, task_in_job, wsum);
       if (jobs.probe[job] != 0 && jobs.which[job] == 0) {  // the task's token sum for qbar, warps in a fixed order
         __syncthreads();
         if (threadIdx.x < 64) {
@@ -758,15 +796,16 @@ __global__ void __launch_bounds__(256, 2) select_fused_kernel(const __nv_bfloat1
       const int64_t ld = kt_stride(g.NB);
       float *qT = sm + (size_t)R * ld;                     // [64][RT] (rows past `rows` are zero)
       const float cs = c.score_mode == SAF3R_SCORE_COSINE ? 1.f : 0.125f;
-      if (R <= 4) score_rows<4>(qt, kt, keys, qT, g, h, I0, rows, cs);
-      else if (R <= 8) score_rows<8>(qt, kt, keys, qT, g, h, I0, rows, cs);
-      else score_rows<kSelRows>(qt, kt, keys, qT, g, h, I0, rows, cs);
+      float *kl = fp.tail_stage ? qT + 64 * kSelRows : nullptr;  // [64][tail quads][4] staging of the left-over columns
+      if (R <= 4) score_rows<4>(qt, kt, keys, qT, g, h, I0, rows, cs, kl);
+      else if (R <= 8) score_rows<8>(qt, kt, keys, qT, g, h, I0, rows, cs, kl);
+      else if constexpr (kOcc <= 2) score_rows<kSelRows>(qt, kt, keys, qT, g, h, I0, rows, cs, kl);
       __syncthreads();
       const int64_t base = plan.head_base[h];  // BLOCK_TOPK rows all have the same length: offsets are a closed form
       const int len = plan.const_len[h];
       for (int r = warp; r < rows; r += 8) {
         int32_t *out = col_idx + base + (int64_t)(I0 + r) * len;
-        if (c.topk_scope == SAF3R_SCOPE_GLOBAL) warp_topn_bisect(keys + (size_t)r * ld, g.NB, (int)i64min(c.keep_blocks, g.NB), out);
+        if (c.topk_scope == SAF3R_SCOPE_GLOBAL) warp_topn_bisect<(kOcc > 2)>(keys + (size_t)r * ld, g.NB, (int)i64min(c.keep_blocks, g.NB), out);
         else warp_per_frame_emit(keys + (size_t)r * ld, g, c.topk_per_frame, out);
       }
       continue;
@@ -784,7 +823,7 @@ __global__ void __launch_bounds__(256, 2) select_fused_kernel(const __nv_bfloat1
     if (x < fp.n_probe) {
       const int h = sets.probe[x];
       wait_count(pscore_done + h, fp.pchunks);
-      probe_topn_task(probe_keys, probe_list, g, h, (int)i64min(cfg.c[h].keep_blocks, g.NB), reinterpret_cast<uint32_t *>(sm));
+      probe_topn_task<(kOcc > 2)>(probe_keys, probe_list, g, h, (int)i64min(cfg.c[h].keep_blocks, g.NB), reinterpret_cast<uint32_t *>(sm));
       signal_count(probe_done + h);
       continue;
     }
