@@ -316,28 +316,18 @@ __device__ __forceinline__ void emit_light_row(const SelGeom &g, const saf3r_hea
 }
 constexpr int kLightRows = 32;  // rows per CTA of the light emitters (8 warps x 4 rows)
 
-// Which heads each launch serves (host-built).
+// Which heads each kind of task serves (host-built).
 struct HeadSets {
   int32_t n_emit, n_light, n_block, n_probe, n_cached;
-  uint8_t cached[SAF3R_MAX_HEADS];  // launch 2: CACHED heads (rows copied from the index cache)
-  uint8_t emit[SAF3R_MAX_HEADS];   // launch 1: closed-form heads whose rows all have the same length (no dependence at all)
-  uint8_t light[SAF3R_MAX_HEADS];  // launch 2: per-row-length STATIC heads (need row_ptr)
-  uint8_t block[SAF3R_MAX_HEADS];  // launch 2: BLOCK_TOPK heads (score + top-n)
-  uint8_t probe[SAF3R_MAX_HEADS];  // launch 2: QUERY_PROBE heads, one probe CTA each (probe + the head's lists)
+  uint8_t cached[SAF3R_MAX_HEADS];  // CACHED heads (rows copied from the index cache; need row_ptr)
+  uint8_t emit[SAF3R_MAX_HEADS];   // closed-form heads whose rows all have the same length (no dependence at all)
+  uint8_t light[SAF3R_MAX_HEADS];  // per-row-length STATIC heads (need row_ptr)
+  uint8_t block[SAF3R_MAX_HEADS];  // BLOCK_TOPK heads (score strips: scores + top-n)
+  uint8_t probe[SAF3R_MAX_HEADS];  // QUERY_PROBE heads (probe-score chunks, one top-n task, list copies)
 };
 
-// ------------------------------------------------------------------------------------------------ pool + row_ptr + probe
-// One launch, two kinds of CTA (256 threads):
-//   blockIdx.x <  pool_ctas : 8 warps, ONE WARP PER TOKEN BLOCK.  job j = (tensor, head) pairs that the head's rule reads
-//                            (host-built list, QUERY_PROBE heads first), warp w -> (job = w / NB, J = w % NB).  A warp
-//                            streams its block's B x 128 B with 16-byte loads (lane = 16-byte chunk (l&7) of rows
-//                            (l>>3) + 4i, eight loads in flight), accumulates in fp32, folds the four row groups with
-//                            shuffles and writes the 64-float mean.
-//                            The Q job of a QUERY_PROBE head also writes its CTA's token sum (for qbar).
-//   next H CTAs             : one CTA per head writes that head's row_ptr entries: head_base + I*len for heads whose
-//                            rows all have the same length, a block scan of the closed-form lengths otherwise.
-//   remaining CTAs          : the lists of the closed-form heads whose rows all have the same length (DENSE, UNIFORM_STRIDE,
-//                            STATIC/ANCHOR): 32 rows per CTA, written under the pooling's HBM time.
+// ------------------------------------------------------------------------------------------------ pool / row_ptr / probe tasks
+// (tasks of select_fused_kernel, each run by a whole 256-thread CTA; the ticket order is described at the kernel)
 constexpr int kPoolBlocksPerTask = 8;  // one block per warp
 constexpr int kPoolLoads = 16;         // independent 16-byte loads in flight per lane (64 token rows per round; 8 measured the same)
 struct PoolJobs {
@@ -522,14 +512,11 @@ __device__ __forceinline__ void pool_task(const __nv_bfloat16 *__restrict__ q, c
   }
 }
 
-// ------------------------------------------------------------------------------------------------ select
-// 1-D grid, 256 threads (8 warps): one probe CTA per QUERY_PROBE head (probe, top-n, and the head's lists), then
-// n_block * ceil(NB/R) heavy CTAs (R = 16 rows, fewer when NB is large or the BLOCK_TOPK heads are few), then light CTAs
-// (32 rows each) for the per-row-length STATIC heads.
-//   BLOCK_TOPK heads: score rows s[I][J] = Qtilde_I . Ktilde_J * c (fp32 FMA in the order d = 0..63, as packed
-//   row pairs; each thread owns two columns J and keeps 16 row accumulators for each) stored as order-preserving keys
-//   in shared memory, then one warp per row: bisection top-n or per-frame top-k.
-// dynamic smem: R*NB keys + 64*R floats (Qtilde rows, transposed so that four rows of one d are one 16-byte load).
+// ------------------------------------------------------------------------------------------------ score strips
+// BLOCK_TOPK heads: score rows s[I][J] = Qtilde_I . Ktilde_J * c (fp32 FMA in the order d = 0..63, as packed row pairs) stored as
+// order-preserving keys in shared memory (R rows x NB keys; the NB x NB matrix never exists), then one warp per row: bisection
+// top-n or per-frame top-k.  Dynamic smem of a strip: R*NBp keys + 64*kSelRows floats (Qtilde rows, transposed so that four rows
+// of one d are one 16-byte load) + the optional staging area of the left-over columns.
 constexpr int kSelRows = 16;
 
 __device__ __forceinline__ uint64_t sel_pack2(float lo, float hi) {
