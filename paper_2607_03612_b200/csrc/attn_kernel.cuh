@@ -3,11 +3,13 @@
 // One CTA per (head h, q-block I), two CTAs resident per SM.  At D = 64 the exponentials, not the tensor pipe, bound
 // this kernel (16 384 exp per 128x128 tile against 16 MUFU lanes/clk/SM = 1024 clk, versus 512 clk of MMA), so the
 // softmax of a tile is split by COLUMNS over two warp groups that use different pipes:
-//   warps 0-3   "MUFU" softmax: thread r owns q-row r (TMEM lane r), columns [0, kSplit): p = ex2.approx(s*c - m*c)
-//   warps 4-7   "FMA"  softmax: same rows, columns [kSplit, B): 2^x by Cody-Waite + degree-3 polynomial on the FMA/ALU
+//   warps 0-3   "MUFU" softmax: thread r owns q-row r (TMEM lane r), the first kSplitLo / kSplitHi columns of the tile's two
+//               64-key halves: p = ex2.approx(s*c - m*c)
+//   warps 4-7   "FMA"  softmax: same rows, the other columns of each half: 2^x by Cody-Waite + degree-3 polynomial on the FMA/ALU
 //               pipes (no MUFU).  The two halves of a row exchange their partial row max through shared memory.
 //   warp  8     TMA producer: Q tile once, then K_J into a 3-stage ring and V_J into a 2-stage ring
-//   warp  9     TMEM allocator + MMA issuer (one thread): S = Q K_J^T (tcgen05 SS), O += P V_J (tcgen05 TS: P from TMEM)
+//   warp  9     TMEM allocator + MMA issuer (one thread): S = Q K_J^T (tcgen05 SS); per 64-key half of P: O += P V_J and the row
+//               sums l += P 1 (tcgen05 TS: P from TMEM; N = 16 all-ones B tile), so the softmax warps add nothing per element
 //   warps 10-11 idle (they only complete the third warpgroup so that setmaxnreg can hand its registers over); in the token-list
 //               mode warp 8 gathers the K tiles and warp 10 the V tiles with cp.async instead of TMA
 // Running max is lazy (moves only when a row max grows by more than 2^8), so O in TMEM is rescaled rarely.  And it is
@@ -16,7 +18,8 @@
 // 2^kFreezeLog2 of the row's reference max for all 32 rows of a warp, no later tile can overflow (p <= 2^64, far inside the
 // bf16 / fp32 exponent range) and none can underflow relative to the true max, so the remaining tiles skip the row-max pass,
 // the exchange between the two halves and the named barrier altogether - about an eighth of the softmax instructions.
-// TMEM columns: S [0,B) fp32, O [128,192) fp32, P [192,192+B/2) packed bf16.
+// TMEM columns: S [0,B) fp32, O [128,192) fp32, l [192,208) fp32, P [208,240): one 64-key half of the tile (packed bf16; of the second
+// half only the FMA group's keys [96,128)), PB [240,256): the MUFU group's keys [64,96) of the second half.
 #pragma once
 #include <type_traits>
 
@@ -56,7 +59,9 @@ constexpr int kTmemP = 208;  // P of ONE 64-key half of the tile, packed bf16 (3
 constexpr float kLazyLog2 = 8.f;
 constexpr int kSleepTma = 128, kSleepMma = 48;  // ns between two mbarrier polls of the producer / issuer warps
 constexpr float kFreezeLog2 = 64.f;  // freeze the reference max when no logit can exceed it by more than 2^64
-constexpr int kSplitLo128 = 40, kSplitHi128 = 40;  // columns of the first / second 64-key half whose exponentials use the MUFU (rest: FMA-pipe polynomial); multiples of 8
+constexpr int kTmemPB = 240; // second P buffer (16 columns): the MUFU group's keys [64, 96) of the tile, so that the group on the critical path never waits for the first half's MMAs
+constexpr int kSplitLo128 = 40, kSplitHi128 = 32;
+static_assert(kSplitHi128 == 32, "the MUFU group's second-half keys must be exactly the two K = 16 steps that read kTmemPB");  // columns of the first / second 64-key half whose exponentials use the MUFU (rest: FMA-pipe polynomial); multiples of 8
 constexpr int kRegsMufu = 112, kRegsFma = 88, kRegsIdle = 40;  // 128*(112+88+40) = 30720 = 384 threads * 80 registers
 
 template <int B>
@@ -231,10 +236,13 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
           }
         }
       } else {
-        mbar_wait(bar_pv0_done, e & 1);  // the MMAs of the first half have read the P buffer
-        tc_fence_after();
+        if (kFma || NH == 1) {
+          mbar_wait(bar_pv0_done, e & 1);  // the MMAs of the first half have read the P buffer
+          tc_fence_after();
+        }
       }
-      tmem_st_n<nch(hh) / 2>(tP + c0(hh) / 2, pk);
+      if (hh == 1 && !kFma) tmem_st_n<nch(hh) / 2>(tmem + lane_off + kTmemPB, pk);   // the MUFU group's second-half keys [64, 96): a buffer of their own
+      else tmem_st_n<nch(hh) / 2>(tP + c0(hh) / 2, pk);
       tmem_st_wait();
       tc_fence_before();
       mbar_arrive(bar_p_full + 8 * hh);
@@ -460,10 +468,10 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
               const uint64_t vdesc = umma_desc_sw128(sbase + L::kV + sv * B * 128);
 #pragma unroll
               for (int kk = 0; kk < 4; ++kk)   // O += P_half . V_half (K = 16 keys per MMA; P packed: 8 columns per step)
-                umma_ts(tO, tP + kk * 8, vdesc + (uint64_t)(hh * 4 + kk) * 128, idesc_pv, (e > 0 || hh > 0 || kk > 0) ? 1u : 0u);
+                umma_ts(tO, (hh == 1 && kk < 2) ? tmem + kTmemPB + kk * 8 : tP + kk * 8, vdesc + (uint64_t)(hh * 4 + kk) * 128, idesc_pv, (e > 0 || hh > 0 || kk > 0) ? 1u : 0u);
 #pragma unroll
               for (int kk = 0; kk < 4; ++kk)   // l += P_half . 1 (N = 16 identical columns)
-                umma_ts(tL, tP + kk * 8, odesc + 2 * kk, idesc_l, (e > 0 || hh > 0 || kk > 0) ? 1u : 0u);
+                umma_ts(tL, (hh == 1 && kk < 2) ? tmem + kTmemPB + kk * 8 : tP + kk * 8, odesc + 2 * kk, idesc_l, (e > 0 || hh > 0 || kk > 0) ? 1u : 0u);
               if (hh + 1 < NH) {
                 umma_commit(bar_pv0_done);
               } else {
