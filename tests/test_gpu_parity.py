@@ -285,6 +285,53 @@ def test_select_planted_exact_ties(env):
             assert np.all(hl.scores[:, 7] == hl.scores[:, 3]) and np.all(hl.scores[:, 12] == hl.scores[:, 3])
 
 
+def test_select_planted_ties_across_the_staged_tail(env):
+    """NB = 1074 (the C3 block count): columns [0, 1024) are scored by the register-tiled groups, columns [1024, 1074) from the
+    shared-memory staging of the left-over columns, in strips of 8 rows with three CTAs per SM.  K blocks duplicated ACROSS the
+    two paths must give bit-identical scores, so that an exact tie at the cut goes to the lower index with no near-tie excuse:
+    in every row of the GPU lists a kept copy implies that every lower-indexed copy is kept too."""
+    sf, ctx, torch = env
+    sh = sy.Shape(S=50, G=37, H=3, D=64, B=64)                   # N = 68700, NB = 1074, tail 28
+    assert sh.NB == 1074
+    gens = [sy.GEN_SAME_POSITION, sy.GEN_SINK, sy.GEN_SAME_POSITION]
+    cfgs = [sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=107),
+            sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=61),
+            sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=23, score_mode=sy.SCORE_COSINE)]
+    L = sy.make_layer(sh, gens, cfgs, seed=23)
+    B = sh.B
+    copies = ((1030, 5), (1060, 5), (1050, 700), (1072, 1023), (1024, 1023))   # (dst in the tail path, src in the group path)
+    for h in range(sh.H):
+        for dst, src in copies:
+            L.k[h][dst * B:(dst + 1) * B] = L.k[h][src * B:(src + 1) * B]
+    strip_rows, smem = ctx.select_plan(c_shape(sf, sh), L.cfgs)
+    assert strip_rows == 8, "NB <= 1152 takes 8-row strips (three CTAs per SM)"
+    q, k, _ = upload(L)
+    lists = ctx.select(q, k, c_shape(sf, sh), L.cfgs)
+    torch.cuda.synchronize()
+    assert ctx.check_lists(c_shape(sf, sh), lists) == 0
+    rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
+    hls = oracle_lists(L)
+    stats = compare_lists(L, rp, col, hls, tag="NB=1074 planted ties across the staged tail (3 heads)")
+    print("NB=1074 planted-tie near-ties:", stats)
+    assert stats["tie_floored"] <= 1e-4 * stats["entries"]
+    groups = {}
+    for dst, src in copies:
+        groups.setdefault(src, [src]).append(dst)
+    hit = 0
+    for h, hl in enumerate(hls):
+        if hl.scores is not None:                                # the planted ties really are exact in the oracle
+            for dst, src in copies:
+                assert np.all(hl.scores[:, dst] == hl.scores[:, src])
+        r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
+        for I in range(sh.NB):
+            row = set(col[r[I]:r[I + 1]].tolist())
+            for src, members in groups.items():
+                kept = [m in row for m in sorted(members)]
+                assert kept == sorted(kept, reverse=True), f"head {h} row {I}: copies of block {src} kept out of index order: {kept}"
+                hit += any(kept) and not all(kept)
+    print("rows whose cut falls inside a planted tie group:", hit)
+
+
 def test_select_large_nb_paths(env):
     """NB = 1160 > 1152: the top-n keeps 72 keys per lane in registers (the 36-key variant ends at NB = 1152; only NB > 2304, the
     C5 shape, reads its keys from shared memory) and the score stage runs its 1024-column main pass plus a left-over pass;
