@@ -106,6 +106,50 @@ def test_sparse_attn_empty_and_handmade_lists(env):
         assert np.abs(ls[~empty] - ref_lse[~empty]).max() <= 1e-2
 
 
+@pytest.mark.parametrize("B", [128, 64])
+def test_running_max_moves_every_tile_and_never_freezes(env, B):
+    """Hand-made inputs that drive the rare paths of the running max: head 0's logits GROW by 8 (11.5 in log2) from one k-block to
+    the next, so the reference max moves on every tile and O and the row-sum column in TMEM are rescaled each time; head 1's
+    logits SHRINK by 8 per block (the first tile sets the max, every later weight underflows towards 0); head 2 is head 0 with
+    one key of enormous norm in a block that no list contains, so the Cauchy-Schwarz bound never lets the max freeze.  Dense
+    lists, a strided subset and a single-block list; outputs and lse against the oracle."""
+    sf, ctx, torch = env
+    S, G, H, D = 3, 17, 3, 64
+    sh = sy.Shape(S=S, G=G, H=H, D=D, B=B)                     # N = 882
+    N, NB = sh.N, sh.NB
+    rng = np.random.default_rng(31)
+    u = rng.standard_normal(D).astype(np.float32)
+    u /= np.linalg.norm(u)
+    blk = (np.arange(N) // B).astype(np.float32)
+    qf = np.tile(8.0 * u, (N, 1)) + 0.05 * rng.standard_normal((N, D)).astype(np.float32)
+    k_up = (blk[:, None] + 1.0) * 8.0 * u[None, :]
+    k_dn = (NB - blk[:, None]) * 8.0 * u[None, :]
+    k_big = k_up.copy()
+    k_big[(NB - 1) * B + 3] = 4000.0 * u                        # |k| = 4000 in the last block, which head 2's lists leave out
+    vf = rng.standard_normal((H, N, D)).astype(np.float32)
+    q = np.stack([sy.f32_to_bf16_bits(qf)] * H)
+    k = np.stack([sy.f32_to_bf16_bits(x.astype(np.float32)) for x in (k_up, k_dn, k_big)])
+    v = sy.f32_to_bf16_bits(vf)
+    rows = []
+    for h in range(H):
+        for I in range(NB):
+            if h == 2:
+                rows.append(np.arange(0, NB - 1, dtype=np.int32))                    # everything but the last block
+            else:
+                rows.append([np.arange(NB, dtype=np.int32), np.arange(I % 2, NB, 2, dtype=np.int32),
+                             np.array([I], np.int32)][I % 3])
+    row_ptr = np.concatenate([[0], np.cumsum([len(r) for r in rows])]).astype(np.int64)
+    col = np.concatenate(rows)
+    qd, kd, vd = (torch.from_numpy(x.view(np.int16)).cuda().view(torch.bfloat16) for x in (q, k, v))
+    out, lse = ctx.sparse_attn(qd, kd, vd, c_shape(sf, sh), dev_lists(sf, torch, row_ptr, col), out_fp32=True, want_lse=True)
+    torch.cuda.synchronize()
+    for h in range(H):
+        rp = row_ptr[h * NB:(h + 1) * NB + 1]
+        ref, ref_lse = orc.attn_lists(q[h], k[h], v[h], B, rp - rp[0], col[rp[0]:rp[-1]])
+        check_attention(out[h].cpu().numpy(), ref, f"runmax B={B} head {h}")
+        assert np.abs(lse[h].cpu().numpy() - ref_lse).max() <= 2e-2 * max(1.0, float(np.abs(ref_lse).max()) / 64.0)
+
+
 def test_strided_layout_nhd(env):
     """[N][H][D] tensors through the two strides."""
     sf, ctx, torch = env
