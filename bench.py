@@ -473,7 +473,7 @@ def run_ours(args):
             e_ms = (time.perf_counter() - t0) * 1e3 / e_steps
             nbytes = qh.numel() * 2
             result["e2e"] = {"value": e_ms, "unit": UNIT, "h2d_bytes_per_step": 3 * nbytes, "d2h_bytes_per_step": nbytes,
-                             "steps": e_steps, "api": "saf3r_layer_host (pinned host q/k/v -> device, select + sparse_attn, out -> host; pipelined over 8 head groups)"}
+                             "steps": e_steps, "api": "saf3r_layer_host (pinned host q/k/v -> device, select + sparse_attn, out -> host; pipelined over 9 head groups)"}
 
         if world == 1 and not args.skip_cpu:
             ms, sel, cores, busy, sample = cpu_oracle_layer_ms(layers[0])

@@ -155,7 +155,7 @@ saf3r_status saf3r_dense_attn(saf3r_ctx *ctx, const void *q_dev, const void *k_d
 
 /* End-to-end convenience for HOST buffers (one global-attention layer): copies q/k/v (contiguous [H][N][D] bf16, ideally
  * pinned) to the device scratch, runs select + sparse_attn, copies the bf16 output back to out_host; returns after
- * enqueueing (synchronise `cuda_stream` before reading out_host).  The work is pipelined over up to eight groups of heads
+ * enqueueing (synchronise `cuda_stream` before reading out_host).  The work is pipelined over up to nine groups of heads (the last one a single head, to keep the exposed tail short)
  * on context-owned side streams that are forked from and joined back to `cuda_stream` with events, so that the copies of
  * one group overlap the compute of another; to `cuda_stream` it behaves like one ordered operation.
  * scratch_dev must hold saf3r_layer_host_scratch_bytes(...) bytes; shape strides are ignored (contiguous). */

@@ -930,7 +930,7 @@ saf3r_status saf3r_static_broadcast_attn(saf3r_ctx *ctx, const void *q, const vo
 // saf3r_layer_host pipelines the layer over groups of heads (heads are independent): the host->device copy of
 // group g+1 runs under the select + attention of group g, and the device->host copy of group g under the compute of group
 // g+1 (separate copy engines), on ctx-owned side streams forked from / joined to the caller's stream with events.
-constexpr int kHostGroups = 8, kHostStreams = 3;
+constexpr int kHostGroups = 9, kHostStreams = 3;
 struct HostGroup { int h0, hn; size_t ws, row_ptr, col_idx; int64_t entries; };
 struct HostLayout {
   size_t q, k, v, out, total;
@@ -955,7 +955,10 @@ static HostLayout host_layout(const SelGeom &g, const saf3r_head_cfg *cfg) {
   for (int i = 0; i < l.n_groups; ++i) {
     HostGroup &gr = l.grp[i];
     gr.h0 = h0;
-    gr.hn = (g.H - h0 + (l.n_groups - i) - 1) / (l.n_groups - i);
+    // when there are more heads than groups the LAST group is a single head: what follows the last host->device copy (that
+    // group's select + attention + device->host copy) is exposed, so it is kept as short as the split allows
+    const int tail = g.H > l.n_groups ? 1 : 0;
+    gr.hn = (tail && i == l.n_groups - 1) ? g.H - h0 : (g.H - tail - h0 + (l.n_groups - tail - i) - 1) / (l.n_groups - tail - i);
     h0 += gr.hn;
     const SelGeom sg = sub_geom(g, gr.hn);
     gr.ws = off; off += ws_layout(sg).total;
