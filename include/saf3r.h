@@ -199,6 +199,43 @@ saf3r_status saf3r_token_set_attn(saf3r_ctx *ctx, const void *q_dev, const void 
                                   size_t workspace_bytes, void *out_dev, int out_is_fp32, float *lse_dev_or_null,
                                   void *cuda_stream);
 
+/* ---- saf3r_token_probe_select for callers that must not allocate device memory -------------------------------------------
+ * Who this is for.  Some hosts of this library cannot obtain device memory at the moment they need a result: a plug-in inside
+ * an inference server or engine whose memory planner has already claimed the GPU and hands the plug-in only its input and
+ * output buffers; a process held under a fixed device-memory quota; a latency-critical loop that may not take the device-wide
+ * stall a cudaMalloc / cudaFree implies.  For them every other selection call is unusable, because saf3r_create allocates
+ * (a counter and the key-norm ring) and saf3r_token_probe_select wants a caller-made workspace.
+ *
+ * What it is.  The same three launches as saf3r_token_probe_select (Query-Probe Top-K at token level, PAPER.md:L98, L122-124:
+ * qbar = (1/N) sum_i q_i, p[j] = qbar . k_j / sqrt(D), the K key tokens with the largest p written ascending to idx_dev[h][0..K)),
+ * the same kernels, hence the same idx bit for bit - but it takes no context and no workspace.  Its scratch (partial query
+ * sums, one 32-bit key per (head, token), one histogram per head) lives in a fixed array compiled into the library,
+ * SAF3R_NOALLOC_SCRATCH_BYTES (about 4.6 MiB) of device memory that every GPU which loads libsaf3r.so holds from module load
+ * until the process exits, whether or not this call is ever made.
+ *
+ * Limit.  num_heads * N <= SAF3R_NOALLOC_MAX_KEYS (2^20; e.g. 16 heads x 32 frames x 1374 tokens = 703 488 fits, the 100-frame
+ * configuration does not).  Anything larger is refused with SAF3R_ERR_CAPACITY before a kernel is enqueued; use
+ * saf3r_token_probe_select with your own workspace then.  The other argument rules are those of saf3r_token_probe_select.
+ *
+ * Device and first call.  It works on the CURRENT CUDA device of the calling thread (there is no context to name one); q, k and
+ * idx must live there, and the device must be sm_100 (SAF3R_ERR_UNSUPPORTED otherwise).  The first call on each device looks up
+ * the device address of the built-in array (cudaGetSymbolAddress, which may make the runtime load the library's code onto that
+ * device) and remembers it; later calls only launch.  Make that first call during start-up, before any stream capture begins.
+ * It calls no cudaMalloc / cudaFree / cudaMallocAsync and no library routine that allocates.
+ *
+ * Sharing.  There is ONE array per device and every call uses it.  It keeps whatever the previous call left; the call itself
+ * re-zeroes the part that has to start at zero (the histograms, by its first kernel), so nothing needs clearing between calls.
+ * Two calls of one process whose kernels can run at the same time on one device (different streams, or different host threads)
+ * overwrite each other's scratch and return garbage without any error: keep all calls on a device in one stream order, or order
+ * them with events.  Separate processes each have their own copy and do not interfere.
+ *
+ * Errors.  Returns a saf3r_status; when err_buf != NULL and err_len > 0 a NUL-terminated message is written there on failure
+ * (there is no context to hold it).  Enqueues on cuda_stream and returns; thread-safe on the host side. */
+#define SAF3R_NOALLOC_MAX_KEYS (1 << 20)
+#define SAF3R_NOALLOC_SCRATCH_BYTES (147456 + 4 * SAF3R_NOALLOC_MAX_KEYS + 8192 * SAF3R_MAX_HEADS)
+saf3r_status saf3r_token_probe_select_noalloc(const void *q_dev, const void *k_dev, const saf3r_shape *shape, int32_t K,
+                                              int32_t *idx_dev, void *cuda_stream, char *err_buf, size_t err_len);
+
 /* ---- Token-wise per-frame Top-K: the paper's primary definition of the DINO Top-K kernel (SURVEY 8(f) NEXT-2 iii) ----------------
  * "we pre-compute the cosine similarity between each patch token and all other patch tokens using the DINO features, and select
  * the Top-K most similar tokens from each frame as the keys and values for attention"; the indices are computed

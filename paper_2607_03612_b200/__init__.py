@@ -29,7 +29,8 @@ EXPORTS = ("saf3r_create", "saf3r_destroy", "saf3r_last_error", "saf3r_query_siz
            "saf3r_set_stage_timing", "saf3r_last_select_stage_ms", "saf3r_select_cached", "saf3r_token_stride_attn",
            "saf3r_token_query_sizes", "saf3r_token_probe_select", "saf3r_token_set_attn", "saf3r_check_lists", "saf3r_select_plan", "saf3r_union_lists",
            "saf3r_static_broadcast_workspace_bytes", "saf3r_static_broadcast_attn", "saf3r_token_topk_query_sizes",
-           "saf3r_token_topk_select", "saf3r_token_lists_count", "saf3r_token_lists_fill", "saf3r_token_lists_attn", "saf3r_nmse_accumulate")
+           "saf3r_token_topk_select", "saf3r_token_lists_count", "saf3r_token_lists_fill", "saf3r_token_lists_attn", "saf3r_nmse_accumulate",
+           "saf3r_token_probe_select_noalloc")
 
 
 class Saf3rError(RuntimeError):
@@ -81,6 +82,7 @@ def load_library():
         L.saf3r_token_stride_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.c_int32, C.c_int32, vp, i32, vp, vp]
         L.saf3r_token_query_sizes.argtypes = [C.POINTER(ShapeC), C.c_int32, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         L.saf3r_token_probe_select.argtypes = [vp, vp, vp, C.POINTER(ShapeC), C.c_int32, vp, C.c_size_t, vp, vp]
+        L.saf3r_token_probe_select_noalloc.argtypes = [vp, vp, C.POINTER(ShapeC), C.c_int32, vp, vp, C.c_char_p, C.c_size_t]
         L.saf3r_token_set_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), vp, C.c_int32, vp, C.c_size_t, vp, i32, vp, vp]
         L.saf3r_check_lists.argtypes = [vp, C.POINTER(ShapeC), C.POINTER(ListsC), C.POINTER(i64), vp]
         L.saf3r_sparse_attn.argtypes = [vp, vp, vp, vp, C.POINTER(ShapeC), C.POINTER(ListsC), vp, i32, vp, vp]
@@ -417,6 +419,26 @@ class Context:
                                               arr, scratch.data_ptr(), scratch.numel() * scratch.element_size(),
                                               out_host.data_ptr(), _stream_ptr(stream)))
         return out_host
+
+
+NOALLOC_MAX_KEYS = 1 << 20  # SAF3R_NOALLOC_MAX_KEYS: num_heads * N the built-in scratch of the call below is sized for
+
+
+def token_probe_select_noalloc(q, k, shape: ShapeC, K: int, idx, stream=None):
+    """saf3r_token_probe_select_noalloc: token-level Query-Probe Top-K for hosts that cannot allocate device memory when they
+    call (a plug-in whose engine owns the whole GPU heap, a process under a memory quota, a loop that may not stall on
+    cudaMalloc).  No Context and no workspace: the scratch is a fixed ~4.6 MiB array inside libsaf3r.so, so num_heads * N must
+    stay <= NOALLOC_MAX_KEYS (Saf3rError with status ERR_CAPACITY otherwise).  `idx` is the caller's int32 [H][K] device tensor and
+    receives the same indices Context.token_probe_select returns; q / k / idx must be on the current CUDA device.  All calls on a
+    device share the one array: keep them in one stream order.  The first call per device does a one-off address look-up; make it
+    at start-up.  This wrapper allocates nothing either."""
+    L = load_library()
+    err = C.create_string_buffer(512)
+    st = L.saf3r_token_probe_select_noalloc(q.data_ptr(), k.data_ptr(), C.byref(shape), int(K), idx.data_ptr(), _stream_ptr(stream),
+                                            err, len(err))
+    if st != OK:
+        raise Saf3rError(st, err.value.decode())
+    return idx
 
 
 def token_topk_query_sizes(shape: ShapeC, K: int) -> tuple[int, int, int]:

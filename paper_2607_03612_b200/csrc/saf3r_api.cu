@@ -6,6 +6,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -688,6 +689,92 @@ saf3r_status saf3r_token_probe_select(saf3r_ctx *ctx, const void *q, const void 
   token_topk_kernel<<<g.H, 1024, 0, st>>>(keys, hist1, idx, g.N, K);
   ctx->launches += 3;
   CU_CHECK(cudaGetLastError());
+  return SAF3R_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ allocation-free token probe
+// saf3r_token_probe_select_noalloc (include/saf3r.h): for hosts that cannot get device memory when they call us (a plug-in whose
+// engine has planned all of it, a process under a memory quota, a loop that may not stall on cudaMalloc).  The scratch the three
+// token-probe kernels need is this array, part of the library image on every device that loads it.  Fixed layout, sized for the
+// documented maximum so that it does not depend on the shape of the call:
+//   [0, kNaPartBytes)                      partial query sums, H * ceil(N / kTokChunk) * 64 floats (<= 576 rows of 256 B)
+//   [kNaPartBytes, +4 * MAX_KEYS)          one order-preserving 32-bit key per (head, key token)
+//   [.., + MAX_HEADS * kTokBins1 * 4)      one first-level histogram per head (zeroed by token_qsum_kernel on every call)
+constexpr size_t kNaPartBytes = ((size_t)SAF3R_NOALLOC_MAX_KEYS / kTokChunk + SAF3R_MAX_HEADS) * 64 * sizeof(float);
+constexpr size_t kNaKeysBytes = (size_t)SAF3R_NOALLOC_MAX_KEYS * sizeof(uint32_t);
+constexpr size_t kNaHistBytes = (size_t)SAF3R_MAX_HEADS * kTokBins1 * sizeof(uint32_t);
+static_assert(kNaPartBytes % 256 == 0 && kNaKeysBytes % 256 == 0, "sub-buffers of the built-in scratch must stay 256-byte aligned");
+static_assert(kNaPartBytes + kNaKeysBytes + kNaHistBytes == (size_t)SAF3R_NOALLOC_SCRATCH_BYTES, "saf3r.h states the size of this array");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[SAF3R_NOALLOC_SCRATCH_BYTES];
+
+// In host code `g_noalloc_scratch` is only a handle for the runtime, not an address a kernel can use: the device address differs per
+// GPU and has to be asked for with that GPU current.  Looked up once per device and kept; guarded because there is no context
+// (and so no single-thread rule) on this path.
+constexpr int kNaMaxDevices = 64;
+static std::mutex g_noalloc_mu;
+static unsigned char *g_noalloc_ptr[kNaMaxDevices] = {};
+
+static saf3r_status noalloc_fail(char *err_buf, size_t err_len, saf3r_status st, const std::string &msg) {
+  if (err_buf && err_len) snprintf(err_buf, err_len, "%s", msg.c_str());
+  return st;
+}
+
+static saf3r_status noalloc_scratch(unsigned char **out, char *err_buf, size_t err_len) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return noalloc_fail(err_buf, err_len, SAF3R_ERR_CUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
+  if (dev < 0 || dev >= kNaMaxDevices) return noalloc_fail(err_buf, err_len, SAF3R_ERR_UNSUPPORTED, "device ordinal beyond the per-device table of the built-in scratch");
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[dev]) {  // first call on this device: the set-up the header asks callers to do before any stream capture
+    int major = 0;
+    e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return noalloc_fail(err_buf, err_len, SAF3R_ERR_CUDA, std::string("cudaDeviceGetAttribute: ") + cudaGetErrorString(e));
+    if (major != 10) return noalloc_fail(err_buf, err_len, SAF3R_ERR_UNSUPPORTED, "the current device is not sm_100; this library is sm_100a only and has no CPU fallback");
+    unsigned char *p = nullptr;
+    e = cudaGetSymbolAddress((void **)&p, g_noalloc_scratch);
+    if (e != cudaSuccess || !p)
+      return noalloc_fail(err_buf, err_len, SAF3R_ERR_CUDA, std::string("cudaGetSymbolAddress(built-in scratch): ") + cudaGetErrorString(e));
+    g_noalloc_ptr[dev] = p;
+  }
+  *out = g_noalloc_ptr[dev];
+  return SAF3R_OK;
+}
+
+extern "C" {
+
+saf3r_status saf3r_token_probe_select_noalloc(const void *q, const void *k, const saf3r_shape *shape, int32_t K, int32_t *idx,
+                                              void *stream_, char *err_buf, size_t err_len) {
+  if (err_buf && err_len) err_buf[0] = 0;
+  if (const char *m = validate_shape(shape, true)) return noalloc_fail(err_buf, err_len, SAF3R_ERR_INVALID_ARG, m);
+  if (const char *m = unsupported_shape(shape)) return noalloc_fail(err_buf, err_len, SAF3R_ERR_UNSUPPORTED, m);
+  const SelGeom g = make_geom(shape);
+  if (K < 1 || K > g.N) return noalloc_fail(err_buf, err_len, SAF3R_ERR_INVALID_ARG, "token probe: need 1 <= K <= N");
+  if (!q || !k || !idx) return noalloc_fail(err_buf, err_len, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  if (((uintptr_t)q | (uintptr_t)k) & 15) return noalloc_fail(err_buf, err_len, SAF3R_ERR_INVALID_ARG, "q/k must be 16-byte aligned");
+  if ((int64_t)g.H * g.N > (int64_t)SAF3R_NOALLOC_MAX_KEYS)
+    return noalloc_fail(err_buf, err_len, SAF3R_ERR_CAPACITY,
+                        "num_heads * N = " + std::to_string((int64_t)g.H * g.N) + " exceeds SAF3R_NOALLOC_MAX_KEYS = " +
+                            std::to_string((int64_t)SAF3R_NOALLOC_MAX_KEYS) +
+                            ", the size of the built-in scratch: call saf3r_token_probe_select with a workspace of your own");
+  const int n_chunks = (int)((g.N + kTokChunk - 1) / kTokChunk);
+  if ((size_t)g.H * n_chunks * 64 * sizeof(float) > kNaPartBytes)  // implied by the check above; kept as the layout's own guard
+    return noalloc_fail(err_buf, err_len, SAF3R_ERR_CAPACITY, "partial query sums exceed the built-in scratch");
+  unsigned char *base = nullptr;
+  if (saf3r_status s = noalloc_scratch(&base, err_buf, err_len)) return s;
+  cudaStream_t st = (cudaStream_t)stream_;
+  float *part = (float *)base;
+  uint32_t *keys = (uint32_t *)(base + kNaPartBytes), *hist1 = (uint32_t *)(base + kNaPartBytes + kNaKeysBytes);
+  // Same three launches as saf3r_token_probe_select.  Everything read is written earlier in this very call: `part` by the first
+  // kernel (which also zeroes the H histograms in use), `keys` and the histogram counts by the second; what an earlier call left
+  // behind in the array is never looked at.
+  token_qsum_kernel<<<dim3(n_chunks, g.H), 256, 0, st>>>((const __nv_bfloat16 *)q, part, hist1, g);
+  token_probe_kernel<<<dim3((unsigned)((g.N + kTokTile - 1) / kTokTile), g.H), 256, 0, st>>>((const __nv_bfloat16 *)k, part, keys, hist1,
+                                                                                           g, n_chunks);
+  token_topk_kernel<<<g.H, 1024, 0, st>>>(keys, hist1, idx, g.N, K);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return noalloc_fail(err_buf, err_len, SAF3R_ERR_CUDA, std::string("token probe launch: ") + cudaGetErrorString(e));
   return SAF3R_OK;
 }
 
