@@ -530,9 +530,10 @@ __device__ __forceinline__ uint64_t sel_fma2(uint64_t a, uint64_t b, uint64_t c)
   return d;
 }
 
-// (Qtilde / Ktilde^T were written earlier in the SAME launch by other CTAs.  Reading them through L1 / the read-only path is safe
-// here: no thread of this SM touches a line of head h before the acquire that follows the head's last pool task, L1 is empty of
-// them at kernel start, and the GPU never prefetches into L1 - so the first touch fetches the finished line from L2.)
+// (Qtilde / Ktilde^T were written earlier in the SAME launch by other CTAs, so they are NOT read-only for this kernel: the
+// read-only path (ld.global.nc / __ldg, or const __restrict__ letting the compiler pick it) is undefined for them under the PTX
+// memory model.  They are read with ld.global.cg (__ldcg: L2 only, coherent) after the ld.acquire.gpu + bar.sync that follows the
+// head's last pool task - the same loads probe_score_task uses.)
 // Score rows I0 .. I0+rows-1 (rows <= RT) of head h against every k-block: keys[r][J] = key(Qtilde_{I0+r} . Ktilde_J * cs).
 // Groups of 1024 columns: each thread owns four consecutive columns (one 16-byte load of Ktilde^T per d, coalesced across
 // the warp) and RT rows, 4*RT accumulators as packed row pairs.  The columns left over (< 1024) are spread over all threads
@@ -542,11 +543,11 @@ __device__ __forceinline__ uint64_t sel_fma2(uint64_t a, uint64_t b, uint64_t c)
 // tasks over all threads reading shared memory: one L2 round trip for the tail instead of a latency-bound pass of its own.
 constexpr int kSelTailCols = 128;
 template <int RT>
-__device__ __forceinline__ void score_rows(const float *__restrict__ qt, const float *__restrict__ kt, uint32_t *keys, float *qT,
+__device__ __forceinline__ void score_rows(const float *qt, const float *kt, uint32_t *keys, float *qT,
                                            const SelGeom &g, int h, int I0, int rows, float cs, float *kl) {
   for (int i = threadIdx.x; i < 64 * RT; i += blockDim.x) {
     const int d = i / RT, r = i % RT;
-    qT[i] = r < rows ? qt[((int64_t)h * g.NB + I0 + r) * 64 + d] : 0.f;
+    qT[i] = r < rows ? __ldcg(qt + ((int64_t)h * g.NB + I0 + r) * 64 + d) : 0.f;
   }
   const int64_t ld = kt_stride(g.NB);
   const float *kh = kt + (int64_t)h * 64 * ld;
@@ -575,7 +576,7 @@ __device__ __forceinline__ void score_rows(const float *__restrict__ qt, const f
     for (int d0 = 0; d0 < 64; d0 += KB) {
       float4 kvb[KB];
 #pragma unroll
-      for (int i = 0; i < KB; ++i) kvb[i] = __ldg(reinterpret_cast<const float4 *>(kp + (int64_t)(d0 + i) * ld));
+      for (int i = 0; i < KB; ++i) kvb[i] = __ldcg(reinterpret_cast<const float4 *>(kp + (int64_t)(d0 + i) * ld));
 #pragma unroll
       for (int i = 0; i < KB; ++i) {
         const float4 kv = kvb[i];
@@ -639,7 +640,7 @@ __device__ __forceinline__ void score_rows(const float *__restrict__ qt, const f
     for (int c = 0; c < 4; ++c) a[c][0] = a[c][1] = 0ull;
 #pragma unroll 8
     for (int d = 0; d < 64; ++d) {
-      const float4 kv = __ldg(reinterpret_cast<const float4 *>(kp + (int64_t)d * ld));
+      const float4 kv = __ldcg(reinterpret_cast<const float4 *>(kp + (int64_t)d * ld));
       const float4 t = *reinterpret_cast<const float4 *>(qT + d * RT + 4 * rgp);
       const uint64_t qa = sel_pack2(t.x, t.y), qb = sel_pack2(t.z, t.w);
       const uint64_t k0 = sel_pack2(kv.x, kv.x), k1 = sel_pack2(kv.y, kv.y), k2 = sel_pack2(kv.z, kv.z), k3 = sel_pack2(kv.w, kv.w);
