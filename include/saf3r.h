@@ -255,7 +255,10 @@ saf3r_status saf3r_token_probe_select_noalloc(const void *q_dev, const void *k_d
  *   not fit capacity_tiles is left unwritten.  Both depend only on idx: once per sequence, shared by all heads and layers.
  * saf3r_token_lists_attn: o_i = sum_j softmax_j(q_i.k_j/sqrt(D)) v_j over the keys j of query i's own list: the block-sparse kernel
  *   with K/V rows gathered by index (cp.async) and the bit mask applied before the row max; q, k, v, out, lse as in
- *   saf3r_sparse_attn; the lists are shared by all heads of the call. */
+ *   saf3r_sparse_attn; the lists are shared by all heads of the call.  Requires tile_ptr[NB] <= capacity_tiles (tile_ptr lives on
+ *   the device, so the call cannot check it on the host): a q-tile whose tile range ends beyond capacity_tiles - what a _fill with
+ *   too small a capacity leaves unwritten - is skipped on the device, its rows come out zero with lse = -inf, and nothing is read
+ *   outside key_idx / mask.  key_idx entries outside [0, N) are treated as padding, never dereferenced. */
 typedef struct {
   int64_t *tile_ptr;       /* dev, [NB + 1]: tiles of q-tile I = [tile_ptr[I], tile_ptr[I+1]) */
   int32_t *key_idx;        /* dev, [capacity_tiles * block]: gathered key token of every tile column, -1 = padding */

@@ -45,6 +45,7 @@ struct AttnParams {
   const int64_t *tile_ptr;
   const int32_t *key_idx;
   const uint32_t *mask;  // [tile][B rows][B/32 words]
+  int64_t capacity_tiles;  // tiles key_idx / mask hold: a q-tile whose range ends beyond it (a short-capacity _fill left it unwritten) is skipped
   const __nv_bfloat16 *k_base, *v_base;
   int64_t kv_stride_head, kv_stride_token;
 };
@@ -296,15 +297,16 @@ __device__ __forceinline__ void softmax_half(const AttnParams &p, uint8_t *smem,
 // when every lane's copies have landed.
 template <int B>
 __device__ __forceinline__ void gather_tile(const __nv_bfloat16 *__restrict__ base, int64_t stride_token, const int32_t *__restrict__ idx,
-                                            uint32_t stage, uint32_t bar_full) {
+                                            int32_t n_kv, uint32_t stage, uint32_t bar_full) {
   const int lane = threadIdx.x & 31, ch = lane & 7, rr = lane >> 3;
 #pragma unroll 8
   for (int it = 0; it < B / 4; ++it) {
     const int row = it * 4 + rr;
     const int j = __ldg(idx + row);
     const uint32_t dst = stage + row * 128 + ((ch ^ (row & 7)) << 4);
-    const __nv_bfloat16 *src = base + (int64_t)(j < 0 ? 0 : j) * stride_token + ch * 8;
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(j < 0 ? 0 : 16) : "memory");
+    const bool pad = j < 0 || j >= n_kv;  // -1 = padding; an index beyond the key tokens (a malformed caller-made list) is never dereferenced
+    const __nv_bfloat16 *src = base + (int64_t)(pad ? 0 : j) * stride_token + ch * 8;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(pad ? 0 : 16) : "memory");
   }
   asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar_full) : "memory");
 }
@@ -338,7 +340,8 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
   int n_ent = p.NB_kv;
   if (kTok) {
     e0 = p.tile_ptr[I];
-    n_ent = (int)(p.tile_ptr[I + 1] - e0);
+    const int64_t e1 = p.tile_ptr[I + 1];
+    n_ent = (e0 < 0 || e1 < e0 || e1 > p.capacity_tiles) ? 0 : (int)(e1 - e0);  // out of the buffers: zero rows, lse = -inf
   } else if (p.row_ptr != nullptr) {
     const int64_t r = (int64_t)h * p.NB + I;
     e0 = p.row_ptr[r];
@@ -390,7 +393,7 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
           int sk = 0, phk = 0;
           for (int e = 0; e < n_ent; ++e) {
             mbar_wait_relaxed<kSleepTma>(bar_k_empty + 8 * sk, phk ^ 1);
-            gather_tile<B>(kb, p.kv_stride_token, p.key_idx + (e0 + e) * B, sbase + L::kK + sk * B * 128, bar_k_full + 8 * sk);
+            gather_tile<B>(kb, p.kv_stride_token, p.key_idx + (e0 + e) * B, p.N_kv, sbase + L::kK + sk * B * 128, bar_k_full + 8 * sk);
             if (++sk == kKStages) { sk = 0; phk ^= 1; }
           }
         } else {
@@ -422,7 +425,7 @@ saf3r_attn_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_consta
       int sv = 0, phv = 0;
       for (int e = 0; e < n_ent; ++e) {
         mbar_wait_relaxed<kSleepTma>(bar_v_empty + 8 * sv, phv ^ 1);
-        gather_tile<B>(vb, p.kv_stride_token, p.key_idx + (e0 + e) * B, sbase + L::kV + sv * B * 128, bar_v_full + 8 * sv);
+        gather_tile<B>(vb, p.kv_stride_token, p.key_idx + (e0 + e) * B, p.N_kv, sbase + L::kV + sv * B * 128, bar_v_full + 8 * sv);
         if (++sv == kVStages) { sv = 0; phv ^= 1; }
       }
     } else if (warp == 9) {

@@ -929,6 +929,7 @@ saf3r_status saf3r_token_lists_attn(saf3r_ctx *ctx, const void *q, const void *k
   if (const char *m = unsupported_shape(shape)) return fail(ctx, SAF3R_ERR_UNSUPPORTED, m);
   if (!q || !k || !v || !out || !lists || !lists->tile_ptr || !lists->key_idx || !lists->mask)
     return fail(ctx, SAF3R_ERR_INVALID_ARG, "null pointer argument");
+  if (lists->capacity_tiles < 0) return fail(ctx, SAF3R_ERR_INVALID_ARG, "token lists: capacity_tiles must be >= 0");
   if (((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) return fail(ctx, SAF3R_ERR_INVALID_ARG, "q/k/v/out must be 16-byte aligned");
   const SelGeom g = make_geom(shape);
   CUtensorMap mq;
@@ -942,7 +943,7 @@ saf3r_status saf3r_token_lists_attn(saf3r_ctx *ctx, const void *q, const void *k
   p.out_fp32 = out_is_fp32 ? 1 : 0;
   p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)shape->head_dim));
   p.head_order = nullptr;
-  p.tile_ptr = lists->tile_ptr; p.key_idx = lists->key_idx; p.mask = lists->mask;
+  p.tile_ptr = lists->tile_ptr; p.key_idx = lists->key_idx; p.mask = lists->mask; p.capacity_tiles = lists->capacity_tiles;
   p.k_base = (const __nv_bfloat16 *)k; p.v_base = (const __nv_bfloat16 *)v;
   p.kv_stride_head = g.stride_head; p.kv_stride_token = g.stride_token;
   cudaStream_t st = (cudaStream_t)stream_;

@@ -925,3 +925,49 @@ def test_token_topk_per_frame_at_c2_size_sampled(env):
             i1 = min(sh.N, i0 + 128)
             ref, _ = orc.attn_token_lists(L.q[h], L.k[h], L.v[h], gi[i0:i1].reshape(i1 - i0, -1), i0, i1)
             check_attention(out[h].cpu().numpy(), ref, f"tokenwise-C2 head {h} ({gens[h]})")
+
+
+def test_token_lists_attn_short_capacity_and_bad_indices_stay_in_bounds(env):
+    """include/saf3r.h, saf3r_token_lists_attn: a q-tile whose tile range ends beyond capacity_tiles (what a short-capacity _fill
+    leaves unwritten) is skipped - zero rows, lse = -inf - while the q-tiles that fit are unchanged; a key index outside [0, N) is
+    padding (same output as -1), never dereferenced."""
+    sf, ctx, torch = env
+    H, B, K = 2, 64, 3
+    L = small_layer(4, 16, H, B, [sy.GEN_SAME_POSITION, sy.GEN_UNIFORM], [sy.cfg(type=sy.HEAD_DENSE)] * H, seed=141)
+    sh = L.shape
+    shape = c_shape(sf, sh)
+    idx = ctx.token_topk_select(to_dev(sy.make_features(sh, seed=142)), shape, K)
+    lists = ctx.token_lists_build(shape, idx)
+    q, k, v = upload(L)
+    full, full_lse = ctx.token_lists_attn(q, k, v, shape, lists, out_fp32=True, want_lse=True)
+    torch.cuda.synchronize()
+    tp = lists.tile_ptr.cpu().numpy()
+    cut = sh.NB // 2                                              # q-tiles [0, cut) fit, the rest do not
+    cap = int(tp[cut]) + 1                                        # one tile short of q-tile `cut` unless it has a single tile ...
+    while cut < sh.NB and tp[cut + 1] <= cap:                      # ... in which case it fits too
+        cut += 1
+    assert 0 < cut < sh.NB
+    short = sf.TokenLists(lists.tile_ptr, lists.key_idx[:cap * B].clone(), lists.mask[:cap].clone(), cap)
+    out, lse = ctx.token_lists_attn(q, k, v, shape, short, out_fp32=True, want_lse=True)
+    torch.cuda.synchronize()
+    t_fit = [I for I in range(sh.NB) if tp[I + 1] <= cap]
+    t_cut = [I for I in range(sh.NB) if tp[I + 1] > cap]
+    assert t_fit and t_cut
+    for I in t_fit:
+        assert torch.equal(out[:, I * B:(I + 1) * B], full[:, I * B:(I + 1) * B])
+        assert torch.equal(lse[:, I * B:(I + 1) * B], full_lse[:, I * B:(I + 1) * B])
+    for I in t_cut:
+        assert int((out[:, I * B:(I + 1) * B] != 0).sum()) == 0
+        assert bool(torch.isinf(lse[:, I * B:(I + 1) * B]).all()) and float(lse[:, I * B:(I + 1) * B].max()) < 0
+    # an index beyond the key tokens behaves like padding (its mask bits cleared so that both runs keep the same keys)
+    kidx = lists.key_idx.clone()
+    mask = lists.mask.clone()
+    col = int((kidx[:B] >= 0).nonzero()[0])                        # a real key of tile 0
+    mask[0, :, col // 32] &= ~(1 << (col % 32)) if col % 32 != 31 else 0x7FFFFFFF
+    a_idx, b_idx = kidx.clone(), kidx.clone()
+    a_idx[col] = -1
+    b_idx[col] = sh.N + 12345
+    oa = ctx.token_lists_attn(q, k, v, shape, sf.TokenLists(lists.tile_ptr, a_idx, mask, lists.tiles), out_fp32=True)
+    ob = ctx.token_lists_attn(q, k, v, shape, sf.TokenLists(lists.tile_ptr, b_idx, mask, lists.tiles), out_fp32=True)
+    torch.cuda.synchronize()
+    assert torch.equal(oa, ob) and not bool(torch.isnan(ob).any())
