@@ -16,9 +16,10 @@
  *
  * Citations are PAPER.md line numbers and DESIGN.md readings.
  *
- * Parity pins: every function below is pinned by tests/test_oracle_pins.py (P1..P19 of
+ * Parity pins: every function below is pinned by tests/test_oracle_pins.py (P1..P20 of
  * DESIGN.md; P14-P16 pin orc_attn_tokens / orc_token_probe, P17 orc_union_lists, P18 orc_attn_broadcast_frame0,
- * P19 orc_token_topk_per_frame / orc_token_cosine_row / orc_attn_token_lists).  Unpinned *choices* (not arithmetic): POSITION_BAND radius and the
+ * P19 orc_token_topk_per_frame / orc_token_cosine_row / orc_attn_token_lists; P20 the kept set of the GLOBAL top-n and probe
+ * rules of select_row, P4 the floor form of the fractional stride).  Unpinned *choices* (not arithmetic): POSITION_BAND radius and the
  * DOT-vs-COSINE default for correspondence heads -- "parity unpinned" for those choices.
  */
 #include <math.h>

@@ -138,6 +138,16 @@ def test_p4_uniform_stride_closed_form():
         row = hl.col_idx[hl.row_ptr[0]:hl.row_ptr[1]]
         assert len(row) == n and row[0] == 0 and np.all(np.diff(row) > 0)
         assert np.array_equal(hl.col_idx, np.tile(row, NB))
+    # keep_blocks form when n does not divide NB: block i of the n kept ones is floor(i * NB / n) (reading A1; a ceiling or a
+    # rounding would pass every check above).  NB = 37 is prime, so no n in 2..36 divides it.
+    S3, T3 = 4, 37          # N = 148, B = 4 -> NB = 37
+    q3, k3 = rand_bits(rng, (148, D)), rand_bits(rng, (148, D))
+    for n in (2, 5, 7, 19, 36):
+        hl = orc.select_head(q3, k3, S3, T3, 4, ocfg(sy.cfg(type=sy.HEAD_UNIFORM_STRIDE, stride=0, keep_blocks=n)))
+        expect = np.floor(np.arange(n) * 37 / n).astype(np.int32)
+        assert len(set(expect.tolist())) == n
+        for I in range(37):
+            assert np.array_equal(hl.col_idx[hl.row_ptr[I]:hl.row_ptr[I + 1]], expect), f"keep_blocks={n} row {I}"
     # keep_blocks form equals the stride set when s | NB
     S2, T2 = 4, 24          # N = 96, B = 4 -> NB = 24
     q2, k2 = rand_bits(rng, (96, D)), rand_bits(rng, (96, D))
@@ -646,3 +656,69 @@ def test_p19_token_topk_per_frame_and_per_query_attention():
     assert np.abs(o4 - o5).max() <= 1e-6 and np.abs(l4 - l5).max() <= 1e-5
     o6, l6 = orc.attn_token_lists(q, k, v, np.full((N, 4), -1, np.int32))
     assert np.all(o6 == 0) and np.all(np.isneginf(l6))
+
+
+# ---------------------------------------------------------------- P20
+@pytest.mark.parametrize("mode", ["dot", "cosine", "probe"])
+def test_p20_global_topn_kept_set_is_the_argsort_of_the_mean_token_pair_scores(mode):
+    """PAPER.md:L126 (block-wise similarity Top-K), L98/L124 (query probe): the kept set of row I of a BLOCK_TOPK / GLOBAL head is
+    the n largest of that row's block scores, ties to the lower index, written ascending - checked against numpy on the
+    mean-of-token-pair matrix built here from the tokens (what P7 pins the scores to), never on the oracle's own scores.  A cut one
+    short or one long (n - 1, n + 1), a ranking of a neighbouring row, or a descending / unsorted list fails this.  The oracle
+    ranks the fp32 it stores, so the expected scores are rounded to fp32 before ranking."""
+    cosine, probe = mode == "cosine", mode == "probe"
+    rng = np.random.default_rng(200 + int(cosine))
+    S, T, B, D = 3, 23, 8, 8          # N = 69, NB = 9, tail block of 5 tokens
+    N = S * T
+    NB = (N + B - 1) // B
+    q, k = rand_bits(rng, (N, D), 1.2), rand_bits(rng, (N, D), 1.2)
+    qf, kf = sy.bf16_bits_to_f32(q).astype(np.float64), sy.bf16_bits_to_f32(k).astype(np.float64)
+    if cosine:
+        tok = (qf / np.linalg.norm(qf, axis=1, keepdims=True)) @ (kf / np.linalg.norm(kf, axis=1, keepdims=True)).T
+    else:
+        tok = qf @ kf.T / np.sqrt(D)
+    if probe:    # one row for every I: the mean over ALL queries and the keys of block J
+        E = np.array([[tok[:, J * B:(J + 1) * B].mean() for J in range(NB)]] * NB)
+    else:
+        E = np.array([[tok[I * B:(I + 1) * B, J * B:(J + 1) * B].mean() for J in range(NB)] for I in range(NB)])
+    E32 = E.astype(np.float32)
+    gaps = np.diff(np.sort(E32, axis=1), axis=1).min()
+    assert gaps > 1e-5, "the seeded scores must be tie-free for this pin to be unambiguous"
+    assert len({tuple(np.argsort(-E32[I], kind="stable")[:2]) for I in range(NB)}) > 1 or probe   # rows really differ
+    for n in (1, 2, NB // 2, NB - 1, NB):
+        if probe:
+            c = sy.cfg(type=sy.HEAD_QUERY_PROBE_TOPK, keep_blocks=n)
+        else:
+            c = sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=n,
+                       score_mode=sy.SCORE_COSINE if cosine else sy.SCORE_DOT)
+        hl = orc.select_head(q, k, S, T, B, ocfg(c))
+        assert np.array_equal(hl.row_ptr, np.arange(NB + 1, dtype=np.int64) * n)
+        for I in range(NB):
+            expect = np.sort(np.argsort(-E32[I], kind="stable")[:n]).astype(np.int32)
+            assert np.array_equal(hl.col_idx[hl.row_ptr[I]:hl.row_ptr[I + 1]], expect), f"n={n} row {I}"
+
+
+def test_p20_global_topn_breaks_exact_ties_towards_the_lower_index():
+    """The total order of include/saf3r.h (score descending, then index ascending) at the level of select_head: two k-blocks made
+    of identical tokens have bit-identical scores in every row; when the cut falls between them the lower index is kept."""
+    rng = np.random.default_rng(210)
+    S, T, B, D = 4, 16, 8, 8          # N = 64, NB = 8, no tail
+    N, NB = S * T, 8
+    q, k = rand_bits(rng, (N, D), 1.2), rand_bits(rng, (N, D), 1.2)
+    k[5 * B:6 * B] = k[2 * B:3 * B]   # block 5 == block 2
+    kf = sy.bf16_bits_to_f32(k).astype(np.float64)
+    qf = sy.bf16_bits_to_f32(q).astype(np.float64)
+    E = np.array([[(qf[I * B:(I + 1) * B] @ kf[J * B:(J + 1) * B].T).mean() for J in range(NB)] for I in range(NB)]) / np.sqrt(D)
+    for n in range(1, NB + 1):
+        hl = orc.select_head(q, k, S, T, B, ocfg(sy.cfg(type=sy.HEAD_BLOCK_TOPK, topk_scope=sy.SCOPE_GLOBAL, keep_blocks=n)))
+        for I in range(NB):
+            row = hl.col_idx[hl.row_ptr[I]:hl.row_ptr[I + 1]].tolist()
+            rank = np.argsort(-E[I].astype(np.float32), kind="stable")
+            others = [J for J in rank if J not in (2, 5)]
+            pos2 = int(np.sum(E[I][others] > E[I][2]))              # blocks strictly ahead of the tied pair
+            if n == pos2 + 1:
+                assert 2 in row and 5 not in row, f"n={n} row {I}: the cut splits the tie, block 2 must win"
+            elif n >= pos2 + 2:
+                assert 2 in row and 5 in row
+            else:
+                assert 2 not in row and 5 not in row
