@@ -274,12 +274,15 @@ def test_c2_dense_sampled_rows(env):
 
 
 # ------------------------------------------------------------------------------------------------ C3 (metric point), full size
-def test_c3_full_size_lists_and_sampled_attention(env):
-    """BASELINE.json's metric configuration (S=100, N=137400, NB=1074) in the launch configuration bench.py times:
-    lists of all 16 heads against the oracle (near-tie rule), attention on sampled q-blocks per head evaluated by the
-    oracle on the GPU's own lists (protocol iii), bf16 output path included."""
+@pytest.mark.parametrize("layer", [0, 1, 2, 3])
+def test_c3_full_size_lists_and_sampled_attention(env, layer):
+    """BASELINE.json's metric configuration (S=100, N=137400, NB=1074) in the launch configuration bench.py times, for each of
+    the four seeded layers bench.py keeps resident and rotates through: lists of all 16 heads against the oracle (near-tie rule),
+    attention on sampled q-blocks per head evaluated by the oracle on the GPU's own lists (protocol iii).  The bf16 output path -
+    the one bench.py times - is bounded too: the store rounds to 8 bits of mantissa, |o| <= max|v| ~ 4 gives 2^-9 * 4 ~ 8e-3 on
+    top of the fp32 path's 1e-2, hence max-abs 3e-2 (unchanged) and mean-abs 2e-3 (as test_layer_host_sixteen_*)."""
     sf, ctx, torch = env
-    L = sy.config_c3_layer(0)
+    L = sy.config_c3_layer(layer)
     sh = L.shape
     q, k, v = upload(L)
     shape = c_shape(sf, sh)
@@ -289,17 +292,21 @@ def test_c3_full_size_lists_and_sampled_attention(env):
     torch.cuda.synchronize()
     hls = oracle_lists(L)
     rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
-    stats = compare_lists(L, rp, col, hls, tag="C3 layer 0 (16 heads, full size)")
-    print("C3 near-ties:", stats)
+    stats = compare_lists(L, rp, col, hls, tag=f"C3 layer {layer} (16 heads, full size)")
+    print(f"C3 layer {layer} near-ties:", stats)
     assert stats["tie_floored"] <= 1e-3 * stats["entries"]
-    rng = np.random.default_rng(3)
+    rng = np.random.default_rng(3 + layer)
+    worst_bf = [0.0, 0.0]
     for h in range(sh.H):
-        qb = np.unique(np.concatenate([rng.choice(sh.NB, 1, replace=False), [sh.NB - 1]])).astype(np.int64)
+        qb = np.unique(np.concatenate([rng.choice(sh.NB - 1, 1, replace=False), [sh.NB - 1]])).astype(np.int64)
         r = rp[h * sh.NB:(h + 1) * sh.NB + 1]
         ref, _ = orc.attn_lists(L.q[h], L.k[h], L.v[h], sh.B, r - r[0], col[r[0]:r[-1]], qb, want_lse=False)
-        check_attention(out[h].cpu().numpy(), ref, f"C3 head {h} ({L.gens[h]})")
+        check_attention(out[h].cpu().numpy(), ref, f"C3 layer {layer} head {h} ({L.gens[h]})", tag=f"C3 layer {layer}")
         m = ~np.isnan(ref)
-        assert np.abs(out_bf[h].float().cpu().numpy()[m] - ref[m]).max() <= 3e-2    # bf16 store adds its own rounding
+        d = np.abs(out_bf[h].float().cpu().numpy()[m].astype(np.float64) - ref[m])
+        worst_bf = [max(worst_bf[0], float(d.max())), max(worst_bf[1], float(d.mean()))]
+        assert d.max() <= 3e-2 and d.mean() <= 2e-3, f"bf16 output, layer {layer} head {h}: max-abs {d.max():.3e}, mean-abs {d.mean():.3e}"
+    print(f"C3 layer {layer} bf16 output: worst max-abs {worst_bf[0]:.3e} (bound 3e-2), worst mean-abs {worst_bf[1]:.3e} (bound 2e-3)")
 
 
 # ------------------------------------------------------------------------------------------------ top-n edge cases
