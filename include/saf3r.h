@@ -21,6 +21,12 @@
  *   - Errors: every call returns a saf3r_status; text via saf3r_last_error(ctx).  SAF3R_ERR_CUDA is sticky.
  *   - A context is not thread-safe: use one context per host thread (or serialise calls).  Calls on one context may target
  *     different streams one after another; saf3r_layer_host additionally uses context-owned side streams.
+ *   - Attention calls in flight per context: every *_attn call takes the next of 256 context-owned slots (per-head key-norm
+ *     bounds and the head order its kernel reads) and the slot is reused, without any wait, 256 attention calls later.  Keep
+ *     fewer than 256 attention calls of one context unfinished at a time.  A CUDA graph captured from such calls (e.g. the stack
+ *     of paper_2607_03612_b200/stack.py) has its slots baked in: while a replay of it may be running, do not issue 256 or more
+ *     eager attention calls on the same context from another stream (they would wrap the ring and overwrite the replay's slots,
+ *     which can freeze the running max too early and yield inf/NaN) - use a second context for that stream.
  *   - There is no CPU fallback: on a machine without an sm_100 device saf3r_create fails with SAF3R_ERR_UNSUPPORTED.
  */
 #ifndef SAF3R_H_

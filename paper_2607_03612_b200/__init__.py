@@ -152,9 +152,15 @@ def _stream_ptr(stream=None):
 
 
 def _on_stream(stream, *tensors):
-    """Tensors this binding allocated itself and that kernels enqueued on `stream` touch: tell the caching allocator, so that a
-    block dropped by the caller is not handed to another stream's allocation while those kernels still run."""
+    """Tensors this binding allocated itself (on torch's CURRENT stream) and that kernels enqueued on `stream` touch.  Two hazards
+    of the caching allocator when `stream` is not the current stream: (1) the block may have been recycled from a tensor that
+    kernels already queued on the current stream still use - so `stream` first waits for the current stream's work queued so far;
+    (2) the block may be handed to another allocation while kernels on `stream` still run - so the tensors are recorded on it."""
     if stream is not None:
+        import torch
+        cur = torch.cuda.current_stream()
+        if stream != cur:
+            stream.wait_stream(cur)
         for t in tensors:
             if t is not None:
                 t.record_stream(stream)
@@ -383,9 +389,10 @@ class Context:
         assert o_full.dtype == o_sparse.dtype
         self._check(self.lib.saf3r_nmse_accumulate(self.h, o_full.data_ptr(), o_sparse.data_ptr(), C.byref(shape),
                                                    int(o_full.dtype == torch.float32), acc.data_ptr(), _stream_ptr(stream)))
+        (stream or torch.cuda.current_stream()).synchronize()   # the copy below runs on the current stream, the kernel on `stream`
         a = acc.cpu().tolist()
         H = shape.num_heads
-        return [a[h] / a[H + h] for h in range(H)]
+        return [a[h] / a[H + h] if a[H + h] > 0 else float("nan") for h in range(H)]   # ||O_full|| = 0: Eq. 1 is undefined
 
     # ---- saf3r_static_broadcast_attn
     def static_broadcast_attn(self, q, k, v, shape: ShapeC, workspace=None, out=None, out_fp32=False, want_lse=False, stream=None):

@@ -978,3 +978,35 @@ def test_token_lists_attn_short_capacity_and_bad_indices_stay_in_bounds(env):
     ob = ctx.token_lists_attn(q, k, v, shape, sf.TokenLists(lists.tile_ptr, b_idx, mask, lists.tiles), out_fp32=True)
     torch.cuda.synchronize()
     assert torch.equal(oa, ob) and not bool(torch.isnan(ob).any())
+
+
+def test_binding_on_a_side_stream_matches_the_current_stream(env):
+    """The binding's own allocations (lists, outputs, the NMSE accumulators) when `stream` is not torch's current stream: same
+    results as on the current stream, nmse() reads its sums only after `stream` has finished, and a head whose O_full is all zero
+    reports nan (Eq. 1 is 0/0 there) instead of raising."""
+    sf, ctx, torch = env
+    L = sy.config_c1()
+    sh = L.shape
+    q, k, v = upload(L)
+    shape = c_shape(sf, sh)
+    lists0 = ctx.select(q, k, shape, L.cfgs)
+    out0 = ctx.sparse_attn(q, k, v, shape, lists0, out_fp32=True)
+    full0 = ctx.dense_attn(q, k, v, shape, out_fp32=True)
+    nm0 = ctx.nmse(full0, out0, shape)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    for _ in range(3):                                            # a few rounds so that the allocator recycles blocks
+        junk = torch.randn(1 << 20, device="cuda:0")              # current-stream work whose block is freed right away
+        junk = junk * 2
+        del junk
+        lists1 = ctx.select(q, k, shape, L.cfgs, stream=side)
+        out1 = ctx.sparse_attn(q, k, v, shape, lists1, out_fp32=True, stream=side)
+        full1 = ctx.dense_attn(q, k, v, shape, out_fp32=True, stream=side)
+        nm1 = ctx.nmse(full1, out1, shape, stream=side)
+        side.synchronize()
+        assert torch.equal(lists1.row_ptr, lists0.row_ptr) and torch.equal(lists1.col_idx, lists0.col_idx)
+        assert torch.equal(out1, out0) and torch.equal(full1, full0)
+        assert nm1 == nm0
+    zero = torch.zeros_like(full0)
+    nz = ctx.nmse(zero, out0, shape, stream=side)
+    assert all(np.isnan(x) for x in nz)
