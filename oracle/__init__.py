@@ -31,7 +31,15 @@ class OrcHeadCfg(C.Structure):
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (plain C, -O2, OpenMP across independent rows only)."""
+    """Compile the oracle with gcc (plain C, -O2, OpenMP across independent rows only).  With SAF3R_ORACLE_SANITIZE=1 in the
+    environment a second library is built with AddressSanitizer + UndefinedBehaviorSanitizer (-O1 -g, same source) and loaded
+    instead; the process must then run with LD_PRELOAD=$(gcc -print-file-name=libasan.so) (profiles/r3_oracle_sanitizers.md)."""
+    if os.environ.get("SAF3R_ORACLE_SANITIZE") == "1":
+        out = os.path.join(_HERE, "libsaf3r_oracle_san.so")
+        if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(_SRC):
+            subprocess.check_call(["gcc", "-O1", "-g", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-fsanitize=address,undefined",
+                                   "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer", "-o", out, _SRC, "-lm"])
+        return out
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         subprocess.check_call(["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"])
     return _LIB

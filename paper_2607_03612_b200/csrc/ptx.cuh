@@ -271,22 +271,6 @@ __device__ __forceinline__ uint64_t add_f32x2(uint64_t a, uint64_t b) {
   asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
   return d;
 }
-__device__ __forceinline__ uint64_t mul_f32x2(uint64_t a, uint64_t b) {
-  uint64_t d;
-  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-  return d;
-}
-// acc += lo half (bf16) and acc2 += hi half (bf16) of a packed pair, in fp32 (sm_100 mixed-precision add: FHADD.BF16 reads the
-// half straight out of the packed register).  Used to sum the ROUNDED softmax weights: the row sum then matches what the PV
-// tensor-core product sees bit for bit, so the bf16 rounding of P perturbs o = sum(P v) / sum(P) only through (v_j - o), not v_j.
-__device__ __forceinline__ void add_bf16x2_to_f32(uint32_t pk, float &acc_lo, float &acc_hi) {
-  asm("{\n\t.reg .b16 lo, hi;\n\t"
-      "mov.b32 {lo, hi}, %2;\n\t"
-      "add.rn.f32.bf16 %0, lo, %0;\n\t"
-      "add.rn.f32.bf16 %1, hi, %1;\n\t}"
-      : "+f"(acc_lo), "+f"(acc_hi)
-      : "r"(pk));
-}
 __device__ __forceinline__ float max3(float a, float b, float c) {
   float d;
   asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
