@@ -669,6 +669,104 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_head_parallel(args):
+    """SURVEY 8(e), head-parallel split of ONE layer (strong scaling): the heads of C3 layer 0 are assigned to the N ranks by
+    sharding.assign_heads (longest-processing-time first on the closed-form executed FLOP per head, "for each head
+    h"); every rank holds only its heads' Q/K/V and runs select + sparse_attn on them.  No collective in the data path (an
+    all-gather of O only if the consumer wants every head everywhere - not part of this path); the time of the layer is the MAX
+    over ranks of the device time.  One JSON line, "scaling": "strong".  At N = 1 it is the whole layer on one GPU."""
+    import torch
+    import torch.distributed as dist
+    import paper_2607_03612_b200 as sf
+    from paper_2607_03612_b200 import sharding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+    clocklog = ClockLog(local)
+    peaks = load_peaks()
+    sh = shape_for(args.config)
+    L = make_layers(args.config, 1, args.gen, args.ratio)[0]
+    full_shape = sf.make_shape(sh.S, sh.T, sh.H, sh.D, sh.B)
+    costs = sharding.head_costs(full_shape, L.cfgs)              # closed form: every rank computes the same split, no communication
+    parts = sharding.assign_heads(costs, world)
+    mine = parts[rank]
+    loads = [sum(costs[h] for h in p) for p in parts]
+    ctx = sf.Context(local)
+    stream = torch.cuda.current_stream()
+    total_ms = 0.0
+    launches = 0
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    step = None
+    if mine:
+        up = lambda x: torch.from_numpy(np.ascontiguousarray(x[mine]).view(np.int16)).to(dev).view(torch.bfloat16)
+        q, k, v = up(L.q), up(L.k), up(L.v)
+        cfgs = [L.cfgs[h] for h in mine]
+        shape = sf.make_shape(sh.S, sh.T, len(mine), sh.D, sh.B)
+        entries, ws_bytes = sf.query_sizes(shape, cfgs)
+        lists = sf.Lists(torch.empty(len(mine) * sh.NB + 1, dtype=torch.int64, device=dev), torch.empty(max(entries, 1), dtype=torch.int32, device=dev))
+        ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+        out = torch.empty_like(q)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # one resident layer: flush the 126 MB L2 between steps
+
+        def step():
+            flush.zero_()
+            ctx.select(q, k, shape, cfgs, workspace=ws, lists=lists)
+            ctx.sparse_attn(q, k, v, shape, lists, out=out)
+    for _ in range(args.warmup):
+        if step:
+            step()
+    barrier()
+    l0 = ctx.launch_count()
+    with clocklog.region() as clk:
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            if step:
+                step()
+        e1.record(stream)
+        barrier()
+    launches = ctx.launch_count() - l0
+    mine_ms = e0.elapsed_time(e1)
+    if step:                                                      # the flush is not part of the layer: time it alone and subtract
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record(stream)
+        for _ in range(args.steps):
+            flush.zero_()
+        f1.record(stream)
+        torch.cuda.synchronize()
+        mine_ms -= f0.elapsed_time(f1)
+    total_ms = sharding.max_over_ranks(mine_ms, dev)
+    if rank == 0:
+        ms = total_ms / args.steps
+        print(json.dumps({
+            "metric": METRIC, "value": ms, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+            "higher_is_better": False, "scaling": "strong", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": workload_name(args.config, sh, args.gen, args.ratio), "parallelism": f"head-parallel x{world} (LPT by executed FLOP)",
+                       "l2": "one resident layer per rank, 256 MB L2 flush between timed steps (its time measured alone and subtracted)"},
+            "gpu_launches": int(launches), "heads_by_rank": parts, "executed_flop_by_rank": loads,
+            "lpt_imbalance_max_over_mean": (max(loads) / (sum(loads) / world)) if sum(loads) else None,
+            "executed_tflops_whole_job": sum(loads) / (ms * 1e-3) / 1e12,
+            "roofline": {"bound": "tensor", "achieved": max(loads) / (ms * 1e-3) / 1e12, "peak": peaks["tflops_sustained"], "unit": "TFLOP/s",
+                         "frac": max(loads) / (ms * 1e-3) / 1e12 / peaks["tflops_sustained"], "traffic": None,
+                         "note": "the slowest rank's executed FLOP over the max-over-ranks layer time (includes its select)"},
+            "clocks": clk.summary(),
+            "note": "no data-path collective; the only communication is the barrier and the MAX all-reduce of the timing"}))
+    clocklog.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_stack(args):
     """the whole global-attention stack (default 24 layers) with the per-sequence index
     cache and as one CUDA graph.  Prints one JSON line (an extra, not the contract line)."""
@@ -892,6 +990,8 @@ def main():
     ap.add_argument("--skip-s500", action="store_true", help="skip the bounded 500-frame (C5) point of the default run")
     ap.add_argument("--skip-configs", action="store_true", help="skip the C2 point and the C4 sweep of the default run (`configs` key)")
     ap.add_argument("--skip-profiled", action="store_true", help="skip the C3 point with budgets chosen by the offline search")
+    ap.add_argument("--shard", default="layers", choices=["layers", "heads"],
+                    help="N ranks: independent layers per rank (weak scaling, default) or the heads of ONE layer split over the ranks (strong)")
     ap.add_argument("--stack", action="store_true", help="time the whole stack with the index cache and as one CUDA graph")
     ap.add_argument("--layers", type=int, default=24)
     ap.add_argument("--token", action="store_true", help="time the token-granular variants (NEXT-2) on one layer")
@@ -909,6 +1009,8 @@ def main():
         run_stack(args)
     elif args.impl == "reference":
         run_reference(args)
+    elif args.shard == "heads":
+        run_head_parallel(args)
     else:
         run_ours(args)
 

@@ -1006,7 +1006,58 @@ def test_binding_on_a_side_stream_matches_the_current_stream(env):
         side.synchronize()
         assert torch.equal(lists1.row_ptr, lists0.row_ptr) and torch.equal(lists1.col_idx, lists0.col_idx)
         assert torch.equal(out1, out0) and torch.equal(full1, full0)
-        assert nm1 == nm0
+        assert np.allclose(nm1, nm0, rtol=1e-12, atol=0)       # double atomics: the order of the adds is free, the sums agree to rounding
     zero = torch.zeros_like(full0)
     nz = ctx.nmse(zero, out0, shape, stream=side)
     assert all(np.isnan(x) for x in nz)
+
+
+def test_head_parallel_split_equals_the_whole_layer(env):
+    """the head-parallel split bench.py --shard heads runs (sharding.assign_heads over the closed-form FLOP per head,
+    every rank with only its heads' Q/K/V) gives, head by head, the bits of the whole-layer call: lists and outputs of the
+    sub-layers of a 2-way and a 3-way split, run here one after the other on one GPU, against the 16-head C2 call."""
+    sf, ctx, torch = env
+    from paper_2607_03612_b200 import sharding
+    L = sy.config_c2()
+    sh = L.shape
+    q, k, v = upload(L)
+    shape = c_shape(sf, sh)
+    lists = ctx.select(q, k, shape, L.cfgs)
+    out = ctx.sparse_attn(q, k, v, shape, lists)
+    torch.cuda.synchronize()
+    rp, col = lists.row_ptr.cpu().numpy(), lists.col_idx.cpu().numpy()
+    costs = sharding.head_costs(shape, L.cfgs)
+    for world in (2, 3):
+        parts = sharding.assign_heads(costs, world)
+        assert sorted(h for p in parts for h in p) == list(range(sh.H))
+        for mine in parts:
+            sub_shape = sf.make_shape(sh.S, sh.T, len(mine), sh.D, sh.B)
+            qs, ks, vs = (x[mine].contiguous() for x in (q, k, v))
+            cfgs = [L.cfgs[h] for h in mine]
+            sl = ctx.select(qs, ks, sub_shape, cfgs)
+            so = ctx.sparse_attn(qs, ks, vs, sub_shape, sl)
+            torch.cuda.synchronize()
+            srp, scol = sl.row_ptr.cpu().numpy(), sl.col_idx.cpu().numpy()
+            assert srp[-1] * 4 * sh.B * sh.B * sh.D == sum(costs[h] for h in mine)
+            for n, h in enumerate(mine):
+                a = rp[h * sh.NB:(h + 1) * sh.NB + 1]
+                b = srp[n * sh.NB:(n + 1) * sh.NB + 1]
+                assert np.array_equal(a - a[0], b - b[0]) and np.array_equal(col[a[0]:a[-1]], scol[b[0]:b[-1]]), f"head {h}: lists differ"
+                assert torch.equal(so[n], out[h]), f"head {h}: output differs between the split and the whole layer"
+
+
+def test_bench_head_parallel_mode_prints_a_strong_scaling_line():
+    """python bench.py --shard heads at N = 1 (the mode the driver can run on this box): exits 0 and prints one JSON line with
+    scaling "strong", every head on rank 0, three launches per step."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--shard", "heads", "--config", "c2", "--steps", "4", "--warmup", "3"],
+                       capture_output=True, text=True, timeout=600, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    d = json.loads(r.stdout.strip().splitlines()[-1])
+    assert d["scaling"] == "strong" and d["n_gpus"] == 1 and d["heads_by_rank"] == [list(range(16))]
+    assert d["gpu_launches"] == 3 * 4 and d["lpt_imbalance_max_over_mean"] == 1.0
+    assert 0.3 < d["value"] < 5.0 and d["metric"] == "global_attn_layer_ms"

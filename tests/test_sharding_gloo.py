@@ -32,7 +32,11 @@ def _worker(rank: int, world: int, port: int, q):
         gathered = [None] * world
         dist.all_gather_object(gathered, {"heads": mine, "costs": costs, "layers": sharding.layers_for_rank(24, rank, world)})
         slowest = sharding.max_over_ranks(10.0 + rank)          # rank r "took" 10 + r ms
-        q.put((rank, gathered, slowest, sum(costs[h] for h in mine)))
+        # the head-parallel split end to end on the host side (bench.py --shard heads): the sub-layer this rank would run
+        sub_shape = sf.make_shape(sh.S, sh.T, len(mine), sh.D, sh.B)
+        sub_entries, sub_ws = sf.query_sizes(sub_shape, [cfgs[h] for h in mine])
+        full_entries, _ = sf.query_sizes(shape, cfgs)
+        q.put((rank, gathered, slowest, sum(costs[h] for h in mine), sub_entries, full_entries, sub_ws))
     finally:
         dist.destroy_process_group()
 
@@ -59,6 +63,11 @@ def test_two_rank_partition_and_timing_reduction():
     assert res[0][2] == res[1][2] == 11.0                        # max over ranks
     loads = [res[0][3], res[1][3]]
     assert max(loads) <= 0.5 * sum(loads) + max(g0[0]["costs"])  # LPT bound: within one head of the even split
+    # the two sub-layers list exactly the block pairs of the whole layer, and each rank's executed FLOP is 4*B^2*D per listed pair
+    assert res[0][4] + res[1][4] == res[0][5] == res[1][5]
+    sh = sy.shape_c2()
+    assert [r[4] * 4 * sh.B * sh.B * sh.D for r in res] == loads
+    assert res[0][6] > 0 and res[1][6] > 0
 
 
 def test_assign_heads_properties():
